@@ -1,0 +1,63 @@
+"""Seeded problem instances: the five BASELINE.json configs and tiny pin cases."""
+import numpy as np
+
+from .blocking import build_block
+from .integrals import make_integrals
+from .store import assemble, block_values_from_rblocks, sectors_of
+from .terms import Partition, TermTable
+
+
+def random_psi(n, seed):
+    rng = np.random.Generator(np.random.Philox(seed))
+    x = rng.standard_normal(n)
+    return x / np.linalg.norm(x)
+
+
+def make_blocked_problem(K, nL, N_tot, twoSz_tot=0, D=None, seed=1, banded=False, rotate=False,
+                         force_dmax=True, track=False, ints=None):
+    """Honest blocking (cfg 1-2, tiny pins): L = orbitals [0,nL), dots nL, nL+1, R = the rest."""
+    ints = ints if ints is not None else make_integrals(K, seed, banded=banded)
+    part = Partition(K, nL)
+    rng = np.random.Generator(np.random.Philox(seed + 7919))
+    bL = build_block("L", range(0, nL), ints, K, N_tot, twoSz_tot, D, rng, rotate, force_dmax, track)
+    bR = build_block("R", range(nL + 2, K), ints, K, N_tot, twoSz_tot, D, rng, rotate, force_dmax, track)
+    if nL == 1 or K - nL - 2 == 1:
+        # single-site end blocks keep only sectors that can reach the target
+        pass
+    tt = TermTable(part, ints)
+    pr = assemble(tt, sectors_of(bL), sectors_of(bR), block_values_from_rblocks(bL, bR, ints),
+                  N_tot, twoSz_tot)
+    pr.meta = dict(K=K, nL=nL, nR=K - nL - 2, D=D, seed=seed, mode="blocking", banded=banded)
+    pr.ints, pr.part, pr.bL, pr.bR, pr.tt = ints, part, bL, bR, tt
+    return pr
+
+
+def determinant_map(pr):
+    """For tracked tiny problems: list over psi blocks of (dets, E) with
+    psi_block = E^T-projected determinant coefficients; E = kron(E_L, E_R) per block.
+    Returns (all_dets sorted unique, P) with P the (ndet x psi_size) isometry from the
+    renormalized two-dot basis to determinants: |psi_det> = P psi."""
+    bL, bR, part = pr.bL, pr.bR, pr.part
+    c0, c1 = part.c
+    d0, d1 = part.d
+    site_bits = lambda n, a, b: (0, 1 << b, 1 << a, (1 << a) | (1 << b))[n]  # noqa: E731
+    rows, cols, vals = [], [], []
+    det_index = {}
+    for (iL, n1, n2, iR, dL, dR, off) in pr.layout:
+        EL, ER = bL.E[iL], bR.E[iR]
+        mid = site_bits(n1, c0, c1) | site_bits(n2, d0, d1)
+        M = np.kron(EL, ER)  # (nl*nr) x (dL*dR), row-major psi block index i*dR + j
+        k = 0
+        for dl in bL.dets[iL]:
+            for dr in bR.dets[iR]:
+                det = dl | mid | dr
+                di = det_index.setdefault(det, len(det_index))
+                nz = np.nonzero(M[k])[0]
+                rows += [di] * len(nz)
+                cols += list(off + nz)
+                vals += list(M[k, nz])
+                k += 1
+    dets = np.array(sorted(det_index, key=det_index.get), dtype=np.uint64)
+    P = np.zeros((len(dets), pr.psi_size))
+    P[rows, cols] = vals
+    return dets, P

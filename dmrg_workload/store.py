@@ -1,0 +1,185 @@
+"""Flat arrays handed to `dmrg_ops_load` / `dmrg_plan_create` and to the oracle.
+
+Data model (include/dmrg_sigma.h; PAPER.md:126-141 for the operator store,
+PAPER.md:95-99 for the block-sparse wavefunction):
+  sectors  int32 [nsec,3]  (N, 2Sz, dim)                       per side
+  ops      int32 [nops,8]  (side, kind, p, q, dN, d2Sz, first_block, nblocks)
+  blocks   int64 [nblk,3]  (row_sector, col_sector, offset); dense row-major
+           dim[row] x dim[col], row sector = col sector + charge
+  values   float64 [nvalues]
+  lincomb  CSR (lin_ptr, lin_op, lin_coef): op of kind LINCOMB number j is
+           sum_i lin_coef[i] * ops[lin_op[i]],  lin_ptr[j] <= i < lin_ptr[j+1]
+  site_ops float64 [nsite,16] row-major 4x4, site_parity int32 [nsite]
+  terms    (coef f64; op_l, trans_l, dot1, dot2, op_r, trans_r int32)
+"""
+import numpy as np
+
+from .conventions import SITE_Q, spin_of
+
+KIND = {"H": 0, "C": 1, "A": 2, "B": 3, "P": 4, "Q": 5, "S": 6, "LIN": 7}
+
+
+def op_charge(op):
+    """(dN, d2Sz) of a stored operator."""
+    k = op.kind
+    if k == "H":
+        return (0, 0)
+    if k == "C":
+        return (1, spin_of(op.p))
+    if k == "A":
+        return (2, spin_of(op.p) + spin_of(op.q))
+    if k == "B":
+        return (0, spin_of(op.p) - spin_of(op.q))
+    if k == "P":
+        return (-2, -spin_of(op.p) - spin_of(op.q))
+    if k == "Q":
+        return (0, spin_of(op.q) - spin_of(op.p))
+    if k == "S":
+        return (-1, -spin_of(op.p))
+    raise ValueError(k)
+
+
+class Problem:
+    """Everything one bond needs: store arrays, terms, psi layout."""
+
+    def __init__(self):
+        self.secL = self.secR = None
+        self.ops = None
+        self.blocks = None
+        self.values = None
+        self.lin_ptr = self.lin_op = self.lin_coef = None
+        self.site_ops = self.site_parity = None
+        self.term_coef = self.term_idx = None
+        self.N_tot = self.twoSz_tot = 0
+        self.layout = None
+        self.psi_size = 0
+        self.meta = {}
+
+
+def _op_sort_key(op):
+    return (0 if op.side == "L" else 1, KIND[op.kind], op.p, op.q)
+
+
+def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot):
+    """Build a Problem from a TermTable.
+
+    block_values(op, row_sector, col_sector, shape) -> ndarray or None (block absent);
+    called for every stored (non-LINCOMB) op and every charge-allowed sector pair.
+    """
+    from .sectors import psi_layout
+    from .terms import BlockOp, dot_parity
+    pr = Problem()
+    pr.N_tot, pr.twoSz_tot = N_tot, twoSz_tot
+    pr.secL = np.array(secL, dtype=np.int32).reshape(-1, 3)
+    pr.secR = np.array(secR, dtype=np.int32).reshape(-1, 3)
+    secs = {"L": secL, "R": secR}
+    sidx = {s: {(q[0], q[1]): i for i, q in enumerate(secs[s])} for s in "LR"}
+    ref = tt.referenced_ops()
+    stored = sorted([o for s in "LR" for o in ref[s] if o.kind != "LIN"], key=_op_sort_key)
+    op_id = {}
+    ops_rows, blk_rows, vals = [], [], []
+    off = 0
+    for op in stored:
+        dq = op_charge(op)
+        first = len(blk_rows)
+        sl = secs[op.side]
+        for ic, qc in enumerate(sl):
+            ir = sidx[op.side].get((qc[0] + dq[0], qc[1] + dq[1]))
+            if ir is None:
+                continue
+            shape = (sl[ir][2], qc[2])
+            m = block_values(op, ir, ic, shape)
+            if m is None:
+                continue
+            assert m.shape == shape
+            blk_rows.append((ir, ic, off))
+            vals.append(np.ascontiguousarray(m, dtype=np.float64).ravel())
+            off += shape[0] * shape[1]
+        op_id[op] = len(ops_rows)
+        ops_rows.append((0 if op.side == "L" else 1, KIND[op.kind], op.p, op.q, dq[0], dq[1],
+                         first, len(blk_rows) - first))
+    lin_ptr, lin_op, lin_coef = [0], [], []
+    for side in "LR":
+        for j, lc in enumerate(tt.lincombs[side]):
+            op = BlockOp(side, "LIN", j, -1)
+            charges = {op_charge(BlockOp(side, "C", lab, -1)) for lab, _ in lc}
+            assert len(charges) == 1, "lincomb mixes charges"
+            dq = charges.pop()
+            op_id[op] = len(ops_rows)
+            ops_rows.append((0 if side == "L" else 1, KIND["LIN"], len(lin_ptr) - 1, -1, dq[0], dq[1], 0, 0))
+            for lab, cf in lc:
+                lin_op.append(op_id[BlockOp(side, "C", lab, -1)])
+                lin_coef.append(cf)
+            lin_ptr.append(len(lin_op))
+    pr.ops = np.array(ops_rows, dtype=np.int64).reshape(-1, 8)
+    pr.blocks = np.array(blk_rows, dtype=np.int64).reshape(-1, 3)
+    pr.values = np.concatenate(vals) if vals else np.zeros(0)
+    pr.lin_ptr = np.array(lin_ptr, dtype=np.int64)
+    pr.lin_op = np.array(lin_op, dtype=np.int32)
+    pr.lin_coef = np.array(lin_coef, dtype=np.float64)
+    # site operators, deduplicated by value
+    site_index, site_ops, site_par = {}, [], []
+
+    def site_id(m):
+        key = m.tobytes()
+        if key not in site_index:
+            site_index[key] = len(site_ops)
+            site_ops.append(m.ravel().copy())
+            site_par.append(dot_parity(m))
+        return site_index[key]
+
+    site_id(np.eye(4))
+    coefs, idx = [], []
+    for coef, Ls, c, d, Rs in tt.terms:
+        ol, tl = (-1, 0) if Ls is None else (op_id[Ls[0]], int(Ls[1]))
+        orr, trr = (-1, 0) if Rs is None else (op_id[Rs[0]], int(Rs[1]))
+        coefs.append(coef)
+        idx.append((ol, tl, site_id(c), site_id(d), orr, trr))
+    pr.term_coef = np.array(coefs, dtype=np.float64)
+    pr.term_idx = np.array(idx, dtype=np.int32).reshape(-1, 6)
+    pr.site_ops = np.array(site_ops, dtype=np.float64).reshape(-1, 16)
+    pr.site_parity = np.array(site_par, dtype=np.int32)
+    pr.layout, pr.psi_size = psi_layout(secL, secR, N_tot, twoSz_tot)
+    pr.op_id = op_id
+    pr.stored_ops = stored
+    return pr
+
+
+def block_values_from_rblocks(blkL, blkR, ints):
+    """block_values callback serving honest renormalized blocks (blocking.py)."""
+    cache = {}
+
+    def get(op):
+        if op in cache:
+            return cache[op]
+        b = blkL if op.side == "L" else blkR
+        k = op.kind
+        if k == "H":
+            d = b.ops[("H",)]
+        elif k == "C":
+            d = b.ops[("C", op.p)]
+        elif k == "A":
+            d = b.ops[("A", op.p, op.q)]
+        elif k == "B":
+            d = b.ops[("B", op.p, op.q)]
+        elif k == "S":
+            d = b.ops[("S", op.p)]
+        elif k == "P":
+            d = b.compl_P(op.p, op.q, ints)
+        elif k == "Q":
+            d = b.compl_Q(op.p, op.q, ints)
+        else:
+            raise ValueError(k)
+        cache.clear()
+        cache[op] = d
+        return d
+
+    def fn(op, ir, ic, shape):
+        m = get(op).get((ir, ic))
+        return m
+
+    return fn
+
+
+def sectors_of(blk):
+    return [(q[0], q[1], d) for q, d in zip(blk.sectors, blk.dims)]
