@@ -1,0 +1,190 @@
+/*
+ * dmrg_sigma.h -- C ABI of the B200-native two-dot DMRG sigma-vector library.
+ *
+ * What it computes (arxiv/paper_2311_02854; line numbers are /root/reference/PAPER.md):
+ *   sigma = H psi in the two-dot product space V_L x V_C1 x V_C2 x V_R, with H written as a
+ *   sum of O(K^2) operator products  H = sum_mu O^L_mu O^C1_mu O^C2_mu O^R_mu   (Eq. 5),
+ *     sigma[l'c1'c2'r'] = sum_mu sum_{l c1 c2 r} zeta [O^L]_{l'l} [O^C1]_{c1'c1} [O^C2]_{c2'c2}
+ *                         [O^R]_{r'r} psi[l c1 c2 r]                               (Eq. 7)
+ *   evaluated block by block over U(1)_N x U(1)_Sz symmetry sectors as
+ *     X          = psi_blk * (O^R_blk)^T                                          (Eq. 11)
+ *     sigma_blk += (c_mu zeta o1 o2) * O^L_blk * X                                (Eqs. 12-13)
+ *   the dot factors being numbers for N,Sz symmetry, and called repeatedly by a
+ *   Davidson eigensolver.
+ *
+ * Conventions:
+ *   - All floating point data are IEEE FP64.  All matrices are dense ROW-MAJOR.
+ *   - A sector is (N, 2Sz, dim).  An operator block O[row_sector, col_sector] is a
+ *     dim[row] x dim[col] matrix; row sector = col sector + (dn, d2sz) of the operator.
+ *   - Site (dot) basis: 0 vac, 1 beta, 2 alpha, 3 alpha-beta, (N,2Sz) = (0,0),(1,-1),(1,1),(2,0)
+ *     (PAPER.md:49).
+ *   - psi/sigma block (iL, c1, c2, iR) exists iff the four (N,2Sz) add up to the target; it is a
+ *     dense row-major dim_L[iL] x dim_R[iR] matrix ("C order").  Blocks are stored
+ *     back to back, sorted by (iR, c1, c2, iL), so all blocks sharing iR form one contiguous
+ *     row panel.  dmrg_plan_psi_layout returns the table.
+ *   - zeta = (-1)^{ p_C1 N_l + p_C2 (N_l+N_c1) + p_R (N_l+N_c1+N_c2) } with p_X the parity of the
+ *     factor in slot X and N_x the particle numbers of the INPUT (ket) block (PAPER.md:73 names
+ *     zeta without a formula; reading 3).
+ *
+ * Error behaviour: every int-returning entry point returns 0 on success and a negative
+ * DMRG_E* code otherwise; dmrg_last_error() then returns a thread-local message.  No C++
+ * exception crosses this boundary.  Nothing here falls back to a CPU path: without a CUDA
+ * device every call that needs one fails with DMRG_ECUDA.
+ *
+ * Pointer kinds are stated per argument: [host] or [device].
+ */
+#ifndef DMRG_SIGMA_H
+#define DMRG_SIGMA_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DMRG_OK        0
+#define DMRG_EINVAL   (-1)   /* bad argument / inconsistent tables            */
+#define DMRG_ECHARGE  (-2)   /* a term does not conserve (N, 2Sz)              */
+#define DMRG_ENOMEM   (-3)   /* host or device allocation failed               */
+#define DMRG_ECUDA    (-4)   /* CUDA runtime error (text in dmrg_last_error)   */
+#define DMRG_ENOCONV  (-5)   /* dmrg_davidson hit max_iter (outputs are valid) */
+
+/* operator kinds, Eq. (19): {a+_p, A_pq, B_ps, P_pq, Q_ps, S_p, H}; LINCOMB is a
+ * linear combination of one-index operators (the paper's "intermediates"). */
+enum { DMRG_OP_H = 0, DMRG_OP_CRE = 1, DMRG_OP_A = 2, DMRG_OP_B = 3, DMRG_OP_P = 4, DMRG_OP_Q = 5,
+       DMRG_OP_S = 6, DMRG_OP_LINCOMB = 7 };
+
+typedef struct { int32_t n, two_sz, dim; } dmrg_sector;
+
+typedef struct {
+    int32_t side;         /* 0 = L, 1 = R                                                          */
+    int32_t kind;         /* DMRG_OP_*; informational except DMRG_OP_LINCOMB                        */
+    int32_t p, q;         /* spin-orbital labels (-1 unused); for LINCOMB p = row of lin_ptr        */
+    int32_t dn, d2sz;     /* charge: row sector = col sector + (dn, d2sz); parity = dn & 1          */
+    int64_t first_block;  /* index into blocks[]; ignored for LINCOMB                                */
+    int32_t nblocks;      /* number of stored (non-zero) blocks; ignored for LINCOMB                 */
+    int32_t reserved;
+} dmrg_op_desc;
+
+typedef struct { int32_t row_sector, col_sector; int64_t offset; } dmrg_block_desc; /* offset into values[] */
+
+typedef struct {
+    double  coef;            /* integral-derived coefficient c_mu                                   */
+    int32_t op_l, trans_l;   /* operator id or -1 = identity; trans != 0 uses every block transposed */
+    int32_t dot1, dot2;      /* ids into site_ops[]                                                  */
+    int32_t op_r, trans_r;
+} dmrg_term;
+
+typedef struct { int32_t il, c1, c2, ir, dl, dr; int64_t offset; } dmrg_psi_block;
+
+typedef struct dmrg_ops  dmrg_ops;    /* block-sparse operator store resident in HBM */
+typedef struct dmrg_plan dmrg_plan;   /* GEMM-pair plan for one bond                  */
+
+/* ---------------------------------------------------------------------------------------------
+ * dmrg_ops_load: copy the block-sparse operator store {a+, A, B, P, Q, S, H}^{L,R} (Eq. 19-24,
+ * PAPER.md:126-141, Fig. 1b "only the nonzero blocks are stored") into HBM and form the
+ * linear-combination operators O = sum_s alpha_s a_s ("intermediates") on the device.
+ *   secL/secR [host]  sector tables of the left / right renormalized basis
+ *   ops       [host]  nops descriptors; the blocks of op i are blocks[first_block .. +nblocks)
+ *   blocks    [host]  nblocks descriptors; at most one block per (op, row_sector)
+ *   values    [host] or [device] (values_on_device != 0): nvalues doubles; block b is the row-major
+ *             dim[row] x dim[col] matrix at values + blocks[b].offset.  Not retained: the store
+ *             keeps its own (row-padded) copy, the caller may free `values` on return.
+ *   lin_ptr   [host]  CSR over LINCOMB operators (nlin+1 entries); LINCOMB op with p = j is
+ *             sum_{i in [lin_ptr[j], lin_ptr[j+1])} lin_coef[i] * ops[lin_op[i]]; all summands must be
+ *             stored (non-LINCOMB) operators of the same side and charge as the LINCOMB op.
+ * Ownership: *out owns its HBM; free with dmrg_ops_free.  Synchronous.
+ */
+int dmrg_ops_load(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* secR, int32_t nsecR,
+                  const dmrg_op_desc* ops, int32_t nops,
+                  const dmrg_block_desc* blocks, int64_t nblocks,
+                  const double* values, int64_t nvalues, int32_t values_on_device,
+                  const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin,
+                  dmrg_ops** out);
+void    dmrg_ops_free(dmrg_ops* ops);
+int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store */
+
+/* ---------------------------------------------------------------------------------------------
+ * dmrg_plan_create: the "CPU preprocessing" of PAPER.md:97-99,145 -- expand every term mu and every
+ * symmetry-block combination into GEMM pairs (Eq. 14), de-duplicate and merge the X = psi R^T
+ * products, concatenate all contributions of one sigma block into one long-K GEMM in a fixed
+ * order (the deterministic Eq. 13), tile, sort by cost, and upload the descriptors.
+ *   terms      [host] nterms operator-pair terms (all four slots; identity = op -1 / site op 0..)
+ *   site_ops   [host] nsite row-major 4x4 dot matrices; site_parity[i] = fermion parity of site op i
+ *   n_total, two_sz_total: target quantum numbers of psi
+ *   workspace_bytes: HBM the plan may use for the X intermediates (0 = default 8 GiB, clamped to
+ *              what one term needs); terms are processed in chunks that fit it.
+ * Fails with DMRG_ECHARGE if a term does not conserve (N, 2Sz).  The plan borrows `ops`
+ * (which must outlive it) and owns its descriptors and workspace.  Synchronous.
+ */
+int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,
+                     const double* site_ops, const int32_t* site_parity, int32_t nsite,
+                     int32_t n_total, int32_t two_sz_total, int64_t workspace_bytes,
+                     dmrg_plan** out);
+void    dmrg_plan_destroy(dmrg_plan* plan);
+int64_t dmrg_plan_psi_size(const dmrg_plan* plan);            /* doubles in psi / sigma         */
+int64_t dmrg_plan_num_psi_blocks(const dmrg_plan* plan);
+int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host], num_psi_blocks */);
+
+/* plan statistics, all per one dmrg_sigma call.  keys:
+ *  0 tasks (term x block x dot transition)   1 algorithmic flops (2 dL dR dR' + 2 dL' dL dR' per task,
+ *    identity factors cost 0 -- the paper's cost measure, Table 1 caption PAPER.md:151)
+ *  2 executed stage-1 flops after de-duplication, unpadded    3 executed stage-2 flops, unpadded
+ *  4 executed flops including tile padding                     5 stage-1 GEMM jobs   6 chunks
+ *  7 kernel launches per sigma   8 device bytes held by the plan (descriptors + workspace)
+ *  9 algorithmic operand bytes read per sigma (operator blocks once per use + X write/read + psi/sigma)
+ * 10 stage-1 tiles   11 stage-2 tiles   12 canonical flops (= key 1 without de-duplication)        */
+double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
+
+/* ---------------------------------------------------------------------------------------------
+ * dmrg_sigma: sigma = H psi (Eq. 7).  psi, sigma [device], dmrg_plan_psi_size doubles each, must not
+ * alias; sigma is OVERWRITTEN.  Work is enqueued on `cuda_stream` (a cudaStream_t, NULL = default
+ * stream) and the call returns without synchronising.  Bitwise reproducible run to run: every
+ * sigma element is accumulated by one thread block in plan order, no floating-point atomics.
+ */
+int dmrg_sigma(dmrg_plan* plan, const double* psi, double* sigma, void* cuda_stream);
+
+/* dmrg_sigma_host: the same through HOST buffers (pageable or pinned): H2D copy of psi, dmrg_sigma,
+ * D2H copy of sigma, synchronises.  Used for the end-to-end measurement. */
+int dmrg_sigma_host(dmrg_plan* plan, const double* psi_host, double* sigma_host, void* cuda_stream);
+
+/* dmrg_hdiag: diagonal of H in the psi layout ("diagonal part of Hamiltonian"), used as
+ * the Davidson preconditioner.  diag [device], overwritten.  Asynchronous on `cuda_stream`. */
+int dmrg_hdiag(dmrg_plan* plan, double* diag, void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * dmrg_davidson: single-root Davidson (Ref. 74; parameters = DESIGN.md reading 11).
+ *   x [device] in: initial guess (any non-zero norm), out: normalised Ritz vector.
+ *   iteration k: w_k = H b_k (dmrg_sigma); G_ik = b_i.w_k; (theta, y) = lowest eigenpair of G;
+ *   x = sum y_i b_i; r = sum y_i w_i - theta x; stop if |r| <= tol; t = r den/(den^2+delta^2),
+ *   den = theta - Hd, delta = 1e-3; orthogonalise t against b_1..b_m (classical Gram-Schmidt twice),
+ *   normalise -> b_{m+1}.  At m = max_space the basis collapses to {x}.  One iteration = one H psi.
+ *   All vector work runs on the device; the host sees only O(m) scalars per iteration.
+ *   thetas [host, may be NULL] receives theta_k for k < *iters (capacity max_iter).
+ * Returns DMRG_OK if |r| <= tol, DMRG_ENOCONV if max_iter was reached (outputs still valid).
+ * Synchronises `cuda_stream`.
+ */
+int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_space, double tol,
+                  double* energy, double* resid_norm, int32_t* iters, double* thetas,
+                  void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Per-stage device timing of the most recent dmrg_sigma with timing enabled (adds CUDA events
+ * around each launch; off by default).  dmrg_plan_stage_ms synchronises and returns milliseconds:
+ * which = 0 stage 1 (Eq. 11), 1 stage 2 + reduction (Eqs. 12-13), 2 whole call. */
+int    dmrg_plan_set_timing(dmrg_plan* plan, int32_t enable);
+double dmrg_plan_stage_ms(dmrg_plan* plan, int32_t which);
+
+/* FP64 pipe micro-benchmarks used as the roofline denominator:
+ * which = 0: dependent-free DFMA stream, 1: DMMA.8x8x4 (mma.sync m8n8k4 f64) stream.
+ * Returns achieved TFLOP/s over `ms` milliseconds of back-to-back launches (>= 1 launch), or a
+ * negative DMRG_E* code. */
+double dmrg_fp64_peak_tflops(int32_t which, double ms, void* cuda_stream);
+
+const char* dmrg_last_error(void);
+const char* dmrg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DMRG_SIGMA_H */

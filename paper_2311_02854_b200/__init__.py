@@ -1,0 +1,249 @@
+"""Python binding of libdmrg_sigma.so (include/dmrg_sigma.h): argument marshalling only.
+
+Every step of the hot path (operator store, planner, sigma kernels, Davidson) runs inside the
+shared library; this module converts numpy arrays / torch tensors to the C structs and pointers.
+There is no CPU fallback: if the library has not been built, importing `lib()` raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libdmrg_sigma.so")
+
+SECTOR_DT = np.dtype([("n", "<i4"), ("two_sz", "<i4"), ("dim", "<i4")], align=True)
+OP_DT = np.dtype([("side", "<i4"), ("kind", "<i4"), ("p", "<i4"), ("q", "<i4"), ("dn", "<i4"), ("d2sz", "<i4"),
+                  ("first_block", "<i8"), ("nblocks", "<i4"), ("reserved", "<i4")], align=True)
+BLOCK_DT = np.dtype([("row_sector", "<i4"), ("col_sector", "<i4"), ("offset", "<i8")], align=True)
+TERM_DT = np.dtype([("coef", "<f8"), ("op_l", "<i4"), ("trans_l", "<i4"), ("dot1", "<i4"), ("dot2", "<i4"),
+                    ("op_r", "<i4"), ("trans_r", "<i4")], align=True)
+PSIBLK_DT = np.dtype([("il", "<i4"), ("c1", "<i4"), ("c2", "<i4"), ("ir", "<i4"), ("dl", "<i4"), ("dr", "<i4"),
+                      ("offset", "<i8")], align=True)
+assert SECTOR_DT.itemsize == 12 and OP_DT.itemsize == 40 and BLOCK_DT.itemsize == 16
+assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
+
+STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
+             "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops")
+
+EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_destroy",
+           "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",
+           "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
+           "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version")
+
+_lib = None
+
+
+class DmrgError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libdmrg_sigma error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load the CUDA library; fails loudly when it has not been built (no fallback path exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2311_02854_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+        L.dmrg_ops_load.argtypes = [vp, i32, vp, i32, vp, i32, vp, i64, vp, i64, i32, vp, vp, vp, i32, C.POINTER(vp)]
+        L.dmrg_ops_load.restype = C.c_int
+        L.dmrg_ops_free.argtypes = [vp]
+        L.dmrg_ops_free.restype = None
+        L.dmrg_ops_device_bytes.argtypes = [vp]
+        L.dmrg_ops_device_bytes.restype = i64
+        L.dmrg_plan_create.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, i64, C.POINTER(vp)]
+        L.dmrg_plan_create.restype = C.c_int
+        L.dmrg_plan_destroy.argtypes = [vp]
+        L.dmrg_plan_destroy.restype = None
+        L.dmrg_plan_psi_size.argtypes = [vp]
+        L.dmrg_plan_psi_size.restype = i64
+        L.dmrg_plan_num_psi_blocks.argtypes = [vp]
+        L.dmrg_plan_num_psi_blocks.restype = i64
+        L.dmrg_plan_psi_layout.argtypes = [vp, vp]
+        L.dmrg_plan_psi_layout.restype = C.c_int
+        L.dmrg_plan_stat.argtypes = [vp, i32]
+        L.dmrg_plan_stat.restype = f64
+        L.dmrg_sigma.argtypes = [vp, vp, vp, vp]
+        L.dmrg_sigma.restype = C.c_int
+        L.dmrg_sigma_host.argtypes = [vp, vp, vp, vp]
+        L.dmrg_sigma_host.restype = C.c_int
+        L.dmrg_hdiag.argtypes = [vp, vp, vp]
+        L.dmrg_hdiag.restype = C.c_int
+        L.dmrg_davidson.argtypes = [vp, vp, i32, i32, f64, C.POINTER(f64), C.POINTER(f64), C.POINTER(i32), vp, vp]
+        L.dmrg_davidson.restype = C.c_int
+        L.dmrg_plan_set_timing.argtypes = [vp, i32]
+        L.dmrg_plan_set_timing.restype = C.c_int
+        L.dmrg_plan_stage_ms.argtypes = [vp, i32]
+        L.dmrg_plan_stage_ms.restype = f64
+        L.dmrg_fp64_peak_tflops.argtypes = [i32, f64, vp]
+        L.dmrg_fp64_peak_tflops.restype = f64
+        L.dmrg_last_error.restype = C.c_char_p
+        L.dmrg_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(rc, allow=()):
+    if rc != 0 and rc not in allow:
+        raise DmrgError(rc, lib().dmrg_last_error().decode())
+    return rc
+
+
+def _ptr(a):
+    """Address of a numpy array (host) or of a torch tensor (device)."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        return a.ctypes.data
+    return a.data_ptr()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        return None
+    return getattr(stream, "cuda_stream", stream)
+
+
+def _structured(rows, dt, cols):
+    rows = np.asarray(rows)
+    out = np.zeros(len(rows), dtype=dt)
+    for name, c in cols:
+        out[name] = rows[:, c]
+    return out
+
+
+class OpsStore:
+    """dmrg_ops_load: block-sparse operator store resident in HBM."""
+
+    def __init__(self, secL, secR, ops, blocks, values, lin_ptr, lin_op, lin_coef):
+        """secL/secR: int [n,3] (N, 2Sz, dim); ops: int [nops,8] (side, kind, p, q, dN, d2Sz, first_block,
+        nblocks); blocks: int [nblk,3] (row_sector, col_sector, offset); values: float64 numpy array (host)
+        or CUDA torch tensor (device); lincomb CSR as in dmrg_sigma.h."""
+        self._h = None
+        sl = _structured(np.asarray(secL).reshape(-1, 3), SECTOR_DT, (("n", 0), ("two_sz", 1), ("dim", 2)))
+        sr = _structured(np.asarray(secR).reshape(-1, 3), SECTOR_DT, (("n", 0), ("two_sz", 1), ("dim", 2)))
+        od = _structured(np.asarray(ops).reshape(-1, 8), OP_DT, (("side", 0), ("kind", 1), ("p", 2), ("q", 3), ("dn", 4),
+                                                                  ("d2sz", 5), ("first_block", 6), ("nblocks", 7)))
+        bd = _structured(np.asarray(blocks).reshape(-1, 3), BLOCK_DT, (("row_sector", 0), ("col_sector", 1), ("offset", 2)))
+        on_dev = 0
+        if isinstance(values, np.ndarray):
+            values = np.ascontiguousarray(values, dtype=np.float64)
+        else:
+            assert values.is_cuda and values.is_contiguous() and values.element_size() == 8
+            on_dev = 1
+        lp = np.ascontiguousarray(lin_ptr, dtype=np.int64)
+        lo = np.ascontiguousarray(lin_op, dtype=np.int32)
+        lc = np.ascontiguousarray(lin_coef, dtype=np.float64)
+        nvalues = int(values.size if on_dev == 0 else values.numel())
+        h = C.c_void_p()
+        _check(lib().dmrg_ops_load(_ptr(sl), len(sl), _ptr(sr), len(sr), _ptr(od), len(od), _ptr(bd), len(bd),
+                                   _ptr(values), nvalues, on_dev, _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1, C.byref(h)))
+        self._h = h
+
+    @property
+    def device_bytes(self):
+        return int(lib().dmrg_ops_device_bytes(self._h))
+
+    def free(self):
+        if self._h is not None:
+            lib().dmrg_ops_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
+
+
+class Plan:
+    """dmrg_plan_create and the calls that take a plan (dmrg_sigma, dmrg_hdiag, dmrg_davidson)."""
+
+    def __init__(self, ops, term_coef, term_idx, site_ops, site_parity, n_total, two_sz_total, workspace_bytes=0):
+        """term_idx: int [nterms,6] (op_l, trans_l, dot1, dot2, op_r, trans_r)."""
+        self._h = None
+        self.ops = ops   # keep the store alive: the plan borrows it
+        ti = np.asarray(term_idx).reshape(-1, 6)
+        td = np.zeros(len(ti), dtype=TERM_DT)
+        td["coef"] = np.asarray(term_coef, dtype=np.float64)
+        for name, c in (("op_l", 0), ("trans_l", 1), ("dot1", 2), ("dot2", 3), ("op_r", 4), ("trans_r", 5)):
+            td[name] = ti[:, c]
+        so = np.ascontiguousarray(site_ops, dtype=np.float64).reshape(-1, 16)
+        sp = np.ascontiguousarray(site_parity, dtype=np.int32)
+        h = C.c_void_p()
+        _check(lib().dmrg_plan_create(ops._h, _ptr(td), len(td), _ptr(so), _ptr(sp), len(so), int(n_total),
+                                      int(two_sz_total), int(workspace_bytes), C.byref(h)))
+        self._h = h
+
+    @property
+    def psi_size(self):
+        return int(lib().dmrg_plan_psi_size(self._h))
+
+    def psi_layout(self):
+        """int64 [nblk,7]: (iL, c1, c2, iR, dL, dR, offset)."""
+        n = int(lib().dmrg_plan_num_psi_blocks(self._h))
+        out = np.zeros(n, dtype=PSIBLK_DT)
+        _check(lib().dmrg_plan_psi_layout(self._h, _ptr(out)))
+        return np.stack([out[k].astype(np.int64) for k in ("il", "c1", "c2", "ir", "dl", "dr", "offset")], axis=1)
+
+    def stats(self):
+        return {k: float(lib().dmrg_plan_stat(self._h, i)) for i, k in enumerate(STAT_KEYS)}
+
+    def sigma(self, psi, sigma, stream=None):
+        """sigma = H psi; psi, sigma: CUDA float64 tensors (device pointers), asynchronous on `stream`."""
+        _check(lib().dmrg_sigma(self._h, _ptr(psi), _ptr(sigma), _stream_ptr(stream)))
+
+    def sigma_host(self, psi, sigma, stream=None):
+        """The same through host numpy buffers (H2D + sigma + D2H, synchronous)."""
+        assert isinstance(psi, np.ndarray) and isinstance(sigma, np.ndarray)
+        assert psi.dtype == np.float64 and sigma.dtype == np.float64 and psi.flags.c_contiguous and sigma.flags.c_contiguous
+        _check(lib().dmrg_sigma_host(self._h, _ptr(psi), _ptr(sigma), _stream_ptr(stream)))
+
+    def hdiag(self, diag, stream=None):
+        _check(lib().dmrg_hdiag(self._h, _ptr(diag), _stream_ptr(stream)))
+
+    def davidson(self, x, max_iter, max_space, tol, stream=None):
+        """x: CUDA float64 tensor, in: guess, out: Ritz vector.  Returns dict(energy, resid, iters, thetas, converged)."""
+        e, r, it = C.c_double(), C.c_double(), C.c_int32()
+        thetas = np.zeros(max_iter)
+        rc = _check(lib().dmrg_davidson(self._h, _ptr(x), int(max_iter), int(max_space), float(tol), C.byref(e), C.byref(r),
+                                        C.byref(it), _ptr(thetas), _stream_ptr(stream)), allow=(-5,))
+        return {"energy": e.value, "resid": r.value, "iters": it.value, "thetas": thetas[:it.value].copy(),
+                "converged": rc == 0}
+
+    def set_timing(self, enable):
+        _check(lib().dmrg_plan_set_timing(self._h, 1 if enable else 0))
+
+    def stage_ms(self):
+        return tuple(float(lib().dmrg_plan_stage_ms(self._h, k)) for k in (0, 1, 2))
+
+    def destroy(self):
+        if self._h is not None:
+            lib().dmrg_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def fp64_peak_tflops(which, ms=200.0, stream=None):
+    """Measured FP64 pipe peak: which = 0 DFMA, 1 DMMA.8x8x4."""
+    v = float(lib().dmrg_fp64_peak_tflops(int(which), float(ms), _stream_ptr(stream)))
+    if v < 0:
+        raise DmrgError(int(v), lib().dmrg_last_error().decode())
+    return v
+
+
+def load_problem(pr, workspace_bytes=0, values=None):
+    """Convenience: OpsStore + Plan from a dmrg_workload Problem (array formats of dmrg_workload/store.py)."""
+    ops = OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks, pr.values if values is None else values,
+                   pr.lin_ptr, pr.lin_op, pr.lin_coef)
+    plan = Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, workspace_bytes)
+    return ops, plan

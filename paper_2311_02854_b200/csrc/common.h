@@ -1,0 +1,108 @@
+// Internal definitions shared by the translation units of libdmrg_sigma.so (not part of the ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/dmrg_sigma.h"
+
+namespace dmrg {
+
+void set_error(const char* fmt, ...);
+
+#define DMRG_CUDA(call)                                                                          \
+    do {                                                                                         \
+        cudaError_t e_ = (call);                                                                 \
+        if (e_ != cudaSuccess) {                                                                 \
+            dmrg::set_error("%s:%d: %s -> %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? DMRG_ENOMEM : DMRG_ECUDA;                 \
+        }                                                                                        \
+    } while (0)
+
+#define DMRG_REQUIRE(cond, ...)               \
+    do {                                      \
+        if (!(cond)) {                        \
+            dmrg::set_error(__VA_ARGS__);     \
+            return DMRG_EINVAL;               \
+        }                                     \
+    } while (0)
+
+static inline int64_t round_up2(int64_t x) { return (x + 1) & ~int64_t(1); }
+
+// ---- address spaces of GEMM operands -------------------------------------------------------
+enum Space : uint32_t { SP_OPS = 0, SP_X = 1, SP_PSI = 2, SP_SIGMA = 3 };
+
+// Segment flags
+enum : uint32_t {
+    SEG_A_MCONTIG = 1u << 0,   // A(m,k) at a_off + k*lda + m   (operator block used transposed)
+    SEG_B_KCONTIG = 1u << 1,   // B(k,n) at b_off + n*ldb + k   (X = psi * O^T with O stored [n][k])
+    SEG_A_IDENT   = 1u << 2,   // A is the identity: acc += alpha * B tile (no GEMM)
+    SEG_A_VEC2    = 1u << 3,   // A operand 16-byte loadable (even offset, even ld)
+    SEG_B_VEC2    = 1u << 4,
+    SEG_A_SPACE_SHIFT = 8,     // 2 bits
+    SEG_B_SPACE_SHIFT = 10,    // 2 bits
+};
+
+// One K-segment of a grouped GEMM job:  C += alpha * A(M x K) * B(K x N)
+struct Seg {
+    int64_t  a_off;
+    int64_t  b_off;
+    int32_t  lda, ldb;
+    int32_t  K;
+    uint32_t flags;
+    double   alpha;
+};
+static_assert(sizeof(Seg) == 40, "Seg layout");
+
+enum : uint32_t { JOB_BETA1 = 1u << 0, JOB_C_SPACE_SHIFT = 8 };
+
+// One output matrix: C (M x N, row-major, ldc) = beta*C + sum over segments
+struct Job {
+    int64_t  c_off;
+    int32_t  ldc, M, N;
+    int32_t  seg_begin, seg_end;
+    uint32_t flags;
+    int32_t  pad_;
+};
+static_assert(sizeof(Job) == 40, "Job layout");
+
+// One CTA of work: tile (tm, tn) of job, tile shape fixed by the kernel variant
+struct Tile {
+    int32_t  job;
+    uint16_t tm, tn;
+};
+static_assert(sizeof(Tile) == 8, "Tile layout");
+
+// tile-shape variants of the grouped GEMM kernel
+struct TileShape { int bm, bn; };
+constexpr int NUM_VARIANTS = 4;
+extern const TileShape kVariants[NUM_VARIANTS];
+constexpr int GEMM_BK = 16;
+
+struct GemmLaunch {       // one launch of one kernel variant
+    int     variant;
+    int64_t tile_begin;   // into the plan's device tile array
+    int64_t ntiles;
+};
+
+int launch_grouped_gemm(int variant, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+                        const double* ops, double* xws, const double* psi, double* sigma, cudaStream_t st);
+int gemm_init();   // sets shared-memory attributes once
+
+}  // namespace dmrg
+
+// ---- the operator store ---------------------------------------------------------------------
+struct dmrg_ops {
+    std::vector<dmrg_sector> sec[2];
+    std::vector<dmrg_op_desc> ops;
+    // per op, per ROW sector: device offset of the block (doubles) or -1; the column sector that the
+    // charge implies (or -1); all blocks are row-major with leading dimension round_up2(dim[col]).
+    std::vector<std::vector<int64_t>> row_off;
+    std::vector<std::vector<int32_t>> colsec;
+    double* d_values = nullptr;
+    int64_t nvalues_dev = 0;     // doubles allocated (stored + lincomb, padded)
+    int64_t device_bytes = 0;
+};

@@ -1,0 +1,580 @@
+// dmrg_plan_create / dmrg_sigma / dmrg_hdiag.
+//
+// The planner is the paper's "CPU preprocessing": every term mu of Eq. (5) and every
+// combination of symmetry blocks becomes a GEMM pair (Eq. 14).  Differences from the paper's design
+// (cublasDgemmBatched per equal-shape group on many streams), chosen for one B200:
+//   * stage-1 products X = psi_blk * (O^R_blk)^T are de-duplicated (X depends only on the R block and
+//     the psi block, and one-index R operators recur in many terms) and, because psi is laid out
+//     with all blocks of one R sector back to back, consecutive psi blocks are merged into one tall
+//     GEMM per R block;
+//   * all contributions to one sigma block are concatenated along K into ONE GEMM whose K-loop walks
+//     the (term, input block) pairs in a fixed order -- this is Eq. (13) without a separate reduction
+//     kernel and without atomics;
+//   * no grouping by equal shape: a single kernel walks a cost-sorted tile list with per-tile shapes.
+// Terms are processed in chunks sized so the X intermediates fit the workspace.
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include <unordered_map>
+
+#include "plan.h"
+
+namespace dmrg {
+
+static const int SITE_N[4] = {0, 1, 1, 2};
+static const int SITE_S[4] = {0, -1, 1, 0};
+
+// relative efficiency guesses of the tile variants (used only to pick a variant per job)
+static const double kVariantEff[NUM_VARIANTS] = {1.00, 1.04, 0.80, 0.45};
+
+struct Task {
+    int32_t term_ord, in_blk, out_blk;
+    int32_t l_trans, r_trans;
+    int32_t dLi, dLo, dRi, dRo;
+    int64_t l_off, r_off;   // device offsets of the operator blocks, -1 = identity
+    double alpha;
+};
+
+struct XLoc { int64_t off; int32_t ld; };
+
+static inline int64_t xkey(int64_t r_off, int r_trans, int in_blk, int64_t nblk) {
+    return (r_off * 2 + r_trans) * nblk + in_blk;
+}
+
+static int choose_variant(int M, int N) {
+    int best = 0;
+    double bc = 1e300;
+    for (int v = 0; v < NUM_VARIANTS; v++) {
+        const double bm = kVariants[v].bm, bn = kVariants[v].bn;
+        const double c = std::ceil(M / bm) * std::ceil(N / bn) * bm * bn / kVariantEff[v];
+        if (c < bc) { bc = c; best = v; }
+    }
+    return best;
+}
+
+struct TileRec { Tile t; double cost; };
+
+static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
+                      const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
+                      int64_t workspace_bytes) {
+    const dmrg_ops* S = P->ops;
+    const auto& secL = S->sec[0];
+    const auto& secR = S->sec[1];
+    const int nL = (int)secL.size(), nR = (int)secR.size();
+    const int nops = (int)S->ops.size();
+
+    // ---- psi block table, sorted by (iR, c1, c2, iL) -- each block dense row-major dL x dR --------
+    std::vector<int32_t> lut((size_t)nL * 16 * nR, -1);
+    {
+        int64_t off = 0;
+        for (int iR = 0; iR < nR; iR++)
+            for (int c1 = 0; c1 < 4; c1++)
+                for (int c2 = 0; c2 < 4; c2++) {
+                    const int NL = n_total - secR[iR].n - SITE_N[c1] - SITE_N[c2];
+                    const int SL = two_sz_total - secR[iR].two_sz - SITE_S[c1] - SITE_S[c2];
+                    for (int iL = 0; iL < nL; iL++)
+                        if (secL[iL].n == NL && secL[iL].two_sz == SL) {
+                            lut[(((size_t)iL * 4 + c1) * 4 + c2) * nR + iR] = (int32_t)P->blocks.size();
+                            P->blocks.push_back({iL, c1, c2, iR, secL[iL].dim, secR[iR].dim, off});
+                            off += (int64_t)secL[iL].dim * secR[iR].dim;
+                            break;
+                        }
+                }
+        P->psi_size = off;
+    }
+    const int64_t nblk = (int64_t)P->blocks.size();
+    DMRG_REQUIRE(nblk > 0, "dmrg_plan_create: no psi block has the target quantum numbers (%d, %d)", n_total, two_sz_total);
+
+    // ---- per-op inverse sector map: rowof[op][c] = row sector r with colsec[r] == c ----------------
+    std::vector<std::vector<int32_t>> rowof(nops);
+    for (int o = 0; o < nops; o++) {
+        const int ns = (int)S->colsec[o].size();
+        rowof[o].assign(ns, -1);
+        for (int r = 0; r < ns; r++)
+            if (S->colsec[o][r] >= 0) rowof[o][S->colsec[o][r]] = r;
+    }
+
+    // ---- validate terms, order them so that terms sharing an R operator are adjacent ------------
+    for (int64_t t = 0; t < nterms; t++) {
+        const dmrg_term& T = terms[t];
+        DMRG_REQUIRE(T.op_l >= -1 && T.op_l < nops && T.op_r >= -1 && T.op_r < nops, "dmrg_plan_create: term %lld: operator id out of range", (long long)t);
+        DMRG_REQUIRE(T.op_l < 0 || S->ops[T.op_l].side == 0, "dmrg_plan_create: term %lld: op_l is not a left-block operator", (long long)t);
+        DMRG_REQUIRE(T.op_r < 0 || S->ops[T.op_r].side == 1, "dmrg_plan_create: term %lld: op_r is not a right-block operator", (long long)t);
+        DMRG_REQUIRE(T.dot1 >= 0 && T.dot1 < nsite && T.dot2 >= 0 && T.dot2 < nsite, "dmrg_plan_create: term %lld: site operator id out of range", (long long)t);
+        int dn = 0, ds = 0;
+        if (T.op_l >= 0) { const int s = T.trans_l ? -1 : 1; dn += s * S->ops[T.op_l].dn; ds += s * S->ops[T.op_l].d2sz; }
+        if (T.op_r >= 0) { const int s = T.trans_r ? -1 : 1; dn += s * S->ops[T.op_r].dn; ds += s * S->ops[T.op_r].d2sz; }
+        const double* o1 = site_ops + 16 * (size_t)T.dot1;
+        const double* o2 = site_ops + 16 * (size_t)T.dot2;
+        for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) {
+            if (o1[4 * a + b] == 0.0) continue;
+            for (int c = 0; c < 4; c++) for (int d = 0; d < 4; d++) {
+                if (o2[4 * c + d] == 0.0) continue;
+                const int tn = dn + SITE_N[a] - SITE_N[b] + SITE_N[c] - SITE_N[d];
+                const int ts = ds + SITE_S[a] - SITE_S[b] + SITE_S[c] - SITE_S[d];
+                if (tn != 0 || ts != 0) {
+                    set_error("dmrg_plan_create: term %lld does not conserve (N, 2Sz): residual (%d, %d)", (long long)t, tn, ts);
+                    return DMRG_ECHARGE;
+                }
+            }
+        }
+    }
+    std::vector<int64_t> order(nterms);
+    for (int64_t t = 0; t < nterms; t++) order[t] = t;
+    std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
+        const dmrg_term &A = terms[a], &B = terms[b];
+        if (A.op_r != B.op_r) return A.op_r < B.op_r;
+        if ((A.trans_r != 0) != (B.trans_r != 0)) return A.trans_r == 0;
+        return false;
+    });
+
+    // ---- enumerate tasks: (term, psi block, dot transition)  (Eq. 7 at the level of blocks) ------
+    std::vector<Task> tasks;
+    std::vector<int64_t> term_task_begin(nterms + 1, 0);
+    double canon_flops = 0.0;
+    for (int64_t to = 0; to < nterms; to++) {
+        const dmrg_term& T = terms[order[to]];
+        term_task_begin[to] = (int64_t)tasks.size();
+        const double* o1 = site_ops + 16 * (size_t)T.dot1;
+        const double* o2 = site_ops + 16 * (size_t)T.dot2;
+        const int p1 = site_parity[T.dot1] & 1, p2 = site_parity[T.dot2] & 1;
+        const int pR = T.op_r >= 0 ? (S->ops[T.op_r].dn & 1) : 0;
+        for (int64_t b = 0; b < nblk; b++) {
+            const dmrg_psi_block& B = P->blocks[b];
+            int iLo = B.il, iRo = B.ir;
+            int64_t l_off = -1, r_off = -1;
+            if (T.op_l >= 0) {
+                if (!T.trans_l) { iLo = rowof[T.op_l][B.il]; if (iLo < 0) continue; l_off = S->row_off[T.op_l][iLo]; }
+                else { l_off = S->row_off[T.op_l][B.il]; iLo = S->colsec[T.op_l][B.il]; }
+                if (l_off < 0 || iLo < 0) continue;
+            }
+            if (T.op_r >= 0) {
+                if (!T.trans_r) { iRo = rowof[T.op_r][B.ir]; if (iRo < 0) continue; r_off = S->row_off[T.op_r][iRo]; }
+                else { r_off = S->row_off[T.op_r][B.ir]; iRo = S->colsec[T.op_r][B.ir]; }
+                if (r_off < 0 || iRo < 0) continue;
+            }
+            const int Nl = secL[B.il].n;
+            const int zexp = p1 * Nl + p2 * (Nl + SITE_N[B.c1]) + pR * (Nl + SITE_N[B.c1] + SITE_N[B.c2]);
+            const double zeta = (zexp & 1) ? -1.0 : 1.0;
+            for (int c1o = 0; c1o < 4; c1o++) {
+                const double v1 = o1[4 * c1o + B.c1];
+                if (v1 == 0.0) continue;
+                for (int c2o = 0; c2o < 4; c2o++) {
+                    const double v2 = o2[4 * c2o + B.c2];
+                    if (v2 == 0.0) continue;
+                    const int32_t ob = lut[(((size_t)iLo * 4 + c1o) * 4 + c2o) * nR + iRo];
+                    if (ob < 0) continue;
+                    Task k;
+                    k.term_ord = (int32_t)to; k.in_blk = (int32_t)b; k.out_blk = ob;
+                    k.l_trans = T.trans_l != 0; k.r_trans = T.trans_r != 0;
+                    k.dLi = B.dl; k.dRi = B.dr; k.dLo = secL[iLo].dim; k.dRo = secR[iRo].dim;
+                    k.l_off = l_off; k.r_off = r_off;
+                    k.alpha = T.coef * zeta * v1 * v2;
+                    tasks.push_back(k);
+                    if (r_off >= 0) canon_flops += 2.0 * k.dLi * k.dRi * k.dRo;
+                    if (l_off >= 0) canon_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                }
+            }
+        }
+    }
+    term_task_begin[nterms] = (int64_t)tasks.size();
+    P->stats[ST_TASKS] = (double)tasks.size();
+    P->stats[ST_CANON_FLOPS] = canon_flops;
+
+    // ---- chunk the (ordered) terms by X workspace --------------------------------------------------
+    auto x_elems = [](const Task& k) { return (int64_t)k.dLi * round_up2(k.dRo); };
+    int64_t ws_elems = (workspace_bytes > 0 ? workspace_bytes : (int64_t(8) << 30)) / 8;
+    {
+        int64_t max_term = 0;
+        std::unordered_map<int64_t, char> seen;
+        for (int64_t to = 0; to < nterms; to++) {
+            seen.clear();
+            int64_t need = 0;
+            for (int64_t i = term_task_begin[to]; i < term_task_begin[to + 1]; i++) {
+                const Task& k = tasks[i];
+                if (k.r_off < 0) continue;
+                if (seen.emplace(xkey(k.r_off, k.r_trans, k.in_blk, nblk), 1).second) need += x_elems(k);
+            }
+            max_term = std::max(max_term, need);
+        }
+        ws_elems = std::max<int64_t>(std::max(ws_elems, max_term), 2);
+    }
+    std::vector<int64_t> chunk_begin;   // term_ord of the first term of each chunk
+    {
+        std::unordered_map<int64_t, char> seen;
+        int64_t used = 0;
+        chunk_begin.push_back(0);
+        for (int64_t to = 0; to < nterms; to++) {
+            int64_t add = 0;
+            std::vector<int64_t> newkeys;
+            for (int64_t i = term_task_begin[to]; i < term_task_begin[to + 1]; i++) {
+                const Task& k = tasks[i];
+                if (k.r_off < 0) continue;
+                const int64_t key = xkey(k.r_off, k.r_trans, k.in_blk, nblk);
+                if (seen.emplace(key, 1).second) { add += x_elems(k); newkeys.push_back(key); }
+            }
+            if (used + add > ws_elems && to > chunk_begin.back()) {
+                chunk_begin.push_back(to);
+                seen.clear();
+                used = 0;
+                add = 0;
+                for (int64_t i = term_task_begin[to]; i < term_task_begin[to + 1]; i++) {
+                    const Task& k = tasks[i];
+                    if (k.r_off < 0) continue;
+                    if (seen.emplace(xkey(k.r_off, k.r_trans, k.in_blk, nblk), 1).second) add += x_elems(k);
+                }
+            }
+            used += add;
+        }
+    }
+    const int64_t nchunks = nterms > 0 ? (int64_t)chunk_begin.size() : 0;
+    chunk_begin.push_back(nterms);
+    P->stats[ST_CHUNKS] = (double)nchunks;
+
+    // ---- build jobs / segments / tiles chunk by chunk ---------------------------------------------
+    std::vector<Job> jobs;
+    std::vector<Seg> segs;
+    std::vector<Tile> tiles;
+    std::vector<std::vector<HdItem>> hd(nblk);
+    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0;
+    int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
+
+    auto psi_vec2 = [&](const dmrg_psi_block& B) { return (B.offset % 2 == 0) && (B.dr % 2 == 0); };
+
+    auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
+        for (int v = 0; v < NUM_VARIANTS; v++) {
+            auto& r = recs[v];
+            if (r.empty()) continue;
+            std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
+            // grid.x limit: split very long lists
+            size_t i = 0;
+            while (i < r.size()) {
+                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);
+                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n});
+                for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
+                i += n;
+            }
+            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)r.size();
+        }
+    };
+
+    for (int64_t ch = 0; ch < nchunks; ch++) {
+        const int64_t t0 = term_task_begin[chunk_begin[ch]], t1 = term_task_begin[chunk_begin[ch + 1]];
+        if (t0 == t1) continue;
+        // -- stage 1: unique (R block, trans, psi block) products, merged into runs of consecutive psi blocks
+        struct XReq { int64_t r_off; int32_t r_trans, in_blk, dRo; };
+        std::vector<XReq> req;
+        {
+            std::unordered_map<int64_t, char> seen;
+            for (int64_t i = t0; i < t1; i++) {
+                const Task& k = tasks[i];
+                if (k.r_off < 0) continue;
+                if (seen.emplace(xkey(k.r_off, k.r_trans, k.in_blk, nblk), 1).second) req.push_back({k.r_off, k.r_trans, k.in_blk, k.dRo});
+            }
+        }
+        std::sort(req.begin(), req.end(), [](const XReq& a, const XReq& b) {
+            if (a.r_off != b.r_off) return a.r_off < b.r_off;
+            if (a.r_trans != b.r_trans) return a.r_trans < b.r_trans;
+            return a.in_blk < b.in_blk;
+        });
+        std::unordered_map<int64_t, XLoc> xloc;
+        xloc.reserve(req.size() * 2);
+        std::vector<TileRec> recs1[NUM_VARIANTS];
+        int64_t xtop = 0;
+        for (size_t i = 0; i < req.size();) {
+            size_t j = i + 1;
+            while (j < req.size() && req[j].r_off == req[i].r_off && req[j].r_trans == req[i].r_trans &&
+                   req[j].in_blk == req[j - 1].in_blk + 1 && P->blocks[req[j].in_blk].ir == P->blocks[req[i].in_blk].ir)
+                j++;
+            const dmrg_psi_block& B0 = P->blocks[req[i].in_blk];
+            const int dRi = B0.dr, dRo = req[i].dRo, ldx = (int)round_up2(dRo);
+            int64_t rows = 0;
+            bool v2 = psi_vec2(B0);
+            for (size_t q = i; q < j; q++) {
+                xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rows * ldx, ldx};
+                rows += P->blocks[req[q].in_blk].dl;
+            }
+            DMRG_REQUIRE(rows < (int64_t(1) << 31), "dmrg_plan_create: merged stage-1 panel too tall");
+            Seg s;
+            s.a_off = B0.offset; s.lda = dRi;
+            s.b_off = req[i].r_off; s.ldb = (int)round_up2(req[i].r_trans ? dRo : dRi);
+            s.K = dRi; s.alpha = 1.0;
+            s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | (v2 ? SEG_A_VEC2 : 0) |
+                      (req[i].r_trans ? 0 : SEG_B_KCONTIG);
+            Job jb;
+            jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = dRo;
+            jb.seg_begin = (int32_t)segs.size(); jb.seg_end = jb.seg_begin + 1;
+            jb.flags = (SP_X << JOB_C_SPACE_SHIFT);
+            jb.pad_ = (dRi + GEMM_BK - 1) / GEMM_BK;
+            segs.push_back(s);
+            const int v = choose_variant(jb.M, jb.N);
+            const int bm = kVariants[v].bm, bn = kVariants[v].bn;
+            const int ntm = (jb.M + bm - 1) / bm, ntn = (jb.N + bn - 1) / bn;
+            DMRG_REQUIRE(ntm < 65536 && ntn < 65536, "dmrg_plan_create: too many tiles in one job");
+            const double kpad4 = 4.0 * ((dRi + 3) / 4);
+            for (int a = 0; a < ntm; a++)
+                for (int b = 0; b < ntn; b++) recs1[v].push_back({{(int32_t)jobs.size(), (uint16_t)a, (uint16_t)b}, kpad4});
+            padded_flops += 2.0 * ntm * bm * ntn * bn * kpad4;
+            s1_flops += 2.0 * rows * dRi * dRo;
+            alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
+            jobs.push_back(jb);
+            s1_jobs++;
+            xtop += rows * ldx;
+            i = j;
+        }
+        ws_peak = std::max(ws_peak, xtop);
+        emit_tiles(recs1, 1);
+
+        // -- stage 2: per sigma block, the ordered list of contributions -----------------------------
+        std::vector<int64_t> idx(t1 - t0);
+        for (int64_t i = 0; i < t1 - t0; i++) idx[i] = t0 + i;
+        std::stable_sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return tasks[a].out_blk < tasks[b].out_blk; });
+        std::vector<TileRec> recs2[NUM_VARIANTS];
+        for (size_t i = 0; i < idx.size();) {
+            size_t j = i;
+            const int ob = tasks[idx[i]].out_blk;
+            while (j < idx.size() && tasks[idx[j]].out_blk == ob) j++;
+            const dmrg_psi_block& OB = P->blocks[ob];
+            Job jb;
+            jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
+            jb.seg_begin = (int32_t)segs.size();
+            jb.flags = (SP_SIGMA << JOB_C_SPACE_SHIFT) | JOB_BETA1;
+            int nst = 0;
+            double kp4 = 0;
+            for (int pass = 0; pass < 2; pass++) {   // identity-L contributions first, then the GEMM segments
+                for (size_t q = i; q < j; q++) {
+                    const Task& k = tasks[idx[q]];
+                    const bool ident = k.l_off < 0;
+                    if (ident != (pass == 0)) continue;
+                    Seg s;
+                    s.alpha = k.alpha;
+                    s.K = k.dLi;
+                    s.flags = 0;
+                    if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
+                    else {
+                        s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
+                        s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | SEG_A_VEC2 | (k.l_trans ? SEG_A_MCONTIG : 0);
+                    }
+                    if (k.r_off < 0) {
+                        const dmrg_psi_block& IB = P->blocks[k.in_blk];
+                        s.b_off = IB.offset; s.ldb = IB.dr;
+                        s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | (psi_vec2(IB) ? SEG_B_VEC2 : 0);
+                        if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
+                    } else {
+                        const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
+                        s.b_off = xl.off; s.ldb = xl.ld;
+                        s.flags |= (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
+                        alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
+                    }
+                    if (!ident) {
+                        nst += (k.dLi + GEMM_BK - 1) / GEMM_BK;
+                        kp4 += 4.0 * ((k.dLi + 3) / 4);
+                        s2_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                        alg_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                        alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
+                    }
+                    segs.push_back(s);
+                    if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
+                }
+            }
+            DMRG_REQUIRE(segs.size() < ((size_t)1 << 31), "dmrg_plan_create: segment table overflow");
+            jb.seg_end = (int32_t)segs.size();
+            jb.pad_ = nst;
+            const int v = choose_variant(jb.M, jb.N);
+            const int bm = kVariants[v].bm, bn = kVariants[v].bn;
+            const int ntm = (jb.M + bm - 1) / bm, ntn = (jb.N + bn - 1) / bn;
+            DMRG_REQUIRE(ntm < 65536 && ntn < 65536, "dmrg_plan_create: too many tiles in one job");
+            for (int a = 0; a < ntm; a++)
+                for (int b = 0; b < ntn; b++) recs2[v].push_back({{(int32_t)jobs.size(), (uint16_t)a, (uint16_t)b}, kp4 + 1.0});
+            padded_flops += 2.0 * ntm * bm * ntn * bn * kp4;
+            alg_bytes += 16.0 * OB.dl * OB.dr;
+            jobs.push_back(jb);
+            i = j;
+        }
+        emit_tiles(recs2, 2);
+    }
+    P->stats[ST_ALG_FLOPS] = alg_flops;
+    P->stats[ST_S1_FLOPS] = s1_flops;
+    P->stats[ST_S2_FLOPS] = s2_flops;
+    P->stats[ST_PADDED_FLOPS] = padded_flops;
+    P->stats[ST_S1_JOBS] = (double)s1_jobs;
+    P->stats[ST_LAUNCHES] = (double)P->launches.size();
+    P->stats[ST_ALG_BYTES] = alg_bytes + 8.0 * P->psi_size;
+    P->stats[ST_S1_TILES] = (double)s1_tiles;
+    P->stats[ST_S2_TILES] = (double)s2_tiles;
+
+    // ---- H diagonal lists (tasks with out == in) --------------------------------------
+    std::vector<HdItem> hd_items;
+    std::vector<HdBlock> hd_blocks(nblk);
+    for (int64_t b = 0; b < nblk; b++) {
+        hd_blocks[b] = {P->blocks[b].offset, P->blocks[b].dl, P->blocks[b].dr, (int32_t)hd_items.size(), 0};
+        hd_items.insert(hd_items.end(), hd[b].begin(), hd[b].end());
+        hd_blocks[b].item_end = (int32_t)hd_items.size();
+    }
+    P->n_hd_blocks = nblk;
+
+    // ---- upload ---------------------------------------------------------------------------------------
+    P->xws_elems = std::max<int64_t>(ws_peak, 2);
+    auto up = [&](void** dptr, const void* src, size_t bytes) -> int {
+        DMRG_CUDA(cudaMalloc(dptr, std::max<size_t>(bytes, 16)));
+        if (bytes) DMRG_CUDA(cudaMemcpy(*dptr, src, bytes, cudaMemcpyHostToDevice));
+        return DMRG_OK;
+    };
+    int rc;
+    if ((rc = up((void**)&P->d_jobs, jobs.data(), jobs.size() * sizeof(Job)))) return rc;
+    if ((rc = up((void**)&P->d_segs, segs.data(), segs.size() * sizeof(Seg)))) return rc;
+    if ((rc = up((void**)&P->d_tiles, tiles.data(), tiles.size() * sizeof(Tile)))) return rc;
+    if ((rc = up((void**)&P->d_hd_items, hd_items.data(), hd_items.size() * sizeof(HdItem)))) return rc;
+    if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
+    DMRG_CUDA(cudaMalloc(&P->d_xws, sizeof(double) * (size_t)P->xws_elems));
+    P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
+                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems);
+    return gemm_init();
+}
+
+// Hd[blk][i][j] = sum_items alpha * (L ? L[i][i] : 1) * (R ? R[j][j] : 1)     one thread per element
+__global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ blocks, const HdItem* __restrict__ items,
+                                                    const double* __restrict__ ops, double* __restrict__ diag) {
+    const HdBlock b = blocks[blockIdx.y];
+    const int64_t n = (int64_t)b.dl * b.dr;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / b.dr), j = (int)(e - (int64_t)i * b.dr);
+        double acc = 0.0;
+        for (int it = b.item_begin; it < b.item_end; it++) {
+            const HdItem h = items[it];
+            const double l = h.l_off >= 0 ? ops[h.l_off + (int64_t)i * h.ldl + i] : 1.0;
+            const double r = h.r_off >= 0 ? ops[h.r_off + (int64_t)j * h.ldr + j] : 1.0;
+            acc = fma(h.alpha, l * r, acc);
+        }
+        diag[b.offset + e] = acc;
+    }
+}
+
+}  // namespace dmrg
+
+using namespace dmrg;
+
+extern "C" {
+
+int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms, const double* site_ops,
+                     const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
+                     int64_t workspace_bytes, dmrg_plan** out) {
+    if (!out) { set_error("dmrg_plan_create: out is NULL"); return DMRG_EINVAL; }
+    *out = nullptr;
+    if (!ops || nterms < 0 || (nterms > 0 && !terms) || !site_ops || !site_parity || nsite <= 0) {
+        set_error("dmrg_plan_create: NULL or empty argument");
+        return DMRG_EINVAL;
+    }
+    dmrg_plan* P = new (std::nothrow) dmrg_plan();
+    if (!P) { set_error("dmrg_plan_create: out of host memory"); return DMRG_ENOMEM; }
+    P->ops = ops;
+    int rc;
+    try {
+        rc = plan_build(P, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, workspace_bytes);
+    } catch (const std::bad_alloc&) {
+        set_error("dmrg_plan_create: out of host memory");
+        rc = DMRG_ENOMEM;
+    } catch (const std::exception& e) {
+        set_error("dmrg_plan_create: %s", e.what());
+        rc = DMRG_EINVAL;
+    }
+    if (rc != DMRG_OK) { dmrg_plan_destroy(P); return rc; }
+    *out = P;
+    return DMRG_OK;
+}
+
+void dmrg_plan_destroy(dmrg_plan* P) {
+    if (!P) return;
+    cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks);
+    for (auto e : P->ev) cudaEventDestroy(e);
+    if (P->dav) davidson_ws_free(P->dav);
+    delete P;
+}
+
+int64_t dmrg_plan_psi_size(const dmrg_plan* P) { return P ? P->psi_size : 0; }
+int64_t dmrg_plan_num_psi_blocks(const dmrg_plan* P) { return P ? (int64_t)P->blocks.size() : 0; }
+int dmrg_plan_psi_layout(const dmrg_plan* P, dmrg_psi_block* out) {
+    if (!P || !out) { set_error("dmrg_plan_psi_layout: NULL argument"); return DMRG_EINVAL; }
+    std::copy(P->blocks.begin(), P->blocks.end(), out);
+    return DMRG_OK;
+}
+double dmrg_plan_stat(const dmrg_plan* P, int32_t key) { return (P && key >= 0 && key < ST_COUNT) ? P->stats[key] : -1.0; }
+
+int dmrg_plan_set_timing(dmrg_plan* P, int32_t enable) {
+    if (!P) { set_error("dmrg_plan_set_timing: NULL plan"); return DMRG_EINVAL; }
+    if (enable && P->ev.empty()) {
+        P->ev.resize(2 * P->launches.size() + 2);
+        for (auto& e : P->ev) DMRG_CUDA(cudaEventCreate(&e));
+    }
+    P->timing = enable != 0;
+    P->timing_valid = false;
+    return DMRG_OK;
+}
+
+double dmrg_plan_stage_ms(dmrg_plan* P, int32_t which) {
+    if (!P || !P->timing_valid) { set_error("dmrg_plan_stage_ms: no timed dmrg_sigma call"); return -1.0; }
+    const size_t nl = P->launches.size();
+    if (cudaEventSynchronize(P->ev[2 * nl + 1]) != cudaSuccess) { set_error("dmrg_plan_stage_ms: event sync failed"); return -1.0; }
+    float ms = 0.f;
+    if (which == 2) { cudaEventElapsedTime(&ms, P->ev[2 * nl], P->ev[2 * nl + 1]); return ms; }
+    double tot = 0.0;
+    for (size_t i = 0; i < nl; i++)
+        if (P->launches[i].stage == which + 1) { cudaEventElapsedTime(&ms, P->ev[2 * i], P->ev[2 * i + 1]); tot += ms; }
+    return tot;
+}
+
+int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream) {
+    if (!P || !psi || !sigma) { set_error("dmrg_sigma: NULL argument"); return DMRG_EINVAL; }
+    if (((uintptr_t)psi & 15) || ((uintptr_t)sigma & 15)) { set_error("dmrg_sigma: psi and sigma must be 16-byte aligned"); return DMRG_EINVAL; }
+    if (psi == sigma) { set_error("dmrg_sigma: psi and sigma must not alias"); return DMRG_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nl = P->launches.size();
+    if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * nl], st));
+    DMRG_CUDA(cudaMemsetAsync(sigma, 0, sizeof(double) * (size_t)P->psi_size, st));
+    for (size_t i = 0; i < nl; i++) {
+        const PlanLaunch& L = P->launches[i];
+        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * i], st));
+        int rc = launch_grouped_gemm(L.variant, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
+                                     P->ops->d_values, P->d_xws, psi, sigma, st);
+        if (rc != DMRG_OK) return rc;
+        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * i + 1], st));
+    }
+    if (P->timing) { DMRG_CUDA(cudaEventRecord(P->ev[2 * nl + 1], st)); P->timing_valid = true; }
+    return DMRG_OK;
+}
+
+int dmrg_sigma_host(dmrg_plan* P, const double* psi_host, double* sigma_host, void* cuda_stream) {
+    if (!P || !psi_host || !sigma_host) { set_error("dmrg_sigma_host: NULL argument"); return DMRG_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    double* d = nullptr;
+    const size_t bytes = sizeof(double) * (size_t)P->psi_size;
+    const size_t pad = (bytes + 255) & ~size_t(255);
+    DMRG_CUDA(cudaMalloc(&d, 2 * pad));
+    double* d_sig = (double*)((char*)d + pad);
+    int rc = DMRG_OK;
+    cudaError_t e = cudaMemcpyAsync(d, psi_host, bytes, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) {
+        rc = dmrg_sigma(P, d, d_sig, cuda_stream);
+        if (rc == DMRG_OK) e = cudaMemcpyAsync(sigma_host, d_sig, bytes, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    cudaFree(d);
+    if (rc != DMRG_OK) return rc;
+    if (e != cudaSuccess) { set_error("dmrg_sigma_host: %s", cudaGetErrorString(e)); return DMRG_ECUDA; }
+    return DMRG_OK;
+}
+
+int dmrg_hdiag(dmrg_plan* P, double* diag, void* cuda_stream) {
+    if (!P || !diag) { set_error("dmrg_hdiag: NULL argument"); return DMRG_EINVAL; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int64_t YB = 32768;
+    for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += YB) {
+        const unsigned ny = (unsigned)std::min<int64_t>(YB, P->n_hd_blocks - y0);
+        hdiag_kernel<<<dim3(16, ny), 256, 0, st>>>(P->d_hd_blocks + y0, P->d_hd_items, P->ops->d_values, diag);
+    }
+    DMRG_CUDA(cudaGetLastError());
+    return DMRG_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,40 @@
+// dmrg_plan internals (not part of the ABI).
+#pragma once
+#include "common.h"
+
+struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // offsets < 0: identity factor
+struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; };
+
+struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
+
+enum {
+    ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
+    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_COUNT
+};
+
+struct DavidsonWs;
+
+struct dmrg_plan {
+    const dmrg_ops* ops = nullptr;
+    std::vector<dmrg_psi_block> blocks;
+    int64_t psi_size = 0;
+    dmrg::Job* d_jobs = nullptr;
+    dmrg::Seg* d_segs = nullptr;
+    dmrg::Tile* d_tiles = nullptr;
+    double* d_xws = nullptr;
+    int64_t xws_elems = 0;
+    std::vector<PlanLaunch> launches;
+    HdItem* d_hd_items = nullptr;
+    HdBlock* d_hd_blocks = nullptr;
+    int64_t n_hd_blocks = 0;
+    double stats[ST_COUNT] = {0};
+    // optional per-stage timing
+    bool timing = false;
+    std::vector<cudaEvent_t> ev;   // 2 per launch + 2
+    bool timing_valid = false;
+    DavidsonWs* dav = nullptr;
+};
+
+namespace dmrg {
+void davidson_ws_free(DavidsonWs* ws);
+}

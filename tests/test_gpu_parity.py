@@ -1,0 +1,189 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): max|d sigma| / ||sigma||_2 <= 1e-11 in FP64; Davidson energies within
+1e-9 Hartree; sigma bitwise identical run to run.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+import oracle  # noqa: E402
+from oracle.davidson import davidson as oracle_davidson  # noqa: E402
+from dmrg_workload.problem import make_blocked_problem, random_psi  # noqa: E402
+
+TOL_SIGMA = 1e-11
+TOL_E = 1e-9
+
+
+def _gpu():
+    import paper_2311_02854_b200 as g
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    return g
+
+
+def _sigma_gpu(plan, psi):
+    d_psi = torch.from_numpy(psi).cuda()
+    d_sig = torch.empty_like(d_psi)
+    plan.sigma(d_psi, d_sig, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    return d_sig.cpu().numpy()
+
+
+CASES = {
+    "cfg1_K8_exact": dict(K=8, nL=3, N_tot=8, D=None, seed=1),
+    "K6_trunc": dict(K=6, nL=2, N_tot=6, D=8, seed=62, force_dmax=False),
+    "K7_asym_rot": dict(K=7, nL=3, N_tot=8, D=10, seed=73, force_dmax=False, rotate=True),
+    "K8_1left": dict(K=8, nL=1, N_tot=8, D=40, seed=5, force_dmax=False),
+    "K10_D60": dict(K=10, nL=4, N_tot=10, D=60, seed=3),
+    "K12_D100": dict(K=12, nL=5, N_tot=12, D=100, seed=1),
+    "K12_D150_odd": dict(K=12, nL=5, N_tot=11, twoSz_tot=1, D=150, seed=2, force_dmax=False),
+}
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def case(request):
+    g = _gpu()
+    pr = make_blocked_problem(**CASES[request.param])
+    ops, plan = g.load_problem(pr)
+    yield request.param, pr, plan
+    plan.destroy()
+    ops.free()
+
+
+def test_layout_matches_workload(case):
+    _, pr, plan = case
+    assert plan.psi_size == pr.psi_size
+    assert np.array_equal(plan.psi_layout(), pr.layout)
+
+
+def test_sigma_matches_oracle(case):
+    name, pr, plan = case
+    for seed in (5, 6):
+        psi = random_psi(pr.psi_size, seed)
+        ref, st = oracle.opair_sigma(pr, psi, return_stats=True)
+        got = _sigma_gpu(plan, psi)
+        err = np.abs(got - ref).max() / np.linalg.norm(ref)
+        assert err <= TOL_SIGMA, (name, err)
+    s = plan.stats()
+    assert s["tasks"] == st["tasks"]
+    assert abs(s["canon_flops"] - st["flops"]) <= 1e-9 * max(1.0, st["flops"])
+
+
+def test_sigma_bitwise_reproducible(case):
+    _, pr, plan = case
+    psi = random_psi(pr.psi_size, 11)
+    a = _sigma_gpu(plan, psi)
+    for _ in range(3):
+        assert np.array_equal(a, _sigma_gpu(plan, psi))
+
+
+def test_sigma_host_entry(case):
+    _, pr, plan = case
+    psi = random_psi(pr.psi_size, 12)
+    out = np.empty_like(psi)
+    plan.sigma_host(psi, out)
+    assert np.array_equal(out, _sigma_gpu(plan, psi))
+
+
+def test_hdiag_matches_oracle(case):
+    name, pr, plan = case
+    ref = oracle.opair_hdiag(pr)
+    d = torch.empty(pr.psi_size, dtype=torch.float64, device="cuda")
+    plan.hdiag(d, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert np.abs(d.cpu().numpy() - ref).max() <= 1e-12 * max(1.0, np.abs(ref).max()), name
+
+
+def test_hermiticity_gpu(case):
+    _, pr, plan = case
+    psi, phi = random_psi(pr.psi_size, 1), random_psi(pr.psi_size, 2)
+    assert abs(phi @ _sigma_gpu(plan, psi) - _sigma_gpu(plan, phi) @ psi) < 1e-12
+
+
+def test_chunked_workspace_gives_same_sigma(case):
+    """A tiny X workspace forces many chunks; sigma must not change beyond rounding."""
+    g = _gpu()
+    name, pr, plan = case
+    psi = random_psi(pr.psi_size, 21)
+    ref = _sigma_gpu(plan, psi)
+    plan2 = g.Plan(plan.ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot,
+                   workspace_bytes=1)
+    assert plan2.stats()["chunks"] > plan.stats()["chunks"] or plan.stats()["chunks"] > 1 or pr.psi_size < 10
+    got = _sigma_gpu(plan2, psi)
+    plan2.destroy()
+    assert np.abs(got - ref).max() / np.linalg.norm(ref) <= 1e-13, name
+
+
+def test_davidson_matches_oracle(case):
+    """Energies agree to 1e-9 Eh.  Davidson from a random start amplifies rounding differences by about
+    10x per iteration (the preconditioner den/(den^2+delta^2) has slope 1/delta^2 = 1e6 where theta crosses
+    Hd), so trajectories are compared only over the first iterations; what is compared at 1e-9 is (i) the
+    converged energy and (ii) the returned theta against the oracle's Rayleigh quotient of the returned x."""
+    name, pr, plan = case
+    if pr.psi_size > 60000:
+        pytest.skip("oracle Davidson too slow here")
+    hd = oracle.opair_hdiag(pr)
+    x0 = random_psi(pr.psi_size, 9)
+    converge = pr.psi_size <= 10000
+    it, tol = (400, 1e-8) if converge else (12, 1e-10)
+    ref = oracle_davidson(lambda v: oracle.opair_sigma(pr, v), hd, x0, max_iter=it, max_space=30, tol=tol)
+    x = torch.from_numpy(x0).cuda()
+    res = plan.davidson(x, max_iter=it, max_space=30, tol=tol, stream=torch.cuda.current_stream())
+    n = min(4, len(ref["thetas"]), len(res["thetas"]))
+    assert np.abs(np.array(ref["thetas"][:n]) - res["thetas"][:n]).max() <= TOL_E, name
+    xn = x.cpu().numpy()
+    assert abs(np.linalg.norm(xn) - 1.0) < 1e-12
+    hx = oracle.opair_sigma(pr, xn)
+    assert abs(xn @ hx - res["energy"]) <= TOL_E, name
+    assert abs(np.linalg.norm(hx - res["energy"] * xn) - res["resid"]) <= 1e-8, name
+    if converge:
+        assert res["converged"] and ref["resid"] <= tol, name
+        assert abs(res["energy"] - ref["energy"]) <= TOL_E, name
+        assert abs(abs(float(xn @ ref["x"])) - 1.0) < 1e-5, name
+
+
+def test_cfg1_davidson_ground_energy():
+    """configs[0]: Davidson ground energy == exact diagonalisation of the dense FCI H (1e-9 Eh)."""
+    g = _gpu()
+    from dmrg_workload.problem import determinant_map
+    pr = make_blocked_problem(8, 3, 8, 0, D=None, seed=1, track=True)
+    dets, Pm = determinant_map(pr)
+    H = oracle.fci_dense_h(dets, 16, pr.ints.dense_h(), pr.ints.dense_V())
+    e0 = np.linalg.eigvalsh(H)[0]
+    ops, plan = g.load_problem(pr)
+    x = torch.from_numpy(random_psi(pr.psi_size, 9)).cuda()
+    res = plan.davidson(x, max_iter=300, max_space=30, tol=1e-8, stream=torch.cuda.current_stream())
+    assert res["converged"] and res["resid"] <= 1e-8
+    assert abs(res["energy"] - e0) < TOL_E
+    # and sigma equals the FCI definition directly
+    psi = random_psi(pr.psi_size, 5)
+    ref = Pm.T @ (H @ (Pm @ psi))
+    assert np.abs(_sigma_gpu(plan, psi) - ref).max() / np.linalg.norm(ref) <= TOL_SIGMA
+    plan.destroy()
+    ops.free()
+
+
+def test_error_paths():
+    g = _gpu()
+    pr = make_blocked_problem(6, 2, 6, 0, D=8, seed=62, force_dmax=False)
+    ops, plan = g.load_problem(pr)
+    # a term that does not conserve charge is rejected
+    bad = pr.term_idx.copy()
+    cre = next(i for i in range(len(pr.ops)) if pr.ops[i][0] == 0 and pr.ops[i][1] == 1)
+    bad[0] = (cre, 0, 0, 0, -1, 0)
+    with pytest.raises(g.DmrgError) as ei:
+        g.Plan(ops, pr.term_coef, bad, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot)
+    assert ei.value.code == -2
+    # aliasing psi / sigma is rejected
+    v = torch.zeros(pr.psi_size, dtype=torch.float64, device="cuda")
+    with pytest.raises(g.DmrgError):
+        plan.sigma(v, v)
+    # empty target sector
+    with pytest.raises(g.DmrgError):
+        g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, 999, 0)
+    plan.destroy()
+    ops.free()
