@@ -3,6 +3,7 @@ import numpy as np
 
 from .blocking import build_block
 from .integrals import make_integrals
+from .sectors import block_sector_model
 from .store import assemble, block_values_from_rblocks, sectors_of
 from .terms import Partition, TermTable
 
@@ -30,6 +31,41 @@ def make_blocked_problem(K, nL, N_tot, twoSz_tot=0, D=None, seed=1, banded=False
     pr.meta = dict(K=K, nL=nL, nR=K - nL - 2, D=D, seed=seed, mode="blocking", banded=banded)
     pr.ints, pr.part, pr.bL, pr.bR, pr.tt = ints, part, bL, bR, tt
     return pr
+
+
+def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False, ints=None):
+    """Direct fill (cfg 3-5; DESIGN.md input recipe): integrals and the term table are the real ones,
+    the sector tables follow the d_max(D) model of sectors.py, and every charge-allowed operator block
+    is filled with seeded N(0, 1/d_max) entries (H, B_pp, Q_pp symmetric).  The contraction workload
+    (block shapes, term list, coefficients, sparsity) is that of an honest bond at this D; the summed
+    operator is Hermitian but is NOT a projected physical Hamiltonian."""
+    ints = ints if ints is not None else make_integrals(K, seed, banded=banded)
+    part = Partition(K, nL)
+    secL = block_sector_model(nL, K, N_tot, twoSz_tot, D)
+    secR = block_sector_model(K - nL - 2, K, N_tot, twoSz_tot, D)
+    tt = TermTable(part, ints)
+    dmax = max(max(s[2] for s in secL), max(s[2] for s in secR))
+    pr = assemble(tt, secL, secR, None, N_tot, twoSz_tot, direct_seed=seed + 104729, direct_scale=dmax ** -0.5)
+    pr.meta = dict(K=K, nL=nL, nR=K - nL - 2, D=D, seed=seed, mode="direct", banded=banded)
+    pr.ints, pr.part, pr.tt = ints, part, tt
+    return pr
+
+
+CONFIGS = {
+    # BASELINE.json configs[0..4]; partition = centre two-dot (DESIGN.md input recipe)
+    "cfg1": dict(gen="blocked", K=8, nL=3, N_tot=8, D=None, seed=1),
+    "cfg2": dict(gen="blocked", K=24, nL=11, N_tot=24, D=500, seed=1),
+    "cfg3": dict(gen="direct", K=36, nL=17, N_tot=36, D=1500, seed=1),
+    "cfg4": dict(gen="direct", K=73, nL=35, N_tot=114, D=1000, seed=1, banded=True),
+    "cfg5": dict(gen="direct", K=73, nL=35, N_tot=114, D=3000, seed=1, banded=True),
+}
+
+
+def make_config(name, **over):
+    kw = dict(CONFIGS[name])
+    kw.update(over)
+    gen = kw.pop("gen")
+    return make_blocked_problem(**kw) if gen == "blocked" else make_direct_problem(**kw)
 
 
 def determinant_map(pr):

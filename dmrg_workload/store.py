@@ -60,12 +60,36 @@ def _op_sort_key(op):
     return (0 if op.side == "L" else 1, KIND[op.kind], op.p, op.q)
 
 
-def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot):
+def _fill_normal(out, seed, nthreads=None):
+    """out[:] ~ N(0,1), reproducible for a given (seed, len(out)) whatever the thread count:
+    the array is cut into fixed 16 Mi-double pieces, piece i drawn from Philox(key=seed, counter block i)."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    piece = 1 << 24
+    n = out.shape[0]
+    npieces = (n + piece - 1) // piece
+
+    def work(i):
+        g = np.random.Generator(np.random.Philox(key=seed, counter=[0, 0, 0, i + 1]))
+        g.standard_normal(out=out[i * piece:min(n, (i + 1) * piece)])
+
+    nthreads = nthreads or min(32, os.cpu_count() or 1)
+    if npieces <= 1 or nthreads <= 1:
+        for i in range(npieces):
+            work(i)
+    else:
+        with ThreadPoolExecutor(nthreads) as ex:
+            list(ex.map(work, range(npieces)))
+
+
+def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, direct_scale=1.0):
     """Build a Problem from a TermTable.
 
     block_values(op, row_sector, col_sector, shape) -> ndarray or None (block absent);
     called for every stored (non-LINCOMB) op and every charge-allowed sector pair.
-    """
+    block_values=None ("direct fill", cfg 3-5): every charge-allowed block is present and filled with
+    seeded N(0, direct_scale^2) entries; H, B_pp and Q_pp blocks are symmetrised so that the summed
+    operator stays Hermitian (the term table adds no h.c. for those)."""
     from .sectors import psi_layout
     from .terms import BlockOp, dot_parity
     pr = Problem()
@@ -78,26 +102,40 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot):
     stored = sorted([o for s in "LR" for o in ref[s] if o.kind != "LIN"], key=_op_sort_key)
     op_id = {}
     ops_rows, blk_rows, vals = [], [], []
+    sym_blocks = []   # direct fill: (offset, d) of square blocks to symmetrise
     off = 0
     for op in stored:
         dq = op_charge(op)
         first = len(blk_rows)
         sl = secs[op.side]
+        self_adjoint = op.kind == "H" or (op.kind in ("B", "Q") and op.p == op.q)
         for ic, qc in enumerate(sl):
             ir = sidx[op.side].get((qc[0] + dq[0], qc[1] + dq[1]))
             if ir is None:
                 continue
             shape = (sl[ir][2], qc[2])
-            m = block_values(op, ir, ic, shape)
-            if m is None:
-                continue
-            assert m.shape == shape
+            if block_values is not None:
+                m = block_values(op, ir, ic, shape)
+                if m is None:
+                    continue
+                assert m.shape == shape
+                vals.append(np.ascontiguousarray(m, dtype=np.float64).ravel())
+            elif self_adjoint:
+                assert ir == ic
+                sym_blocks.append((off, shape[0]))
             blk_rows.append((ir, ic, off))
-            vals.append(np.ascontiguousarray(m, dtype=np.float64).ravel())
             off += shape[0] * shape[1]
         op_id[op] = len(ops_rows)
         ops_rows.append((0 if op.side == "L" else 1, KIND[op.kind], op.p, op.q, dq[0], dq[1],
                          first, len(blk_rows) - first))
+    if block_values is None:
+        values = np.empty(off, dtype=np.float64)
+        _fill_normal(values, int(direct_seed))
+        if direct_scale != 1.0:
+            values *= direct_scale
+        for o, d in sym_blocks:
+            m = values[o:o + d * d].reshape(d, d)
+            m[:] = (m + m.T) * 0.5
     lin_ptr, lin_op, lin_coef = [0], [], []
     for side in "LR":
         for j, lc in enumerate(tt.lincombs[side]):
@@ -113,7 +151,9 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot):
             lin_ptr.append(len(lin_op))
     pr.ops = np.array(ops_rows, dtype=np.int64).reshape(-1, 8)
     pr.blocks = np.array(blk_rows, dtype=np.int64).reshape(-1, 3)
-    pr.values = np.concatenate(vals) if vals else np.zeros(0)
+    if block_values is not None:
+        values = np.concatenate(vals) if vals else np.zeros(0)
+    pr.values = values
     pr.lin_ptr = np.array(lin_ptr, dtype=np.int64)
     pr.lin_op = np.array(lin_op, dtype=np.int32)
     pr.lin_coef = np.array(lin_coef, dtype=np.float64)

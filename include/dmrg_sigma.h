@@ -90,6 +90,9 @@ typedef struct dmrg_plan dmrg_plan;   /* GEMM-pair plan for one bond            
  *   values    [host] or [device] (values_on_device != 0): nvalues doubles; block b is the row-major
  *             dim[row] x dim[col] matrix at values + blocks[b].offset.  Not retained: the store
  *             keeps its own (row-padded) copy, the caller may free `values` on return.
+ *             values == NULL loads the STRUCTURE only (no CUDA call, no device memory): such a store
+ *             can be planned (dmrg_plan_create, dmrg_plan_stat, dmrg_plan_psi_layout) to size a
+ *             problem, but dmrg_sigma / dmrg_hdiag / dmrg_davidson on it fail with DMRG_EINVAL.
  *   lin_ptr   [host]  CSR over LINCOMB operators (nlin+1 entries); LINCOMB op with p = j is
  *             sum_{i in [lin_ptr[j], lin_ptr[j+1])} lin_coef[i] * ops[lin_op[i]]; all summands must be
  *             stored (non-LINCOMB) operators of the same side and charge as the LINCOMB op.

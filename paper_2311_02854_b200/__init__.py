@@ -130,7 +130,9 @@ class OpsStore:
                                                                   ("d2sz", 5), ("first_block", 6), ("nblocks", 7)))
         bd = _structured(np.asarray(blocks).reshape(-1, 3), BLOCK_DT, (("row_sector", 0), ("col_sector", 1), ("offset", 2)))
         on_dev = 0
-        if isinstance(values, np.ndarray):
+        if values is None:
+            nvalues = int(max((b[2] for b in np.asarray(blocks).reshape(-1, 3)), default=0)) + (1 << 40)
+        elif isinstance(values, np.ndarray):
             values = np.ascontiguousarray(values, dtype=np.float64)
         else:
             assert values.is_cuda and values.is_contiguous() and values.element_size() == 8
@@ -138,7 +140,8 @@ class OpsStore:
         lp = np.ascontiguousarray(lin_ptr, dtype=np.int64)
         lo = np.ascontiguousarray(lin_op, dtype=np.int32)
         lc = np.ascontiguousarray(lin_coef, dtype=np.float64)
-        nvalues = int(values.size if on_dev == 0 else values.numel())
+        if values is not None:
+            nvalues = int(values.size if on_dev == 0 else values.numel())
         h = C.c_void_p()
         _check(lib().dmrg_ops_load(_ptr(sl), len(sl), _ptr(sr), len(sr), _ptr(od), len(od), _ptr(bd), len(bd),
                                    _ptr(values), nvalues, on_dev, _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1, C.byref(h)))
@@ -241,9 +244,11 @@ def fp64_peak_tflops(which, ms=200.0, stream=None):
     return v
 
 
-def load_problem(pr, workspace_bytes=0, values=None):
-    """Convenience: OpsStore + Plan from a dmrg_workload Problem (array formats of dmrg_workload/store.py)."""
-    ops = OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks, pr.values if values is None else values,
+def load_problem(pr, workspace_bytes=0, values=None, structure_only=False):
+    """Convenience: OpsStore + Plan from a dmrg_workload Problem (array formats of dmrg_workload/store.py).
+    structure_only=True plans without a device (statistics / layout only)."""
+    ops = OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks,
+                   None if structure_only else (pr.values if values is None else values),
                    pr.lin_ptr, pr.lin_op, pr.lin_coef)
     plan = Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, workspace_bytes)
     return ops, plan

@@ -103,6 +103,7 @@ struct dmrg_ops {
     std::vector<std::vector<int64_t>> row_off;
     std::vector<std::vector<int32_t>> colsec;
     double* d_values = nullptr;
+    bool structure_only = false;   // loaded with values == NULL: planning / statistics only, no device memory
     int64_t nvalues_dev = 0;     // doubles allocated (stored + lincomb, padded)
     int64_t device_bytes = 0;
 };

@@ -250,6 +250,7 @@ static int davidson_impl(dmrg_plan* P, double* x_io, int max_iter, int max_space
 extern "C" int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_space, double tol, double* energy,
                              double* resid_norm, int32_t* iters, double* thetas, void* cuda_stream) {
     if (!plan || !x || max_iter < 1 || max_space < 1) { dmrg::set_error("dmrg_davidson: bad argument"); return DMRG_EINVAL; }
+    if (plan->ops->structure_only) { dmrg::set_error("dmrg_davidson: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     if ((uintptr_t)x & 15) { dmrg::set_error("dmrg_davidson: x must be 16-byte aligned"); return DMRG_EINVAL; }
     try {
         return dmrg::davidson_impl(plan, x, max_iter, max_space, tol, energy, resid_norm, iters, thetas, (cudaStream_t)cuda_stream);

@@ -44,6 +44,21 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 
 struct StageMeta { double alpha; uint32_t flags; int32_t ksteps; };
 
+// fold alpha into the smaller fragment set; |alpha| = 1 flips the sign bit on the integer pipe
+// instead of spending an FP64 issue slot
+template <int FM, int FN>
+__device__ __forceinline__ void scale_frags(double (&af)[FM], double (&bf)[FN], int mode, double alpha) {
+    if (FM <= FN) {
+#pragma unroll
+        for (int i = 0; i < FM; i++)
+            af[i] = mode == 1 ? __hiloint2double(__double2hiint(af[i]) ^ 0x80000000, __double2loint(af[i])) : af[i] * alpha;
+    } else {
+#pragma unroll
+        for (int j = 0; j < FN; j++)
+            bf[j] = mode == 1 ? __hiloint2double(__double2hiint(bf[j]) ^ 0x80000000, __double2loint(bf[j])) : bf[j] * alpha;
+    }
+}
+
 // Stage one operand tile (MN x BK) of a segment into shared memory.
 //   kcontig: global (mn,k) at g + mn*ld + k, shared at mn*KPAD + k
 //   else   : global (mn,k) at g + k*ld + mn, shared at k*(BMN+4) + mn
@@ -121,7 +136,10 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     const int m0 = tile.tm * BM, n0 = tile.tn * BN;
     const int m_lim = job.M - m0, n_lim = job.N - n0;
 
-    const double* const space_r[4] = {ops, xws, psi, sigma};
+    // 8x8 fragments of this warp that intersect the matrix
+    const int fm_eff = max(0, min(FM, (m_lim - wm0 + 7) >> 3)), fn_eff = max(0, min(FN, (n_lim - wn0 + 7) >> 3));
+    const bool full_tile = fm_eff == FM && fn_eff == FN;
+    auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
     double* const c_base = ((job.flags >> JOB_C_SPACE_SHIFT) & 3u) == SP_X ? xws : sigma;
 
     double acc[FM][FN][2];
@@ -135,7 +153,7 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     for (; seg0 < job.seg_end; seg0++) {
         const Seg s = segs[seg0];
         if (!(s.flags & SEG_A_IDENT)) break;
-        const double* b = space_r[(s.flags >> SEG_B_SPACE_SHIFT) & 3u] + s.b_off;
+        const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
 #pragma unroll
         for (int i = 0; i < FM; i++) {
             const int r = m0 + wm0 + 8 * i + lr;
@@ -164,9 +182,9 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
             const int k_lim = ls.K - lk0;
             const bool a_kc = !(ls.flags & SEG_A_MCONTIG);
             const bool b_kc = (ls.flags & SEG_B_KCONTIG) != 0;
-            const double* ga = space_r[(ls.flags >> SEG_A_SPACE_SHIFT) & 3u] + ls.a_off +
+            const double* ga = space_r((ls.flags >> SEG_A_SPACE_SHIFT) & 3u) + ls.a_off +
                                (a_kc ? (int64_t)m0 * ls.lda + lk0 : (int64_t)lk0 * ls.lda + m0);
-            const double* gb = space_r[(ls.flags >> SEG_B_SPACE_SHIFT) & 3u] + ls.b_off +
+            const double* gb = space_r((ls.flags >> SEG_B_SPACE_SHIFT) & 3u) + ls.b_off +
                                (b_kc ? (int64_t)n0 * ls.ldb + lk0 : (int64_t)lk0 * ls.ldb + n0);
             load_operand<BM, NT>(sa, ga, ls.lda, a_kc, (ls.flags & SEG_A_VEC2) != 0, m_lim, k_lim, tid);
             load_operand<BN, NT>(sb, gb, ls.ldb, b_kc, (ls.flags & SEG_B_VEC2) != 0, n_lim, k_lim, tid);
@@ -204,29 +222,35 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
         const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
         const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
         const int mode = mt.alpha == 1.0 ? 0 : (mt.alpha == -1.0 ? 1 : 2);
-        for (int kk = 0; kk < mt.ksteps; kk++) {
-            double af[FM], bf[FN];
+        if (full_tile) {
+            for (int kk = 0; kk < mt.ksteps; kk++) {
+                double af[FM], bf[FN];
 #pragma unroll
-            for (int i = 0; i < FM; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
+                for (int i = 0; i < FM; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
 #pragma unroll
-            for (int j = 0; j < FN; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
-            if (mode != 0) {
-                // fold alpha into the smaller fragment set; |alpha| = 1 flips the sign bit on the
-                // integer pipe instead of spending an FP64 issue slot
-                if (FM <= FN) {
+                for (int j = 0; j < FN; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
+                if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
 #pragma unroll
-                    for (int i = 0; i < FM; i++)
-                        af[i] = mode == 1 ? __hiloint2double(__double2hiint(af[i]) ^ 0x80000000, __double2loint(af[i])) : af[i] * mt.alpha;
-                } else {
+                for (int i = 0; i < FM; i++)
+#pragma unroll
+                    for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            }
+        } else {
+            // ragged tile: 8x8 fragments that lie entirely outside the matrix are skipped (warp-uniform
+            // predicates), so the executed work is padded to multiples of 8, not of the tile size
+            for (int kk = 0; kk < mt.ksteps; kk++) {
+                double af[FM], bf[FN];
+#pragma unroll
+                for (int i = 0; i < FM; i++) af[i] = i < fm_eff ? pa[8 * i * a_sm + 4 * kk * a_sk] : 0.0;
+#pragma unroll
+                for (int j = 0; j < FN; j++) bf[j] = j < fn_eff ? pb[8 * j * b_sn + 4 * kk * b_sk] : 0.0;
+                if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
+#pragma unroll
+                for (int i = 0; i < FM; i++)
 #pragma unroll
                     for (int j = 0; j < FN; j++)
-                        bf[j] = mode == 1 ? __hiloint2double(__double2hiint(bf[j]) ^ 0x80000000, __double2loint(bf[j])) : bf[j] * mt.alpha;
-                }
+                        if (i < fm_eff && j < fn_eff) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
             }
-#pragma unroll
-            for (int i = 0; i < FM; i++)
-#pragma unroll
-                for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
         }
     }
     cp_async_wait<0>();

@@ -69,10 +69,13 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
     DMRG_REQUIRE(secL && secR && nsecL > 0 && nsecR > 0, "dmrg_ops_load: empty sector table");
     DMRG_REQUIRE(nops >= 0 && nblocks >= 0 && nvalues >= 0, "dmrg_ops_load: negative count");
     DMRG_REQUIRE(nops == 0 || ops, "dmrg_ops_load: ops is NULL");
-    DMRG_REQUIRE(nblocks == 0 || (blocks && values), "dmrg_ops_load: blocks/values is NULL");
+    DMRG_REQUIRE(nblocks == 0 || blocks, "dmrg_ops_load: blocks is NULL");
+    S->structure_only = (values == nullptr);
     DMRG_REQUIRE(nlin == 0 || (lin_ptr && lin_op && lin_coef), "dmrg_ops_load: lincomb arrays are NULL");
-    int ndev = 0;
-    DMRG_CUDA(cudaGetDeviceCount(&ndev));
+    if (!S->structure_only) {
+        int ndev = 0;
+        DMRG_CUDA(cudaGetDeviceCount(&ndev));
+    }
     S->sec[0].assign(secL, secL + nsecL);
     S->sec[1].assign(secR, secR + nsecR);
     for (int side = 0; side < 2; side++)
@@ -145,6 +148,8 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
         }
     }
     S->nvalues_dev = top;
+    S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
+    if (S->structure_only) return DMRG_OK;
     DMRG_CUDA(cudaMalloc(&S->d_values, sizeof(double) * (size_t)std::max<int64_t>(top, 2)));
     S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
 

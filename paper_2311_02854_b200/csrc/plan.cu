@@ -24,9 +24,6 @@ namespace dmrg {
 static const int SITE_N[4] = {0, 1, 1, 2};
 static const int SITE_S[4] = {0, -1, 1, 0};
 
-// relative efficiency guesses of the tile variants (used only to pick a variant per job)
-static const double kVariantEff[NUM_VARIANTS] = {1.00, 1.04, 0.80, 0.45};
-
 struct Task {
     int32_t term_ord, in_blk, out_blk;
     int32_t l_trans, r_trans;
@@ -41,18 +38,28 @@ static inline int64_t xkey(int64_t r_off, int r_trans, int in_blk, int64_t nblk)
     return (r_off * 2 + r_trans) * nblk + in_blk;
 }
 
+// Tile variant for an M x N output: the largest tile shape whose tiles are at least ~60 % inside the
+// matrix.  With fragment skipping every variant executes the same ceil(M/8)*ceil(N/8) fragments per
+// k-step, so the choice trades operand re-use (large tiles) against occupancy for small blocks.
 static int choose_variant(int M, int N) {
-    int best = 0;
-    double bc = 1e300;
-    for (int v = 0; v < NUM_VARIANTS; v++) {
+    static const int pref[NUM_VARIANTS] = {1, 0, 2, 3};   // 128x64, 64x64, 32x32, 16x16
+    for (int t = 0; t < NUM_VARIANTS; t++) {
+        const int v = pref[t];
         const double bm = kVariants[v].bm, bn = kVariants[v].bn;
-        const double c = std::ceil(M / bm) * std::ceil(N / bn) * bm * bn / kVariantEff[v];
-        if (c < bc) { bc = c; best = v; }
+        const double util = (double)M * N / (std::ceil(M / bm) * std::ceil(N / bn) * bm * bn);
+        if (util >= 0.6) return v;
     }
-    return best;
+    return NUM_VARIANTS - 1;
 }
 
+static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N + 7) / 8); }
+
 struct TileRec { Tile t; double cost; };
+
+// split-K policy of stage 2 (see the comment at its use)
+constexpr double kCtaSlots = 148.0 * 3;     // resident 64x64 CTAs on a B200
+constexpr double kSplitWaves = 8.0;
+constexpr double kMinSplitStages = 32.0;    // K = 512
 
 static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
                       const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
@@ -242,6 +249,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     auto psi_vec2 = [&](const dmrg_psi_block& B) { return (B.offset % 2 == 0) && (B.dr % 2 == 0); };
 
     auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
+        PlanGroup grp{stage, (int)P->launches.size(), 0};
         for (int v = 0; v < NUM_VARIANTS; v++) {
             auto& r = recs[v];
             if (r.empty()) continue;
@@ -254,8 +262,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
                 i += n;
             }
-            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)r.size();
+            (stage == 1 ? s1_tiles : s2_tiles) += (stage == 3 ? 0 : (int64_t)r.size());
         }
+        grp.nlaunch = (int)P->launches.size() - grp.first_launch;
+        if (grp.nlaunch > 0) P->groups.push_back(grp);
     };
 
     for (int64_t ch = 0; ch < nchunks; ch++) {
@@ -314,7 +324,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             const double kpad4 = 4.0 * ((dRi + 3) / 4);
             for (int a = 0; a < ntm; a++)
                 for (int b = 0; b < ntn; b++) recs1[v].push_back({{(int32_t)jobs.size(), (uint16_t)a, (uint16_t)b}, kpad4});
-            padded_flops += 2.0 * ntm * bm * ntn * bn * kpad4;
+            padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
             s1_flops += 2.0 * rows * dRi * dRo;
             alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
             jobs.push_back(jb);
@@ -329,69 +339,139 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         std::vector<int64_t> idx(t1 - t0);
         for (int64_t i = 0; i < t1 - t0; i++) idx[i] = t0 + i;
         std::stable_sort(idx.begin(), idx.end(), [&](int64_t a, int64_t b) { return tasks[a].out_blk < tasks[b].out_blk; });
-        std::vector<TileRec> recs2[NUM_VARIANTS];
+        // pass A: size every sigma-block job to choose the split-K granularity of this chunk
+        struct Group { size_t i, j; int variant, ntm, ntn, nst; };
+        std::vector<Group> groups;
+        double tile_stages = 0.0;
         for (size_t i = 0; i < idx.size();) {
             size_t j = i;
             const int ob = tasks[idx[i]].out_blk;
-            while (j < idx.size() && tasks[idx[j]].out_blk == ob) j++;
-            const dmrg_psi_block& OB = P->blocks[ob];
-            Job jb;
-            jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
-            jb.seg_begin = (int32_t)segs.size();
-            jb.flags = (SP_SIGMA << JOB_C_SPACE_SHIFT) | JOB_BETA1;
             int nst = 0;
-            double kp4 = 0;
-            for (int pass = 0; pass < 2; pass++) {   // identity-L contributions first, then the GEMM segments
-                for (size_t q = i; q < j; q++) {
-                    const Task& k = tasks[idx[q]];
-                    const bool ident = k.l_off < 0;
-                    if (ident != (pass == 0)) continue;
-                    Seg s;
-                    s.alpha = k.alpha;
-                    s.K = k.dLi;
-                    s.flags = 0;
-                    if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
-                    else {
-                        s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
-                        s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | SEG_A_VEC2 | (k.l_trans ? SEG_A_MCONTIG : 0);
-                    }
-                    if (k.r_off < 0) {
-                        const dmrg_psi_block& IB = P->blocks[k.in_blk];
-                        s.b_off = IB.offset; s.ldb = IB.dr;
-                        s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | (psi_vec2(IB) ? SEG_B_VEC2 : 0);
-                        if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
-                    } else {
-                        const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
-                        s.b_off = xl.off; s.ldb = xl.ld;
-                        s.flags |= (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
-                        alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
-                    }
-                    if (!ident) {
-                        nst += (k.dLi + GEMM_BK - 1) / GEMM_BK;
-                        kp4 += 4.0 * ((k.dLi + 3) / 4);
-                        s2_flops += 2.0 * k.dLo * k.dLi * k.dRo;
-                        alg_flops += 2.0 * k.dLo * k.dLi * k.dRo;
-                        alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
-                    }
-                    segs.push_back(s);
-                    if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
-                }
+            while (j < idx.size() && tasks[idx[j]].out_blk == ob) {
+                if (tasks[idx[j]].l_off >= 0) nst += (tasks[idx[j]].dLi + GEMM_BK - 1) / GEMM_BK;
+                j++;
             }
-            DMRG_REQUIRE(segs.size() < ((size_t)1 << 31), "dmrg_plan_create: segment table overflow");
-            jb.seg_end = (int32_t)segs.size();
-            jb.pad_ = nst;
-            const int v = choose_variant(jb.M, jb.N);
+            const dmrg_psi_block& OB = P->blocks[ob];
+            const int v = choose_variant(OB.dl, OB.dr);
             const int bm = kVariants[v].bm, bn = kVariants[v].bn;
-            const int ntm = (jb.M + bm - 1) / bm, ntn = (jb.N + bn - 1) / bn;
-            DMRG_REQUIRE(ntm < 65536 && ntn < 65536, "dmrg_plan_create: too many tiles in one job");
-            for (int a = 0; a < ntm; a++)
-                for (int b = 0; b < ntn; b++) recs2[v].push_back({{(int32_t)jobs.size(), (uint16_t)a, (uint16_t)b}, kp4 + 1.0});
-            padded_flops += 2.0 * ntm * bm * ntn * bn * kp4;
-            alg_bytes += 16.0 * OB.dl * OB.dr;
-            jobs.push_back(jb);
+            Group g{i, j, v, (OB.dl + bm - 1) / bm, (OB.dr + bn - 1) / bn, nst};
+            DMRG_REQUIRE(g.ntm < 65536 && g.ntn < 65536, "dmrg_plan_create: too many tiles in one job");
+            // cost in units of 64x64x16 tile-stages
+            tile_stages += (double)g.ntm * g.ntn * nst * (bm * bn / 4096.0);
+            groups.push_back(g);
             i = j;
         }
+        // A tile's K-loop is the critical path of the launch: cap it at 1/kSplitWaves of the time the
+        // whole launch would take on a perfectly balanced machine, but never below kMinSplitStages.
+        const double smax = std::max<double>(kMinSplitStages, tile_stages / (kCtaSlots * kSplitWaves));
+        std::vector<TileRec> recs2[NUM_VARIANTS], recs3[NUM_VARIANTS];
+        int64_t ptop = xtop;   // split-K partial tiles live behind the X intermediates
+        std::vector<Seg> ident_segs, gemm_segs;
+        for (const Group& g : groups) {
+            const int ob = tasks[idx[g.i]].out_blk;
+            const dmrg_psi_block& OB = P->blocks[ob];
+            ident_segs.clear();
+            gemm_segs.clear();
+            double kp4 = 0;
+            for (size_t q = g.i; q < g.j; q++) {
+                const Task& k = tasks[idx[q]];
+                const bool ident = k.l_off < 0;
+                Seg s;
+                s.alpha = k.alpha;
+                s.K = k.dLi;
+                s.flags = 0;
+                if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
+                else {
+                    s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
+                    s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | SEG_A_VEC2 | (k.l_trans ? SEG_A_MCONTIG : 0);
+                }
+                if (k.r_off < 0) {
+                    const dmrg_psi_block& IB = P->blocks[k.in_blk];
+                    s.b_off = IB.offset; s.ldb = IB.dr;
+                    s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | (psi_vec2(IB) ? SEG_B_VEC2 : 0);
+                    if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
+                } else {
+                    const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
+                    s.b_off = xl.off; s.ldb = xl.ld;
+                    s.flags |= (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
+                    alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
+                }
+                if (!ident) {
+                    kp4 += 4.0 * ((k.dLi + 3) / 4);
+                    s2_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                    alg_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                    alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
+                }
+                (ident ? ident_segs : gemm_segs).push_back(s);
+                if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
+            }
+            padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
+            alg_bytes += 16.0 * OB.dl * OB.dr;
+            const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
+            auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
+                for (int a = 0; a < g.ntm; a++)
+                    for (int b = 0; b < g.ntn; b++) recs[g.variant].push_back({{job_id, (uint16_t)a, (uint16_t)b}, cost});
+            };
+            Job jb;
+            jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
+            jb.flags = (SP_SIGMA << JOB_C_SPACE_SHIFT) | JOB_BETA1;
+            if (nsplit == 1) {
+                jb.seg_begin = (int32_t)segs.size();
+                segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());
+                segs.insert(segs.end(), gemm_segs.begin(), gemm_segs.end());
+                jb.seg_end = (int32_t)segs.size();
+                jb.pad_ = g.nst;
+                push_tiles(recs2, (int32_t)jobs.size(), g.nst + 1.0);
+                jobs.push_back(jb);
+            } else {
+                // split-K: part p accumulates a contiguous range of segments into its own partial matrix;
+                // a final job adds the partials to sigma in part order (deterministic, no atomics)
+                const int ldp = (int)round_up2(OB.dr);
+                const int64_t psz = (int64_t)OB.dl * ldp;
+                size_t sbeg = 0;
+                int done = 0, nparts = 0;
+                std::vector<int64_t> part_off;
+                while (sbeg < gemm_segs.size()) {
+                    const double target = (double)g.nst * (nparts + 1) / nsplit;
+                    size_t send = sbeg;
+                    int pst = 0;
+                    while (send < gemm_segs.size() && (send == sbeg || done + pst < target)) {
+                        pst += (gemm_segs[send].K + GEMM_BK - 1) / GEMM_BK;
+                        send++;
+                    }
+                    Job pj;
+                    pj.c_off = ptop; pj.ldc = ldp; pj.M = OB.dl; pj.N = OB.dr;
+                    pj.flags = (SP_X << JOB_C_SPACE_SHIFT);
+                    pj.seg_begin = (int32_t)segs.size();
+                    segs.insert(segs.end(), gemm_segs.begin() + sbeg, gemm_segs.begin() + send);
+                    pj.seg_end = (int32_t)segs.size();
+                    pj.pad_ = pst;
+                    push_tiles(recs2, (int32_t)jobs.size(), pst + 1.0);
+                    jobs.push_back(pj);
+                    part_off.push_back(ptop);
+                    ptop += psz;
+                    done += pst;
+                    nparts++;
+                    sbeg = send;
+                }
+                jb.seg_begin = (int32_t)segs.size();
+                segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());
+                for (int64_t po : part_off) {
+                    Seg s;
+                    s.a_off = 0; s.lda = 0; s.b_off = po; s.ldb = ldp; s.K = OB.dl; s.alpha = 1.0;
+                    s.flags = SEG_A_IDENT | (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
+                    segs.push_back(s);
+                }
+                jb.seg_end = (int32_t)segs.size();
+                jb.pad_ = 0;
+                push_tiles(recs3, (int32_t)jobs.size(), 1.0);
+                jobs.push_back(jb);
+            }
+            DMRG_REQUIRE(segs.size() < ((size_t)1 << 31) && jobs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
+        }
+        ws_peak = std::max(ws_peak, ptop);
         emit_tiles(recs2, 2);
+        emit_tiles(recs3, 3);
     }
     P->stats[ST_ALG_FLOPS] = alg_flops;
     P->stats[ST_S1_FLOPS] = s1_flops;
@@ -415,6 +495,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
 
     // ---- upload ---------------------------------------------------------------------------------------
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
+    P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
+                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems);
+    if (S->structure_only) return DMRG_OK;
     auto up = [&](void** dptr, const void* src, size_t bytes) -> int {
         DMRG_CUDA(cudaMalloc(dptr, std::max<size_t>(bytes, 16)));
         if (bytes) DMRG_CUDA(cudaMemcpy(*dptr, src, bytes, cudaMemcpyHostToDevice));
@@ -427,8 +510,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     if ((rc = up((void**)&P->d_hd_items, hd_items.data(), hd_items.size() * sizeof(HdItem)))) return rc;
     if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
     DMRG_CUDA(cudaMalloc(&P->d_xws, sizeof(double) * (size_t)P->xws_elems));
-    P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
-                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems);
+    for (int v = 0; v < NUM_VARIANTS; v++) {
+        DMRG_CUDA(cudaStreamCreateWithFlags(&P->aux[v], cudaStreamNonBlocking));
+        DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_join[v], cudaEventDisableTiming));
+    }
+    DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
     return gemm_init();
 }
 
@@ -488,6 +574,11 @@ void dmrg_plan_destroy(dmrg_plan* P) {
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
     cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks);
     for (auto e : P->ev) cudaEventDestroy(e);
+    for (int v = 0; v < NUM_VARIANTS; v++) {
+        if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
+        if (P->ev_join[v]) cudaEventDestroy(P->ev_join[v]);
+    }
+    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
     if (P->dav) davidson_ws_free(P->dav);
     delete P;
 }
@@ -504,7 +595,7 @@ double dmrg_plan_stat(const dmrg_plan* P, int32_t key) { return (P && key >= 0 &
 int dmrg_plan_set_timing(dmrg_plan* P, int32_t enable) {
     if (!P) { set_error("dmrg_plan_set_timing: NULL plan"); return DMRG_EINVAL; }
     if (enable && P->ev.empty()) {
-        P->ev.resize(2 * P->launches.size() + 2);
+        P->ev.resize(2 * P->groups.size() + 2);
         for (auto& e : P->ev) DMRG_CUDA(cudaEventCreate(&e));
     }
     P->timing = enable != 0;
@@ -514,13 +605,16 @@ int dmrg_plan_set_timing(dmrg_plan* P, int32_t enable) {
 
 double dmrg_plan_stage_ms(dmrg_plan* P, int32_t which) {
     if (!P || !P->timing_valid) { set_error("dmrg_plan_stage_ms: no timed dmrg_sigma call"); return -1.0; }
-    const size_t nl = P->launches.size();
-    if (cudaEventSynchronize(P->ev[2 * nl + 1]) != cudaSuccess) { set_error("dmrg_plan_stage_ms: event sync failed"); return -1.0; }
+    const size_t ng = P->groups.size();
+    if (cudaEventSynchronize(P->ev[2 * ng + 1]) != cudaSuccess) { set_error("dmrg_plan_stage_ms: event sync failed"); return -1.0; }
     float ms = 0.f;
-    if (which == 2) { cudaEventElapsedTime(&ms, P->ev[2 * nl], P->ev[2 * nl + 1]); return ms; }
+    if (which == 2) { cudaEventElapsedTime(&ms, P->ev[2 * ng], P->ev[2 * ng + 1]); return ms; }
     double tot = 0.0;
-    for (size_t i = 0; i < nl; i++)
-        if (P->launches[i].stage == which + 1) { cudaEventElapsedTime(&ms, P->ev[2 * i], P->ev[2 * i + 1]); tot += ms; }
+    for (size_t i = 0; i < ng; i++)
+        if ((which == 0 && P->groups[i].stage == 1) || (which == 1 && P->groups[i].stage >= 2)) {
+            cudaEventElapsedTime(&ms, P->ev[2 * i], P->ev[2 * i + 1]);
+            tot += ms;
+        }
     return tot;
 }
 
@@ -528,19 +622,32 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
     if (!P || !psi || !sigma) { set_error("dmrg_sigma: NULL argument"); return DMRG_EINVAL; }
     if (((uintptr_t)psi & 15) || ((uintptr_t)sigma & 15)) { set_error("dmrg_sigma: psi and sigma must be 16-byte aligned"); return DMRG_EINVAL; }
     if (psi == sigma) { set_error("dmrg_sigma: psi and sigma must not alias"); return DMRG_EINVAL; }
+    if (P->ops->structure_only) { set_error("dmrg_sigma: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t nl = P->launches.size();
-    if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * nl], st));
+    const size_t ng = P->groups.size();
+    if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * ng], st));
     DMRG_CUDA(cudaMemsetAsync(sigma, 0, sizeof(double) * (size_t)P->psi_size, st));
-    for (size_t i = 0; i < nl; i++) {
-        const PlanLaunch& L = P->launches[i];
-        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * i], st));
-        int rc = launch_grouped_gemm(L.variant, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
-                                     P->ops->d_values, P->d_xws, psi, sigma, st);
-        if (rc != DMRG_OK) return rc;
-        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * i + 1], st));
+    for (size_t gi = 0; gi < ng; gi++) {
+        const PlanGroup& G = P->groups[gi];
+        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi], st));
+        // the launches of a group (one per tile variant) are independent: the first runs on the caller's
+        // stream, the others on side streams forked from / joined to it, so their tails overlap
+        if (G.nlaunch > 1) DMRG_CUDA(cudaEventRecord(P->ev_fork, st));
+        for (int li = 0; li < G.nlaunch; li++) {
+            const PlanLaunch& L = P->launches[G.first_launch + li];
+            cudaStream_t ls = li == 0 ? st : P->aux[li % NUM_VARIANTS];
+            if (li > 0) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
+            int rc = launch_grouped_gemm(L.variant, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
+                                         P->ops->d_values, P->d_xws, psi, sigma, ls);
+            if (rc != DMRG_OK) return rc;
+            if (li > 0) {
+                DMRG_CUDA(cudaEventRecord(P->ev_join[li % NUM_VARIANTS], ls));
+                DMRG_CUDA(cudaStreamWaitEvent(st, P->ev_join[li % NUM_VARIANTS], 0));
+            }
+        }
+        if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
     }
-    if (P->timing) { DMRG_CUDA(cudaEventRecord(P->ev[2 * nl + 1], st)); P->timing_valid = true; }
+    if (P->timing) { DMRG_CUDA(cudaEventRecord(P->ev[2 * ng + 1], st)); P->timing_valid = true; }
     return DMRG_OK;
 }
 
@@ -567,6 +674,7 @@ int dmrg_sigma_host(dmrg_plan* P, const double* psi_host, double* sigma_host, vo
 
 int dmrg_hdiag(dmrg_plan* P, double* diag, void* cuda_stream) {
     if (!P || !diag) { set_error("dmrg_hdiag: NULL argument"); return DMRG_EINVAL; }
+    if (P->ops->structure_only) { set_error("dmrg_hdiag: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int64_t YB = 32768;
     for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += YB) {

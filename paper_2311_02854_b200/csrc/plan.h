@@ -6,6 +6,7 @@ struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // of
 struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; };
 
 struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
+struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent
 
 enum {
     ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
@@ -24,13 +25,16 @@ struct dmrg_plan {
     double* d_xws = nullptr;
     int64_t xws_elems = 0;
     std::vector<PlanLaunch> launches;
+    std::vector<PlanGroup> groups;
+    cudaStream_t aux[dmrg::NUM_VARIANTS] = {nullptr};   // side streams: independent launches of a group overlap
+    cudaEvent_t ev_fork = nullptr, ev_join[dmrg::NUM_VARIANTS] = {nullptr};
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
     int64_t n_hd_blocks = 0;
     double stats[ST_COUNT] = {0};
     // optional per-stage timing
     bool timing = false;
-    std::vector<cudaEvent_t> ev;   // 2 per launch + 2
+    std::vector<cudaEvent_t> ev;   // 2 per group + 2
     bool timing_valid = false;
     DavidsonWs* dav = nullptr;
 };
