@@ -42,6 +42,8 @@ enum : uint32_t {
     SEG_A_IDENT   = 1u << 2,   // A is the identity: acc += alpha * B tile (no GEMM)
     SEG_A_VEC2    = 1u << 3,   // A operand 16-byte loadable (even offset, even ld)
     SEG_B_VEC2    = 1u << 4,
+    SEG_ALPHA_ONE = 1u << 5,   // alpha == +1 (set by the planner before upload)
+    SEG_ALPHA_NEG = 1u << 6,   // alpha == -1
     SEG_A_SPACE_SHIFT = 8,     // 2 bits
     SEG_B_SPACE_SHIFT = 10,    // 2 bits
 };
@@ -69,16 +71,18 @@ struct Job {
 };
 static_assert(sizeof(Job) == 40, "Job layout");
 
-// One CTA of work: tile (tm, tn) of job, tile shape fixed by the kernel variant
+// One CTA of work: rows [m0, m0+rows) x cols [n0, n0+cols) of job; rows <= BM, cols <= BN of the kernel
+// variant (the planner cuts a dimension into full pieces plus the remainder).
 struct Tile {
     int32_t  job;
-    uint16_t tm, tn;
+    int32_t  m0, n0;
+    uint16_t rows, cols;
 };
-static_assert(sizeof(Tile) == 8, "Tile layout");
+static_assert(sizeof(Tile) == 16, "Tile layout");
 
 // tile-shape variants of the grouped GEMM kernel
 struct TileShape { int bm, bn; };
-constexpr int NUM_VARIANTS = 4;
+constexpr int NUM_VARIANTS = 5;
 extern const TileShape kVariants[NUM_VARIANTS];
 constexpr int GEMM_BK = 16;
 

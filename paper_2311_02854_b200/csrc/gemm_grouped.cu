@@ -20,7 +20,7 @@
 
 namespace dmrg {
 
-const TileShape kVariants[NUM_VARIANTS] = {{64, 64}, {128, 64}, {32, 32}, {16, 16}};
+const TileShape kVariants[NUM_VARIANTS] = {{64, 64}, {128, 128}, {128, 32}, {32, 128}, {32, 32}};
 
 namespace {
 
@@ -33,9 +33,6 @@ __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int sr
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src, int src_bytes) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
@@ -43,6 +40,29 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 }
 
 struct StageMeta { double alpha; uint32_t flags; int32_t ksteps; };
+
+// ---- mbarrier helpers (shared::cta) ----------------------------------------------------------------
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+// arrive on `bar` once all cp.async issued so far by this thread have landed (counts against the init count)
+__device__ __forceinline__ void mbar_arrive_cp_async(uint32_t bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
 
 // fold alpha into the smaller fragment set; |alpha| = 1 flips the sign bit on the integer pipe
 // instead of spending an FP64 issue slot
@@ -59,64 +79,118 @@ __device__ __forceinline__ void scale_frags(double (&af)[FM], double (&bf)[FN], 
     }
 }
 
-// Stage one operand tile (MN x BK) of a segment into shared memory.
+// predicated cp.async: no instruction is issued when `on` is false
+__device__ __forceinline__ void cp_async16_if(uint32_t dst, const void* src, int src_bytes, bool on) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %3, 0;\n@p cp.async.cg.shared.global [%0], [%1], 16, %2;\n}\n" ::"r"(dst), "l"(src),
+                 "r"(src_bytes), "r"((int)on) : "memory");
+}
+__device__ __forceinline__ void cp_async8_if(uint32_t dst, const void* src, int src_bytes, bool on) {
+    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %3, 0;\n@p cp.async.ca.shared.global [%0], [%1], 8, %2;\n}\n" ::"r"(dst), "l"(src),
+                 "r"(src_bytes), "r"((int)on) : "memory");
+}
+
+// Stage one operand tile (MN x BK) of a segment into shared memory with NT producer threads.
 //   kcontig: global (mn,k) at g + mn*ld + k, shared at mn*KPAD + k
 //   else   : global (mn,k) at g + k*ld + mn, shared at k*(BMN+4) + mn
+// Elements outside [0, mn_lim) x [0, k_lim) are zero-filled (src-size 0); rows >= round_up(mn_lim, 8) and
+// k >= round_up(k_lim, 4) are never read by a fragment and are not copied at all.  Each thread keeps one fixed
+// position along the contiguous direction and walks the other with a constant pointer stride, so a copy costs
+// a 64-bit add, two compares and the LDGSTS -- the producer warp must not be the bottleneck.
 template <int BMN, int NT>
 __device__ __forceinline__ void load_operand(uint32_t sdst, const double* __restrict__ g, int ld, bool kcontig, bool vec2,
                                              int mn_lim, int k_lim, int tid) {
+    const int mn_end = (mn_lim + 7) & ~7, k_end = (k_lim + 3) & ~3;
     if (kcontig) {
         if (vec2) {
-            constexpr int PAIRS = BMN * (BK / 2);
+            constexpr int RPI = NT / (BK / 2), ITERS = BMN / RPI;   // rows per pass
+            const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
+            const int kb = k + 1 < k_lim ? 16 : (k < k_lim ? 8 : 0);
+            const bool lane_on = k < k_end;
+            const double* src = g + (int64_t)r0 * ld + k;
+            const int64_t step = (int64_t)RPI * ld;
+            const uint32_t dst = sdst + (r0 * KPAD + k) * 8;
 #pragma unroll
-            for (int p = tid; p < PAIRS; p += NT) {
-                const int mn = p / (BK / 2), k = (p % (BK / 2)) * 2;
-                const bool ok = mn < mn_lim && k < k_lim;
-                const int bytes = ok ? (k + 1 < k_lim ? 16 : 8) : 0;
-                const double* src = ok ? g + (int64_t)mn * ld + k : g;
-                cp_async16(sdst + (mn * KPAD + k) * 8, src, bytes);
+            for (int i = 0; i < ITERS; i++) {
+                const int row = r0 + RPI * i;
+                const bool in = row < mn_lim;
+                cp_async16_if(dst + i * RPI * KPAD * 8, in ? src : g, in ? kb : 0, lane_on && row < mn_end);
+                src += step;
             }
         } else {
-            constexpr int ELEMS = BMN * BK;
+            constexpr int RPI = NT / BK, ITERS = BMN / RPI;
+            const int r0 = tid / BK, k = tid % BK;
+            const int kb = k < k_lim ? 8 : 0;
+            const bool lane_on = k < k_end;
+            const double* src = g + (int64_t)r0 * ld + k;
+            const int64_t step = (int64_t)RPI * ld;
+            const uint32_t dst = sdst + (r0 * KPAD + k) * 8;
 #pragma unroll
-            for (int p = tid; p < ELEMS; p += NT) {
-                const int mn = p / BK, k = p % BK;
-                const bool ok = mn < mn_lim && k < k_lim;
-                const double* src = ok ? g + (int64_t)mn * ld + k : g;
-                cp_async8(sdst + (mn * KPAD + k) * 8, src, ok ? 8 : 0);
+            for (int i = 0; i < ITERS; i++) {
+                const int row = r0 + RPI * i;
+                const bool in = row < mn_lim;
+                cp_async8_if(dst + i * RPI * KPAD * 8, in ? src : g, in ? kb : 0, lane_on && row < mn_end);
+                src += step;
             }
         }
     } else {
         constexpr int MPAD = BMN + 4;
         if (vec2) {
-            constexpr int PAIRS = BK * (BMN / 2);
+            constexpr int PR = BMN / 2;                              // 16-byte pairs per k-row
+            constexpr int SEGS = PR > NT ? PR / NT : 1;              // passes needed to cover one k-row
+            constexpr int KPI = PR > NT ? 1 : NT / PR;               // k-rows per pass
+            const int k0 = tid / PR, mn0 = (tid % PR) * 2;
 #pragma unroll
-            for (int p = tid; p < PAIRS; p += NT) {
-                const int k = p / (BMN / 2), mn = (p % (BMN / 2)) * 2;
-                const bool ok = mn < mn_lim && k < k_lim;
-                const int bytes = ok ? (mn + 1 < mn_lim ? 16 : 8) : 0;
-                const double* src = ok ? g + (int64_t)k * ld + mn : g;
-                cp_async16(sdst + (k * MPAD + mn) * 8, src, bytes);
+            for (int sg = 0; sg < SEGS; sg++) {
+                const int mn = mn0 + sg * NT * 2;
+                const int mb = mn + 1 < mn_lim ? 16 : (mn < mn_lim ? 8 : 0);
+                const bool lane_on = mn < mn_end;
+                const double* src = g + (int64_t)k0 * ld + mn;
+                const int64_t step = (int64_t)KPI * ld;
+                const uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
+#pragma unroll
+                for (int i = 0; i < BK / KPI; i++) {
+                    const int k = k0 + KPI * i;
+                    const bool in = k < k_lim;
+                    cp_async16_if(dst + i * KPI * MPAD * 8, in ? src : g, in ? mb : 0, lane_on && k < k_end);
+                    src += step;
+                }
             }
         } else {
-            constexpr int ELEMS = BK * BMN;
+            constexpr int PR = BMN;
+            constexpr int SEGS = PR > NT ? PR / NT : 1;
+            constexpr int KPI = PR > NT ? 1 : NT / PR;
+            const int k0 = tid / PR, mn0 = tid % PR;
 #pragma unroll
-            for (int p = tid; p < ELEMS; p += NT) {
-                const int k = p / BMN, mn = p % BMN;
-                const bool ok = mn < mn_lim && k < k_lim;
-                const double* src = ok ? g + (int64_t)k * ld + mn : g;
-                cp_async8(sdst + (k * MPAD + mn) * 8, src, ok ? 8 : 0);
+            for (int sg = 0; sg < SEGS; sg++) {
+                const int mn = mn0 + sg * NT;
+                const int mb = mn < mn_lim ? 8 : 0;
+                const bool lane_on = mn < mn_end;
+                const double* src = g + (int64_t)k0 * ld + mn;
+                const int64_t step = (int64_t)KPI * ld;
+                const uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
+#pragma unroll
+                for (int i = 0; i < BK / KPI; i++) {
+                    const int k = k0 + KPI * i;
+                    const bool in = k < k_lim;
+                    cp_async8_if(dst + i * KPI * MPAD * 8, in ? src : g, in ? mb : 0, lane_on && k < k_end);
+                    src += step;
+                }
             }
         }
     }
 }
 
-template <int BM, int BN, int WM, int WN, int NST, int MINB>
-__global__ void __launch_bounds__(32 * WM * WN, MINB)
+// Warp-specialised kernel.  Warps 0 .. WM*WN-1 are CONSUMERS (LDS + DMMA only, one TM x TN warp tile
+// each); the last warp is the PRODUCER, which walks the job's segment list and issues every cp.async.
+// The two sides meet only through per-stage mbarriers (full: 32 cp.async-completion arrivals + 1
+// release arrival that publishes the stage metadata; empty: one arrival per consumer warp), so there
+// is no CTA-wide barrier in the main loop and the consumer warps drift freely against each other.
+template <int BM, int BN, int WM, int WN, int NST, int NPW, int MAXREG, bool DBUF>
+__global__ void __launch_bounds__(32 * (WM * WN + NPW)) __maxnreg__(MAXREG)
 grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, const Tile* __restrict__ tiles,
                     const double* __restrict__ ops, double* __restrict__ xws, const double* __restrict__ psi,
                     double* __restrict__ sigma) {
-    constexpr int NT = 32 * WM * WN;
+    constexpr int NCW = WM * WN;   // consumer warps
     constexpr int TM = BM / WM, TN = BN / WN;
     constexpr int FM = TM / 8, FN = TN / 8;
     constexpr int A_ELEMS = (BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4);
@@ -126,57 +200,41 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
 
     extern __shared__ __align__(16) double smem[];
     __shared__ StageMeta meta[NST];
+    __shared__ __align__(8) uint64_t bar_full[NST], bar_empty[NST];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wm0 = (warp / WN) * TM, wn0 = (warp % WN) * TN;
-    const int lr = lane >> 2, lc = lane & 3;
 
     const Tile tile = tiles[blockIdx.x];
     const Job job = jobs[tile.job];
-    const int m0 = tile.tm * BM, n0 = tile.tn * BN;
-    const int m_lim = job.M - m0, n_lim = job.N - n0;
-
-    // 8x8 fragments of this warp that intersect the matrix
-    const int fm_eff = max(0, min(FM, (m_lim - wm0 + 7) >> 3)), fn_eff = max(0, min(FN, (n_lim - wn0 + 7) >> 3));
-    const bool full_tile = fm_eff == FM && fn_eff == FN;
+    const int m0 = tile.m0, n0 = tile.n0;
+    const int m_lim = tile.rows, n_lim = tile.cols;   // <= BM, BN and inside the matrix (planner)
+    const int nstages = job.pad_;
     auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
-    double* const c_base = ((job.flags >> JOB_C_SPACE_SHIFT) & 3u) == SP_X ? xws : sigma;
 
-    double acc[FM][FN][2];
+    const uint32_t full_u32 = (uint32_t)__cvta_generic_to_shared(bar_full);
+    const uint32_t empty_u32 = (uint32_t)__cvta_generic_to_shared(bar_empty);
+    if (tid == 0) {
 #pragma unroll
-    for (int i = 0; i < FM; i++)
-#pragma unroll
-        for (int j = 0; j < FN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    // ---- identity-A segments (planner puts them first): acc += alpha * B tile ---------------------
-    int seg0 = job.seg_begin;
-    for (; seg0 < job.seg_end; seg0++) {
-        const Seg s = segs[seg0];
-        if (!(s.flags & SEG_A_IDENT)) break;
-        const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
-#pragma unroll
-        for (int i = 0; i < FM; i++) {
-            const int r = m0 + wm0 + 8 * i + lr;
-#pragma unroll
-            for (int j = 0; j < FN; j++) {
-                const int c = n0 + wn0 + 8 * j + 2 * lc;
-                if (r < job.M) {
-                    if (c < job.N) acc[i][j][0] = fma(s.alpha, b[(int64_t)r * s.ldb + c], acc[i][j][0]);
-                    if (c + 1 < job.N) acc[i][j][1] = fma(s.alpha, b[(int64_t)r * s.ldb + c + 1], acc[i][j][1]);
-                }
-            }
+        for (int s = 0; s < NST; s++) {
+            mbar_init(full_u32 + 8 * s, 32 * NPW + 1);
+            mbar_init(empty_u32 + 8 * s, NCW);
         }
     }
+    __syncthreads();   // the only CTA-wide barrier
 
-    // ---- pipelined GEMM over the remaining segments ------------------------------------------
-    const int nstages = job.pad_;
-    int lseg = seg0, lk0 = 0;
-    Seg ls;
-    if (lseg < job.seg_end) ls = segs[lseg];
-    const uint32_t smem_u32 = (uint32_t)__cvta_generic_to_shared(smem);
-
-    auto issue = [&](int slot) {
-        if (lseg < job.seg_end) {
+    if (warp >= NCW) {
+        // =============================== producer warp(s) ============================================
+        // NPW == 1: one warp stages A and B; NPW == 2 / 4: the first half of the producer warps stages A, the second half B
+        const int pw = warp - NCW;
+        int lseg = job.seg_begin;
+        while (lseg < job.seg_end && (segs[lseg].flags & SEG_A_IDENT)) lseg++;   // identity segments need no staging
+        if (lseg >= job.seg_end) return;
+        Seg ls = segs[lseg];
+        int lk0 = 0;
+        const uint32_t smem_u32 = (uint32_t)__cvta_generic_to_shared(smem);
+        for (int it = 0; it < nstages; it++) {
+            const int slot = it % NST;
+            if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
             const uint32_t sa = smem_u32 + slot * STAGE_ELEMS * 8;
             const uint32_t sb = sa + A_ELEMS * 8;
             const int k_lim = ls.K - lk0;
@@ -186,12 +244,16 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
                                (a_kc ? (int64_t)m0 * ls.lda + lk0 : (int64_t)lk0 * ls.lda + m0);
             const double* gb = space_r((ls.flags >> SEG_B_SPACE_SHIFT) & 3u) + ls.b_off +
                                (b_kc ? (int64_t)n0 * ls.ldb + lk0 : (int64_t)lk0 * ls.ldb + n0);
-            load_operand<BM, NT>(sa, ga, ls.lda, a_kc, (ls.flags & SEG_A_VEC2) != 0, m_lim, k_lim, tid);
-            load_operand<BN, NT>(sb, gb, ls.ldb, b_kc, (ls.flags & SEG_B_VEC2) != 0, n_lim, k_lim, tid);
-            if (tid == 0) {
+            constexpr int HP = NPW > 1 ? NPW / 2 : 1;   // producer warps per operand
+            const int ptid = (pw % HP) * 32 + lane;
+            if (NPW == 1 || pw < HP) load_operand<BM, 32 * HP>(sa, ga, ls.lda, a_kc, (ls.flags & SEG_A_VEC2) != 0, m_lim, k_lim, ptid);
+            if (NPW == 1 || pw >= HP) load_operand<BN, 32 * HP>(sb, gb, ls.ldb, b_kc, (ls.flags & SEG_B_VEC2) != 0, n_lim, k_lim, ptid);
+            mbar_arrive_cp_async(full_u32 + 8 * slot);
+            if (pw == 0 && lane == 0) {
                 meta[slot].alpha = ls.alpha;
                 meta[slot].flags = ls.flags;
                 meta[slot].ksteps = (min(k_lim, BK) + 3) >> 2;
+                mbar_arrive(full_u32 + 8 * slot);   // release: publishes meta[slot]
             }
             lk0 += BK;
             if (lk0 >= ls.K) {
@@ -200,74 +262,135 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
                 if (lseg < job.seg_end) ls = segs[lseg];
             }
         }
-        cp_async_commit();
-    };
+        return;
+    }
 
-#pragma unroll
-    for (int s = 0; s < NST - 1; s++) issue(s);
+    // =================================== consumer warps ================================================
+    // The tile's 8x8 fragments are dealt out evenly to the WM x WN consumer warps (a 56 x 48 tile gives the
+    // 2 x 2 warps 4+3 by 3+3 fragments, not 4+3 by 4+2): the stage buffers couple the warps of a CTA, so the
+    // CTA advances at the pace of its most loaded warp.
+    const int lr = lane >> 2, lc = lane & 3;
+    const int fr_m = (m_lim + 7) >> 3, fr_n = (n_lim + 7) >> 3;
+    const int per_m = (fr_m + WM - 1) / WM, per_n = (fr_n + WN - 1) / WN;
+    const int wm0 = (warp / WN) * per_m * 8, wn0 = (warp % WN) * per_n * 8;
+    const int fm_eff = max(0, min(per_m, fr_m - (warp / WN) * per_m)), fn_eff = max(0, min(per_n, fr_n - (warp % WN) * per_n));
+    const bool full_tile = fm_eff == FM && fn_eff == FN;
+    const bool any_frag = fm_eff > 0 && fn_eff > 0;
 
-    for (int it = 0; it < nstages; it++) {
-        cp_async_wait<NST - 2>();
-        __syncthreads();
-        issue((it + NST - 1) % NST);
-        const int slot = it % NST;
-        const double* sa = smem + slot * STAGE_ELEMS;
-        const double* sb = sa + A_ELEMS;
-        const StageMeta mt = meta[slot];
-        const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
-        const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
-        // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
-        const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
-        const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
-        const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
-        const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
-        const int mode = mt.alpha == 1.0 ? 0 : (mt.alpha == -1.0 ? 1 : 2);
-        if (full_tile) {
-            for (int kk = 0; kk < mt.ksteps; kk++) {
-                double af[FM], bf[FN];
+    double acc[FM][FN][2];
 #pragma unroll
-                for (int i = 0; i < FM; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
+    for (int i = 0; i < FM; i++)
 #pragma unroll
-                for (int j = 0; j < FN; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
-                if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
+        for (int j = 0; j < FN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    // ---- identity-A segments (planner puts them first): acc += alpha * B tile ---------------------
+    for (int sg = job.seg_begin; sg < job.seg_end; sg++) {
+        const Seg s = segs[sg];
+        if (!(s.flags & SEG_A_IDENT)) break;
+        const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
 #pragma unroll
-                for (int i = 0; i < FM; i++)
+        for (int i = 0; i < FM; i++) {
+            const int r = m0 + wm0 + 8 * i + lr;
 #pragma unroll
-                    for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-            }
-        } else {
-            // ragged tile: 8x8 fragments that lie entirely outside the matrix are skipped (warp-uniform
-            // predicates), so the executed work is padded to multiples of 8, not of the tile size
-            for (int kk = 0; kk < mt.ksteps; kk++) {
-                double af[FM], bf[FN];
-#pragma unroll
-                for (int i = 0; i < FM; i++) af[i] = i < fm_eff ? pa[8 * i * a_sm + 4 * kk * a_sk] : 0.0;
-#pragma unroll
-                for (int j = 0; j < FN; j++) bf[j] = j < fn_eff ? pb[8 * j * b_sn + 4 * kk * b_sk] : 0.0;
-                if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
-#pragma unroll
-                for (int i = 0; i < FM; i++)
-#pragma unroll
-                    for (int j = 0; j < FN; j++)
-                        if (i < fm_eff && j < fn_eff) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+            for (int j = 0; j < FN; j++) {
+                const int c = n0 + wn0 + 8 * j + 2 * lc;
+                if (i < fm_eff && j < fn_eff && r < m0 + m_lim) {
+                    if (c < n0 + n_lim) acc[i][j][0] = fma(s.alpha, b[(int64_t)r * s.ldb + c], acc[i][j][0]);
+                    if (c + 1 < n0 + n_lim) acc[i][j][1] = fma(s.alpha, b[(int64_t)r * s.ldb + c + 1], acc[i][j][1]);
+                }
             }
         }
     }
-    cp_async_wait<0>();
+
+    // ---- main loop: wait for a full stage, LDS + DMMA, release it ---------------------------------
+    for (int it = 0; it < nstages; it++) {
+        const int slot = it % NST;
+        mbar_wait(full_u32 + 8 * slot, (it / NST) & 1);
+        if (any_frag) {
+            const double* sa = smem + slot * STAGE_ELEMS;
+            const double* sb = sa + A_ELEMS;
+            const StageMeta mt = meta[slot];
+            const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
+            const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
+            // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
+            const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
+            const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
+            const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
+            const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
+            const int mode = (mt.flags & SEG_ALPHA_ONE) ? 0 : ((mt.flags & SEG_ALPHA_NEG) ? 1 : 2);   // integer test: no FP64-pipe DSETP
+            const int ksteps = mt.ksteps;
+            if (full_tile && DBUF) {
+                // fragments of k-step kk+1 are fetched while the DMMAs of k-step kk issue
+                double af[2][FM], bf[2][FN];
+#pragma unroll
+                for (int i = 0; i < FM; i++) af[0][i] = pa[8 * i * a_sm];
+#pragma unroll
+                for (int j = 0; j < FN; j++) bf[0][j] = pb[8 * j * b_sn];
+#pragma unroll
+                for (int kk = 0; kk < BK / 4; kk++) {
+                    if (kk < ksteps) {
+                        if (kk + 1 < BK / 4 && kk + 1 < ksteps) {
+#pragma unroll
+                            for (int i = 0; i < FM; i++) af[(kk + 1) & 1][i] = pa[8 * i * a_sm + 4 * (kk + 1) * a_sk];
+#pragma unroll
+                            for (int j = 0; j < FN; j++) bf[(kk + 1) & 1][j] = pb[8 * j * b_sn + 4 * (kk + 1) * b_sk];
+                        }
+                        if (mode != 0) scale_frags<FM, FN>(af[kk & 1], bf[kk & 1], mode, mt.alpha);
+#pragma unroll
+                        for (int i = 0; i < FM; i++)
+#pragma unroll
+                            for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[kk & 1][i], bf[kk & 1][j]);
+                    }
+                }
+            } else if (full_tile) {
+                for (int kk = 0; kk < ksteps; kk++) {
+                    double af[FM], bf[FN];
+#pragma unroll
+                    for (int i = 0; i < FM; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
+#pragma unroll
+                    for (int j = 0; j < FN; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
+                    if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
+#pragma unroll
+                    for (int i = 0; i < FM; i++)
+#pragma unroll
+                        for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+                }
+            } else {
+                // ragged tile: 8x8 fragments that lie entirely outside the tile are skipped (warp-uniform
+                // predicates), so the executed work is padded to multiples of 8, not of the tile size
+                for (int kk = 0; kk < ksteps; kk++) {
+                    double af[FM], bf[FN];
+#pragma unroll
+                    for (int i = 0; i < FM; i++) af[i] = i < fm_eff ? pa[8 * i * a_sm + 4 * kk * a_sk] : 0.0;
+#pragma unroll
+                    for (int j = 0; j < FN; j++) bf[j] = j < fn_eff ? pb[8 * j * b_sn + 4 * kk * b_sk] : 0.0;
+                    if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
+#pragma unroll
+                    for (int i = 0; i < FM; i++)
+#pragma unroll
+                        for (int j = 0; j < FN; j++)
+                            if (i < fm_eff && j < fn_eff) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+                }
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty_u32 + 8 * slot);
+    }
 
     // ---- epilogue: C = beta*C + acc ---------------------------------------------------------------
     const bool beta1 = (job.flags & JOB_BETA1) != 0;
-    double* c = c_base + job.c_off;
+    double* c = (((job.flags >> JOB_C_SPACE_SHIFT) & 3u) == SP_X ? xws : sigma) + job.c_off;
 #pragma unroll
     for (int i = 0; i < FM; i++) {
         const int r = m0 + wm0 + 8 * i + lr;
-        if (r >= job.M) continue;
+        if (i >= fm_eff || r >= m0 + m_lim) continue;
 #pragma unroll
         for (int j = 0; j < FN; j++) {
+            if (j >= fn_eff) continue;
             const int col = n0 + wn0 + 8 * j + 2 * lc;
             double* p = c + (int64_t)r * job.ldc + col;
-            if (col < job.N) p[0] = beta1 ? p[0] + acc[i][j][0] : acc[i][j][0];
-            if (col + 1 < job.N) p[1] = beta1 ? p[1] + acc[i][j][1] : acc[i][j][1];
+            if (col < n0 + n_lim) p[0] = beta1 ? p[0] + acc[i][j][0] : acc[i][j][0];
+            if (col + 1 < n0 + n_lim) p[1] = beta1 ? p[1] + acc[i][j][1] : acc[i][j][1];
         }
     }
 }
@@ -278,21 +401,27 @@ constexpr size_t smem_bytes(int nst) {
            (((BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4)) + ((BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4)));
 }
 
-// variant table: must match kVariants
-#define V0 grouped_gemm_kernel<64, 64, 2, 2, 3, 3>
-#define V1 grouped_gemm_kernel<128, 64, 4, 2, 3, 1>
-#define V2 grouped_gemm_kernel<32, 32, 2, 2, 4, 6>
-#define V3 grouped_gemm_kernel<16, 16, 1, 1, 4, 16>
+// variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, producer warps, register cap, double-buffered fragments>
+// Every variant but V1 uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step) with double-buffered fragments.
+#define V0 grouped_gemm_kernel<64, 64, 2, 2, 3, 1, 128, true>      // general blocks, 3 CTAs/SM
+#define V1 grouped_gemm_kernel<128, 128, 4, 4, 4, 4, 96, false>    // large blocks, least operand traffic, 1 CTA/SM
+#define V2 grouped_gemm_kernel<128, 32, 4, 1, 3, 1, 128, true>     // skinny N (stage 1 with a small R' sector)
+#define V3 grouped_gemm_kernel<32, 128, 1, 4, 3, 1, 128, true>     // skinny M
+#define V4 grouped_gemm_kernel<32, 32, 1, 1, 4, 1, 128, true>      // tiny blocks: one consumer warp
+constexpr int V0_T = 160, V1_T = 640, V2_T = 160, V3_T = 160, V4_T = 64;
+constexpr size_t V0_S = smem_bytes<64, 64>(3), V1_S = smem_bytes<128, 128>(4), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
+                 V4_S = smem_bytes<32, 32>(4);
 
 }  // namespace
 
 int gemm_init() {
     static bool done = false;
     if (done) return DMRG_OK;
-    DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<64, 64>(3)));
-    DMRG_CUDA(cudaFuncSetAttribute(V1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<128, 64>(3)));
-    DMRG_CUDA(cudaFuncSetAttribute(V2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<32, 32>(4)));
-    DMRG_CUDA(cudaFuncSetAttribute(V3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes<16, 16>(4)));
+    DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V1_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V2_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V3_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V4, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V4_S));
     done = true;
     return DMRG_OK;
 }
@@ -302,10 +431,11 @@ int launch_grouped_gemm(int variant, const Job* jobs, const Seg* segs, const Til
     if (ntiles <= 0) return DMRG_OK;
     const unsigned g = (unsigned)ntiles;
     switch (variant) {
-        case 0: V0<<<g, 128, smem_bytes<64, 64>(3), st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 1: V1<<<g, 256, smem_bytes<128, 64>(3), st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 2: V2<<<g, 128, smem_bytes<32, 32>(4), st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 3: V3<<<g, 32, smem_bytes<16, 16>(4), st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 0: V0<<<g, V0_T, V0_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 1: V1<<<g, V1_T, V1_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 2: V2<<<g, V2_T, V2_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 3: V3<<<g, V3_T, V3_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 4: V4<<<g, V4_T, V4_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
     DMRG_CUDA(cudaGetLastError());

@@ -14,6 +14,7 @@
 // Terms are processed in chunks sized so the X intermediates fit the workspace.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <new>
 #include <unordered_map>
 
@@ -38,18 +39,30 @@ static inline int64_t xkey(int64_t r_off, int r_trans, int in_blk, int64_t nblk)
     return (r_off * 2 + r_trans) * nblk + in_blk;
 }
 
-// Tile variant for an M x N output: the largest tile shape whose tiles are at least ~60 % inside the
-// matrix.  With fragment skipping every variant executes the same ceil(M/8)*ceil(N/8) fragments per
-// k-step, so the choice trades operand re-use (large tiles) against occupancy for small blocks.
+// Tile variant for an M x N output.  With fragment skipping every variant executes the same
+// ceil(M/8)*ceil(N/8) DMMA fragments per k-step, so the choice is about occupancy and operand traffic:
+// skinny outputs get skinny tiles (all warps busy), everything else the 64x64 tile at 3 CTAs/SM; the
+// 128x128 tile (half the operand traffic, but one CTA per SM, so ragged edges idle its warps) is used
+// only when enabled and the output fills its tiles.
+// Tuning knob: DMRG_VARIANT_MASK = bit mask of allowed variants (default 0b11101: no 128x128).
 static int choose_variant(int M, int N) {
-    static const int pref[NUM_VARIANTS] = {1, 0, 2, 3};   // 128x64, 64x64, 32x32, 16x16
-    for (int t = 0; t < NUM_VARIANTS; t++) {
-        const int v = pref[t];
-        const double bm = kVariants[v].bm, bn = kVariants[v].bn;
-        const double util = (double)M * N / (std::ceil(M / bm) * std::ceil(N / bn) * bm * bn);
-        if (util >= 0.6) return v;
+    static const int mask = [] { const char* e = getenv("DMRG_VARIANT_MASK"); const int m = e ? atoi(e) : 0; return (m & 31) ? (m & 31) | 1 : 29; }();
+    auto ok = [&](int v) { return (mask >> v) & 1; };
+    if (ok(4) && M <= 32 && N <= 32) return 4;
+    if (ok(2) && N <= 32 && M > 32) return 2;
+    if (ok(3) && M <= 32 && N > 32) return 3;
+    if (ok(1)) {
+        const double util = (double)M * N / (std::ceil(M / 128.0) * std::ceil(N / 128.0) * 16384.0);
+        if (util >= 0.75) return 1;
     }
-    return NUM_VARIANTS - 1;
+    return 0;
+}
+
+// cut a dimension d into full pieces of B plus the remainder.  (Equal-sized pieces were tried and lost: they
+// push every tile onto the kernel's ragged path, and the full-tile path is the fast one.)
+static void cut_dim(int d, int B, std::vector<std::pair<int, int>>& out) {
+    out.clear();
+    for (int o = 0; o < d; o += B) out.push_back({o, std::min(B, d - o)});
 }
 
 static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N + 7) / 8); }
@@ -243,6 +256,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     std::vector<Seg> segs;
     std::vector<Tile> tiles;
     std::vector<std::vector<HdItem>> hd(nblk);
+    std::vector<RedJob> reds;   // split-K reductions (stage 3)
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0;
     int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
 
@@ -262,7 +276,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
                 i += n;
             }
-            (stage == 1 ? s1_tiles : s2_tiles) += (stage == 3 ? 0 : (int64_t)r.size());
+            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)r.size();
         }
         grp.nlaunch = (int)P->launches.size() - grp.first_launch;
         if (grp.nlaunch > 0) P->groups.push_back(grp);
@@ -290,6 +304,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         std::unordered_map<int64_t, XLoc> xloc;
         xloc.reserve(req.size() * 2);
         std::vector<TileRec> recs1[NUM_VARIANTS];
+        std::vector<std::pair<int, int>> cut_m, cut_n;
         int64_t xtop = 0;
         for (size_t i = 0; i < req.size();) {
             size_t j = i + 1;
@@ -319,11 +334,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             segs.push_back(s);
             const int v = choose_variant(jb.M, jb.N);
             const int bm = kVariants[v].bm, bn = kVariants[v].bn;
-            const int ntm = (jb.M + bm - 1) / bm, ntn = (jb.N + bn - 1) / bn;
-            DMRG_REQUIRE(ntm < 65536 && ntn < 65536, "dmrg_plan_create: too many tiles in one job");
             const double kpad4 = 4.0 * ((dRi + 3) / 4);
-            for (int a = 0; a < ntm; a++)
-                for (int b = 0; b < ntn; b++) recs1[v].push_back({{(int32_t)jobs.size(), (uint16_t)a, (uint16_t)b}, kpad4});
+            cut_dim(jb.M, bm, cut_m);
+            cut_dim(jb.N, bn, cut_n);
+            for (auto& a : cut_m)
+                for (auto& b : cut_n)
+                    recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
             padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
             s1_flops += 2.0 * rows * dRi * dRo;
             alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
@@ -355,7 +371,6 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             const int v = choose_variant(OB.dl, OB.dr);
             const int bm = kVariants[v].bm, bn = kVariants[v].bn;
             Group g{i, j, v, (OB.dl + bm - 1) / bm, (OB.dr + bn - 1) / bn, nst};
-            DMRG_REQUIRE(g.ntm < 65536 && g.ntn < 65536, "dmrg_plan_create: too many tiles in one job");
             // cost in units of 64x64x16 tile-stages
             tile_stages += (double)g.ntm * g.ntn * nst * (bm * bn / 4096.0);
             groups.push_back(g);
@@ -364,7 +379,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         // A tile's K-loop is the critical path of the launch: cap it at 1/kSplitWaves of the time the
         // whole launch would take on a perfectly balanced machine, but never below kMinSplitStages.
         const double smax = std::max<double>(kMinSplitStages, tile_stages / (kCtaSlots * kSplitWaves));
-        std::vector<TileRec> recs2[NUM_VARIANTS], recs3[NUM_VARIANTS];
+        std::vector<TileRec> recs2[NUM_VARIANTS];
+        const size_t red_begin = reds.size();
         int64_t ptop = xtop;   // split-K partial tiles live behind the X intermediates
         std::vector<Seg> ident_segs, gemm_segs;
         for (const Group& g : groups) {
@@ -408,9 +424,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
+            cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
+            cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
-                for (int a = 0; a < g.ntm; a++)
-                    for (int b = 0; b < g.ntn; b++) recs[g.variant].push_back({{job_id, (uint16_t)a, (uint16_t)b}, cost});
+                for (auto& a : cut_m)
+                    for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
             };
             Job jb;
             jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
@@ -430,7 +448,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 const int64_t psz = (int64_t)OB.dl * ldp;
                 size_t sbeg = 0;
                 int done = 0, nparts = 0;
-                std::vector<int64_t> part_off;
+                std::vector<int64_t> part_off;   // consecutive: part p lives at part_off[0] + p * psz
                 while (sbeg < gemm_segs.size()) {
                     const double target = (double)g.nst * (nparts + 1) / nsplit;
                     size_t send = sbeg;
@@ -443,6 +461,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     pj.c_off = ptop; pj.ldc = ldp; pj.M = OB.dl; pj.N = OB.dr;
                     pj.flags = (SP_X << JOB_C_SPACE_SHIFT);
                     pj.seg_begin = (int32_t)segs.size();
+                    if (nparts == 0) segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());   // identity-L terms ride with part 0
                     segs.insert(segs.end(), gemm_segs.begin() + sbeg, gemm_segs.begin() + send);
                     pj.seg_end = (int32_t)segs.size();
                     pj.pad_ = pst;
@@ -454,31 +473,20 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     nparts++;
                     sbeg = send;
                 }
-                jb.seg_begin = (int32_t)segs.size();
-                segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());
-                for (int64_t po : part_off) {
-                    Seg s;
-                    s.a_off = 0; s.lda = 0; s.b_off = po; s.ldb = ldp; s.K = OB.dl; s.alpha = 1.0;
-                    s.flags = SEG_A_IDENT | (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
-                    segs.push_back(s);
-                }
-                jb.seg_end = (int32_t)segs.size();
-                jb.pad_ = 0;
-                push_tiles(recs3, (int32_t)jobs.size(), 1.0);
-                jobs.push_back(jb);
+                reds.push_back({OB.offset, part_off[0], psz, OB.dl, OB.dr, ldp, nparts});
             }
             DMRG_REQUIRE(segs.size() < ((size_t)1 << 31) && jobs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
         }
         ws_peak = std::max(ws_peak, ptop);
         emit_tiles(recs2, 2);
-        emit_tiles(recs3, 3);
+        if (reds.size() > red_begin) P->groups.push_back({3, (int)red_begin, (int)(reds.size() - red_begin)});
     }
     P->stats[ST_ALG_FLOPS] = alg_flops;
     P->stats[ST_S1_FLOPS] = s1_flops;
     P->stats[ST_S2_FLOPS] = s2_flops;
     P->stats[ST_PADDED_FLOPS] = padded_flops;
     P->stats[ST_S1_JOBS] = (double)s1_jobs;
-    P->stats[ST_LAUNCHES] = (double)P->launches.size();
+    P->stats[ST_LAUNCHES] = (double)P->launches.size() + (double)std::count_if(P->groups.begin(), P->groups.end(), [](const PlanGroup& g) { return g.stage == 3; });
     P->stats[ST_ALG_BYTES] = alg_bytes + 8.0 * P->psi_size;
     P->stats[ST_S1_TILES] = (double)s1_tiles;
     P->stats[ST_S2_TILES] = (double)s2_tiles;
@@ -503,10 +511,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         if (bytes) DMRG_CUDA(cudaMemcpy(*dptr, src, bytes, cudaMemcpyHostToDevice));
         return DMRG_OK;
     };
+    for (Seg& sg : segs) sg.flags |= sg.alpha == 1.0 ? SEG_ALPHA_ONE : (sg.alpha == -1.0 ? SEG_ALPHA_NEG : 0u);
     int rc;
     if ((rc = up((void**)&P->d_jobs, jobs.data(), jobs.size() * sizeof(Job)))) return rc;
     if ((rc = up((void**)&P->d_segs, segs.data(), segs.size() * sizeof(Seg)))) return rc;
     if ((rc = up((void**)&P->d_tiles, tiles.data(), tiles.size() * sizeof(Tile)))) return rc;
+    if ((rc = up((void**)&P->d_reds, reds.data(), reds.size() * sizeof(RedJob)))) return rc;
     if ((rc = up((void**)&P->d_hd_items, hd_items.data(), hd_items.size() * sizeof(HdItem)))) return rc;
     if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
     DMRG_CUDA(cudaMalloc(&P->d_xws, sizeof(double) * (size_t)P->xws_elems));
@@ -516,6 +526,20 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     }
     DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
     return gemm_init();
+}
+
+// sigma_blk += sum_p partial_p, parts added in order (the deterministic end of split-K)     grid (chunks, jobs)
+__global__ void __launch_bounds__(256) splitk_reduce_kernel(const RedJob* __restrict__ reds, const double* __restrict__ xws,
+                                                            double* __restrict__ sigma) {
+    const RedJob r = reds[blockIdx.y];
+    const int64_t n = (int64_t)r.M * r.N;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / r.N), j = (int)(e - (int64_t)i * r.N);
+        const double* p = xws + r.part_off + (int64_t)i * r.ldp + j;
+        double acc = sigma[r.sigma_off + e];
+        for (int k = 0; k < r.nparts; k++) acc += p[(int64_t)k * r.part_stride];
+        sigma[r.sigma_off + e] = acc;
+    }
 }
 
 // Hd[blk][i][j] = sum_items alpha * (L ? L[i][i] : 1) * (R ? R[j][j] : 1)     one thread per element
@@ -572,7 +596,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_reds);
     for (auto e : P->ev) cudaEventDestroy(e);
     for (int v = 0; v < NUM_VARIANTS; v++) {
         if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
@@ -632,6 +656,15 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi], st));
         // the launches of a group (one per tile variant) are independent: the first runs on the caller's
         // stream, the others on side streams forked from / joined to it, so their tails overlap
+        if (G.stage == 3) {   // first_launch / nlaunch index the reduction table here
+            for (int y0 = 0; y0 < G.nlaunch; y0 += 32768) {
+                const unsigned ny = (unsigned)std::min(32768, G.nlaunch - y0);
+                splitk_reduce_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_reds + G.first_launch + y0, P->d_xws, sigma);
+            }
+            DMRG_CUDA(cudaGetLastError());
+            if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
+            continue;
+        }
         if (G.nlaunch > 1) DMRG_CUDA(cudaEventRecord(P->ev_fork, st));
         for (int li = 0; li < G.nlaunch; li++) {
             const PlanLaunch& L = P->launches[G.first_launch + li];

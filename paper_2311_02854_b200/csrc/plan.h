@@ -5,8 +5,10 @@
 struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // offsets < 0: identity factor
 struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; };
 
+struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
+
 struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
-struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent
+struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent (stage 3: range of the RedJob table)
 
 enum {
     ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
@@ -28,6 +30,7 @@ struct dmrg_plan {
     std::vector<PlanGroup> groups;
     cudaStream_t aux[dmrg::NUM_VARIANTS] = {nullptr};   // side streams: independent launches of a group overlap
     cudaEvent_t ev_fork = nullptr, ev_join[dmrg::NUM_VARIANTS] = {nullptr};
+    RedJob* d_reds = nullptr;
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
     int64_t n_hd_blocks = 0;
