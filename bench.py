@@ -124,10 +124,8 @@ def oracle_sample(pr, psi, total_flops, seconds):
 
 
 def dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
+    from paper_2311_02854_b200 import replicas
+    return replicas.dist_env()
 
 
 def run_reference(args):
@@ -184,9 +182,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU path)")
     torch.cuda.set_device(local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2311_02854_b200 import replicas
+    replicas.init("nccl", torch.device("cuda", local))
     stream = torch.cuda.current_stream()
 
     t0 = time.perf_counter()
@@ -212,10 +209,7 @@ def main():
     peak_dfma = g.fp64_peak_tflops(0, 300.0, stream)
 
     def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
+        replicas.barrier(torch.cuda.synchronize)
 
     # ---- warm-up: W Davidson iterations (allocates the Davidson workspace) ---------------------
     W, K = max(args.warmup, 3), args.steps
@@ -240,13 +234,9 @@ def main():
     s1_ms, s2_ms, call_ms = plan.stage_ms()   # per-launch CUDA events of the last H psi of the timed region
     plan.set_timing(False)
     assert res["iters"] == K
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
-    ms_step = ms_total / K
     flops = st["canon_flops"]
-    value = world * flops / (ms_step * 1e-3) * 1e-12
+    thr, ms_step = replicas.job_throughput(flops, ms_total / K, world, "cuda")   # max over ranks
+    value = thr * 1e-12
 
     # ---- kernel-only H psi (no Davidson vector work) and the roofline of the GEMM kernel --------
     ts = []
@@ -317,6 +307,7 @@ def main():
     plan.destroy()
     ops.free()
     if world > 1:
+        import torch.distributed as dist
         dist.destroy_process_group()
 
 
