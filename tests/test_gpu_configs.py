@@ -117,7 +117,8 @@ def test_direct_configs_sampled_parity(name, budget):
     ref, st = oracle.opair_sigma(pr, psi, only_out=blocks, return_stats=True)
     assert st["tasks"] > 0
     assert _block_err(pr, s_psi, ref, blocks) / nrm <= TOL_SIGMA
-    small = blocks[:1]                                                 # the smallest block: cheap second oracle call
+    lay = np.asarray(pr.layout)
+    small = [int(np.argmin(lay[:, 4] * lay[:, 5]))]                    # the smallest block: cheap second oracle call
     ref_x = oracle.opair_sigma(pr, xn, only_out=small)
     assert _block_err(pr, hx, ref_x, small) / np.linalg.norm(hx) <= TOL_SIGMA
     s = plan.stats()
