@@ -33,7 +33,7 @@ def make_blocked_problem(K, nL, N_tot, twoSz_tot=0, D=None, seed=1, banded=False
     return pr
 
 
-def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False, ints=None):
+def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False, ints=None, structure_only=False):
     """Direct fill (cfg 3-5; DESIGN.md input recipe): integrals and the term table are the real ones,
     the sector tables follow the d_max(D) model of sectors.py, and every charge-allowed operator block
     is filled with seeded N(0, 1/d_max) entries (H, B_pp, Q_pp symmetric).  The contraction workload
@@ -45,7 +45,8 @@ def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False,
     secR = block_sector_model(K - nL - 2, K, N_tot, twoSz_tot, D)
     tt = TermTable(part, ints)
     dmax = max(max(s[2] for s in secL), max(s[2] for s in secR))
-    pr = assemble(tt, secL, secR, None, N_tot, twoSz_tot, direct_seed=seed + 104729, direct_scale=dmax ** -0.5)
+    pr = assemble(tt, secL, secR, None, N_tot, twoSz_tot, direct_seed=None if structure_only else seed + 104729,
+                  direct_scale=dmax ** -0.5)
     pr.meta = dict(K=K, nL=nL, nR=K - nL - 2, D=D, seed=seed, mode="direct", banded=banded)
     pr.ints, pr.part, pr.tt = ints, part, tt
     return pr

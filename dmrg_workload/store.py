@@ -128,7 +128,9 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
         op_id[op] = len(ops_rows)
         ops_rows.append((0 if op.side == "L" else 1, KIND[op.kind], op.p, op.q, dq[0], dq[1],
                          first, len(blk_rows) - first))
-    if block_values is None:
+    if block_values is None and direct_seed is None:
+        values = None   # structure only (sizing / planning without the 8-byte-per-element store)
+    elif block_values is None:
         values = np.empty(off, dtype=np.float64)
         _fill_normal(values, int(direct_seed))
         if direct_scale != 1.0:

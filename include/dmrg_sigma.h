@@ -136,7 +136,9 @@ int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host
  *  4 executed flops including tile padding                     5 stage-1 GEMM jobs   6 chunks
  *  7 kernel launches per sigma   8 device bytes held by the plan (descriptors + workspace)
  *  9 algorithmic operand bytes read per sigma (operator blocks once per use + X write/read + psi/sigma)
- * 10 stage-1 tiles   11 stage-2 tiles   12 canonical flops (= key 1 without de-duplication)        */
+ * 10 stage-1 tiles   11 stage-2 tiles   12 canonical flops (= key 1 without de-duplication)
+ * 13 executed flops with every segment's K padded to whole 16-wide pipeline stages
+ * 14 the same with M and N padded to whole tiles as well                                           */
 double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
 
 /* ---------------------------------------------------------------------------------------------

@@ -180,6 +180,136 @@ __device__ __forceinline__ void load_operand(uint32_t sdst, const double* __rest
     }
 }
 
+// One pipeline stage of one consumer warp: up to BK/4 k-steps of FMe x FNe DMMA fragments (the top-left part of
+// the warp's FM x FN accumulator grid).  With DBUF the fragments of k-step kk+1 are fetched while the DMMAs of
+// k-step kk issue (two k-steps per loop trip, so the buffer index is static).
+template <int FM, int FN, int FMe, int FNe, bool DBUF>
+__device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const double* __restrict__ pa, const double* __restrict__ pb,
+                                              int a_sm, int a_sk, int b_sn, int b_sk, int ksteps, int mode, double alpha) {
+    static_assert(FM <= 4 && FN <= 4, "ragged-tile dispatch covers up to 4 x 4 fragments per warp");
+    auto load = [&](double (&af)[FMe], double (&bf)[FNe], int kk) {
+#pragma unroll
+        for (int i = 0; i < FMe; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
+#pragma unroll
+        for (int j = 0; j < FNe; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
+    };
+    auto mma = [&](double (&af)[FMe], double (&bf)[FNe]) {
+        if (mode != 0) scale_frags<FMe, FNe>(af, bf, mode, alpha);
+#pragma unroll
+        for (int i = 0; i < FMe; i++)
+#pragma unroll
+            for (int j = 0; j < FNe; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+    };
+    if (DBUF) {
+        double a0[FMe], b0[FNe], a1[FMe], b1[FNe];
+        load(a0, b0, 0);
+#pragma unroll 1
+        for (int kk = 0; kk < ksteps; kk += 2) {
+            const bool two = kk + 1 < ksteps;
+            if (two) load(a1, b1, kk + 1);
+            mma(a0, b0);
+            if (two) {
+                if (kk + 2 < ksteps) load(a0, b0, kk + 2);
+                mma(a1, b1);
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int kk = 0; kk < ksteps; kk++) {
+            double a0[FMe], b0[FNe];
+            load(a0, b0, kk);
+            mma(a0, b0);
+        }
+    }
+}
+
+struct ConsumerCtx {
+    const Job* job; const Seg* segs; const double* ops; double* xws; const double* psi; double* sigma;
+    const double* smem; const StageMeta* meta; uint32_t full_u32, empty_u32;
+    int m0, n0, m_lim, n_lim, nstages, lane, wm0, wn0, fm_eff, fn_eff;
+};
+
+// Everything one consumer warp does for one tile, with FMe x FNe accumulator fragments (<= the 4 x 4 of a 32x32
+// warp tile): identity-A segments, the mbarrier-paced main loop, the epilogue.  Fragments (i, j) with
+// i >= fm_eff or j >= fn_eff (a warp ragged in both directions keeps all its columns) are computed on
+// zero-filled or neighbouring data and never stored.
+template <int BM, int BN, int NST, int FMe, int FNe, bool DBUF>
+__device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
+    constexpr int A_ELEMS = (BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4);
+    constexpr int B_ELEMS = (BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4);
+    constexpr int STAGE_ELEMS = A_ELEMS + B_ELEMS;
+    const Job& job = *cx.job;
+    const int lane = cx.lane, lr = lane >> 2, lc = lane & 3;
+    const int m0 = cx.m0, n0 = cx.n0, wm0 = cx.wm0, wn0 = cx.wn0;
+    const int fm_eff = cx.fm_eff, fn_eff = cx.fn_eff;
+    const bool any_frag = fm_eff > 0 && fn_eff > 0;
+    auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? cx.ops : (sp == SP_X ? cx.xws : (sp == SP_PSI ? cx.psi : cx.sigma)); };
+
+    double acc[FMe][FNe][2];
+#pragma unroll
+    for (int i = 0; i < FMe; i++)
+#pragma unroll
+        for (int j = 0; j < FNe; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    // ---- identity-A segments (planner puts them first): acc += alpha * B tile ---------------------
+    for (int sg = job.seg_begin; sg < job.seg_end; sg++) {
+        const Seg s = cx.segs[sg];
+        if (!(s.flags & SEG_A_IDENT)) break;
+        const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
+#pragma unroll
+        for (int i = 0; i < FMe; i++) {
+            const int r = m0 + wm0 + 8 * i + lr;
+#pragma unroll
+            for (int j = 0; j < FNe; j++) {
+                const int c = n0 + wn0 + 8 * j + 2 * lc;
+                if (i < fm_eff && j < fn_eff && r < m0 + cx.m_lim) {
+                    if (c < n0 + cx.n_lim) acc[i][j][0] = fma(s.alpha, b[(int64_t)r * s.ldb + c], acc[i][j][0]);
+                    if (c + 1 < n0 + cx.n_lim) acc[i][j][1] = fma(s.alpha, b[(int64_t)r * s.ldb + c + 1], acc[i][j][1]);
+                }
+            }
+        }
+    }
+
+    // ---- main loop: wait for a full stage, LDS + DMMA, release it ---------------------------------
+    for (int it = 0; it < cx.nstages; it++) {
+        const int slot = it % NST;
+        mbar_wait(cx.full_u32 + 8 * slot, (it / NST) & 1);
+        if (any_frag) {
+            const double* sa = cx.smem + slot * STAGE_ELEMS;
+            const double* sb = sa + A_ELEMS;
+            const StageMeta mt = cx.meta[slot];
+            const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
+            const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
+            // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
+            const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
+            const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
+            const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
+            const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
+            const int mode = (mt.flags & SEG_ALPHA_ONE) ? 0 : ((mt.flags & SEG_ALPHA_NEG) ? 1 : 2);   // integer test: no FP64-pipe DSETP
+            compute_stage<FMe, FNe, FMe, FNe, DBUF>(acc, pa, pb, a_sm, a_sk, b_sn, b_sk, mt.ksteps, mode, mt.alpha);
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(cx.empty_u32 + 8 * slot);
+    }
+
+    // ---- epilogue: C = beta*C + acc ---------------------------------------------------------------
+    const bool beta1 = (job.flags & JOB_BETA1) != 0;
+    double* c = (((job.flags >> JOB_C_SPACE_SHIFT) & 3u) == SP_X ? cx.xws : cx.sigma) + job.c_off;
+#pragma unroll
+    for (int i = 0; i < FMe; i++) {
+        const int r = m0 + wm0 + 8 * i + lr;
+        if (i >= fm_eff || r >= m0 + cx.m_lim) continue;
+#pragma unroll
+        for (int j = 0; j < FNe; j++) {
+            if (j >= fn_eff) continue;
+            const int col = n0 + wn0 + 8 * j + 2 * lc;
+            double* p = c + (int64_t)r * job.ldc + col;
+            if (col < n0 + cx.n_lim) p[0] = beta1 ? p[0] + acc[i][j][0] : acc[i][j][0];
+            if (col + 1 < n0 + cx.n_lim) p[1] = beta1 ? p[1] + acc[i][j][1] : acc[i][j][1];
+        }
+    }
+}
+
 // Warp-specialised kernel.  Warps 0 .. WM*WN-1 are CONSUMERS (LDS + DMMA only, one TM x TN warp tile
 // each); the last warp is the PRODUCER, which walks the job's segment list and issues every cp.async.
 // The two sides meet only through per-stage mbarriers (full: 32 cp.async-completion arrivals + 1
@@ -267,130 +397,32 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
 
     // =================================== consumer warps ================================================
     // The tile's 8x8 fragments are dealt out evenly to the WM x WN consumer warps (a 56 x 48 tile gives the
-    // 2 x 2 warps 4+3 by 3+3 fragments, not 4+3 by 4+2): the stage buffers couple the warps of a CTA, so the
-    // CTA advances at the pace of its most loaded warp.
-    const int lr = lane >> 2, lc = lane & 3;
+    // 2 x 2 warps 4+3 by 3+3 fragments): the stage buffers couple the warps of a CTA, so the CTA advances at
+    // the pace of its most loaded warp.
+    ConsumerCtx cx;
+    cx.job = &job; cx.segs = segs; cx.ops = ops; cx.xws = xws; cx.psi = psi; cx.sigma = sigma;
+    cx.smem = smem; cx.meta = meta; cx.full_u32 = full_u32; cx.empty_u32 = empty_u32;
+    cx.m0 = m0; cx.n0 = n0; cx.m_lim = m_lim; cx.n_lim = n_lim; cx.nstages = nstages; cx.lane = lane;
     const int fr_m = (m_lim + 7) >> 3, fr_n = (n_lim + 7) >> 3;
     const int per_m = (fr_m + WM - 1) / WM, per_n = (fr_n + WN - 1) / WN;
-    const int wm0 = (warp / WN) * per_m * 8, wn0 = (warp % WN) * per_n * 8;
-    const int fm_eff = max(0, min(per_m, fr_m - (warp / WN) * per_m)), fn_eff = max(0, min(per_n, fr_n - (warp % WN) * per_n));
-    const bool full_tile = fm_eff == FM && fn_eff == FN;
-    const bool any_frag = fm_eff > 0 && fn_eff > 0;
-
-    double acc[FM][FN][2];
-#pragma unroll
-    for (int i = 0; i < FM; i++)
-#pragma unroll
-        for (int j = 0; j < FN; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
-
-    // ---- identity-A segments (planner puts them first): acc += alpha * B tile ---------------------
-    for (int sg = job.seg_begin; sg < job.seg_end; sg++) {
-        const Seg s = segs[sg];
-        if (!(s.flags & SEG_A_IDENT)) break;
-        const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
-#pragma unroll
-        for (int i = 0; i < FM; i++) {
-            const int r = m0 + wm0 + 8 * i + lr;
-#pragma unroll
-            for (int j = 0; j < FN; j++) {
-                const int c = n0 + wn0 + 8 * j + 2 * lc;
-                if (i < fm_eff && j < fn_eff && r < m0 + m_lim) {
-                    if (c < n0 + n_lim) acc[i][j][0] = fma(s.alpha, b[(int64_t)r * s.ldb + c], acc[i][j][0]);
-                    if (c + 1 < n0 + n_lim) acc[i][j][1] = fma(s.alpha, b[(int64_t)r * s.ldb + c + 1], acc[i][j][1]);
-                }
-            }
+    cx.wm0 = (warp / WN) * per_m * 8; cx.wn0 = (warp % WN) * per_n * 8;
+    cx.fm_eff = max(0, min(per_m, fr_m - (warp / WN) * per_m));
+    cx.fn_eff = max(0, min(per_n, fr_n - (warp % WN) * per_n));
+    // The whole consumer body (accumulators, main loop, epilogue) is specialised on the number of fragment rows
+    // OR columns of this warp, so a partly filled tile costs in proportion to its fragments.  (Specialising on
+    // both counts at once made ptxas spill; a warp ragged in both directions pads its columns to the warp tile.)
+    if (cx.fm_eff == FM || cx.fm_eff == 0) {
+        switch (cx.fn_eff) {
+            case 1: consumer_body<BM, BN, NST, FM, 1, DBUF>(cx); break;
+            case 2: if constexpr (FN >= 2) consumer_body<BM, BN, NST, FM, 2, DBUF>(cx); break;
+            case 3: if constexpr (FN >= 3) consumer_body<BM, BN, NST, FM, 3, DBUF>(cx); break;
+            default: consumer_body<BM, BN, NST, FM, FN, DBUF>(cx); break;   // full warp tile, or a warp with no fragment
         }
-    }
-
-    // ---- main loop: wait for a full stage, LDS + DMMA, release it ---------------------------------
-    for (int it = 0; it < nstages; it++) {
-        const int slot = it % NST;
-        mbar_wait(full_u32 + 8 * slot, (it / NST) & 1);
-        if (any_frag) {
-            const double* sa = smem + slot * STAGE_ELEMS;
-            const double* sb = sa + A_ELEMS;
-            const StageMeta mt = meta[slot];
-            const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
-            const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
-            // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
-            const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
-            const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
-            const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
-            const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
-            const int mode = (mt.flags & SEG_ALPHA_ONE) ? 0 : ((mt.flags & SEG_ALPHA_NEG) ? 1 : 2);   // integer test: no FP64-pipe DSETP
-            const int ksteps = mt.ksteps;
-            if (full_tile && DBUF) {
-                // fragments of k-step kk+1 are fetched while the DMMAs of k-step kk issue
-                double af[2][FM], bf[2][FN];
-#pragma unroll
-                for (int i = 0; i < FM; i++) af[0][i] = pa[8 * i * a_sm];
-#pragma unroll
-                for (int j = 0; j < FN; j++) bf[0][j] = pb[8 * j * b_sn];
-#pragma unroll
-                for (int kk = 0; kk < BK / 4; kk++) {
-                    if (kk < ksteps) {
-                        if (kk + 1 < BK / 4 && kk + 1 < ksteps) {
-#pragma unroll
-                            for (int i = 0; i < FM; i++) af[(kk + 1) & 1][i] = pa[8 * i * a_sm + 4 * (kk + 1) * a_sk];
-#pragma unroll
-                            for (int j = 0; j < FN; j++) bf[(kk + 1) & 1][j] = pb[8 * j * b_sn + 4 * (kk + 1) * b_sk];
-                        }
-                        if (mode != 0) scale_frags<FM, FN>(af[kk & 1], bf[kk & 1], mode, mt.alpha);
-#pragma unroll
-                        for (int i = 0; i < FM; i++)
-#pragma unroll
-                            for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[kk & 1][i], bf[kk & 1][j]);
-                    }
-                }
-            } else if (full_tile) {
-                for (int kk = 0; kk < ksteps; kk++) {
-                    double af[FM], bf[FN];
-#pragma unroll
-                    for (int i = 0; i < FM; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
-#pragma unroll
-                    for (int j = 0; j < FN; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
-                    if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
-#pragma unroll
-                    for (int i = 0; i < FM; i++)
-#pragma unroll
-                        for (int j = 0; j < FN; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-                }
-            } else {
-                // ragged tile: 8x8 fragments that lie entirely outside the tile are skipped (warp-uniform
-                // predicates), so the executed work is padded to multiples of 8, not of the tile size
-                for (int kk = 0; kk < ksteps; kk++) {
-                    double af[FM], bf[FN];
-#pragma unroll
-                    for (int i = 0; i < FM; i++) af[i] = i < fm_eff ? pa[8 * i * a_sm + 4 * kk * a_sk] : 0.0;
-#pragma unroll
-                    for (int j = 0; j < FN; j++) bf[j] = j < fn_eff ? pb[8 * j * b_sn + 4 * kk * b_sk] : 0.0;
-                    if (mode != 0) scale_frags<FM, FN>(af, bf, mode, mt.alpha);
-#pragma unroll
-                    for (int i = 0; i < FM; i++)
-#pragma unroll
-                        for (int j = 0; j < FN; j++)
-                            if (i < fm_eff && j < fn_eff) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
-                }
-            }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(empty_u32 + 8 * slot);
-    }
-
-    // ---- epilogue: C = beta*C + acc ---------------------------------------------------------------
-    const bool beta1 = (job.flags & JOB_BETA1) != 0;
-    double* c = (((job.flags >> JOB_C_SPACE_SHIFT) & 3u) == SP_X ? xws : sigma) + job.c_off;
-#pragma unroll
-    for (int i = 0; i < FM; i++) {
-        const int r = m0 + wm0 + 8 * i + lr;
-        if (i >= fm_eff || r >= m0 + m_lim) continue;
-#pragma unroll
-        for (int j = 0; j < FN; j++) {
-            if (j >= fn_eff) continue;
-            const int col = n0 + wn0 + 8 * j + 2 * lc;
-            double* p = c + (int64_t)r * job.ldc + col;
-            if (col < n0 + n_lim) p[0] = beta1 ? p[0] + acc[i][j][0] : acc[i][j][0];
-            if (col + 1 < n0 + n_lim) p[1] = beta1 ? p[1] + acc[i][j][1] : acc[i][j][1];
+    } else {
+        switch (cx.fm_eff) {
+            case 1: consumer_body<BM, BN, NST, 1, FN, DBUF>(cx); break;
+            case 2: if constexpr (FM >= 2) consumer_body<BM, BN, NST, 2, FN, DBUF>(cx); break;
+            default: if constexpr (FM >= 3) consumer_body<BM, BN, NST, 3, FN, DBUF>(cx); break;
         }
     }
 }

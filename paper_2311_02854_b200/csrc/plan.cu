@@ -257,7 +257,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     std::vector<Tile> tiles;
     std::vector<std::vector<HdItem>> hd(nblk);
     std::vector<RedJob> reds;   // split-K reductions (stage 3)
-    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0;
+    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0;
     int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
 
     auto psi_vec2 = [&](const dmrg_psi_block& B) { return (B.offset % 2 == 0) && (B.dr % 2 == 0); };
@@ -341,6 +341,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 for (auto& b : cut_n)
                     recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
             padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
+            stage_flops += 2.0 * frag_area(jb.M, jb.N) * 16.0 * jb.pad_;
+            tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * 16.0 * jb.pad_;
             s1_flops += 2.0 * rows * dRi * dRo;
             alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
             jobs.push_back(jb);
@@ -422,6 +424,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
             }
             padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
+            stage_flops += 2.0 * frag_area(OB.dl, OB.dr) * 16.0 * g.nst;
+            tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * 16.0 * g.nst;
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
             cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
@@ -485,6 +489,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     P->stats[ST_S1_FLOPS] = s1_flops;
     P->stats[ST_S2_FLOPS] = s2_flops;
     P->stats[ST_PADDED_FLOPS] = padded_flops;
+    P->stats[ST_STAGE_FLOPS] = stage_flops;   // K padded to whole 16-wide stages per segment
+    P->stats[ST_TILE_FLOPS] = tile_flops;     // ... and M, N padded to whole tiles: what a fill-independent tile time costs
     P->stats[ST_S1_JOBS] = (double)s1_jobs;
     P->stats[ST_LAUNCHES] = (double)P->launches.size() + (double)std::count_if(P->groups.begin(), P->groups.end(), [](const PlanGroup& g) { return g.stage == 3; });
     P->stats[ST_ALG_BYTES] = alg_bytes + 8.0 * P->psi_size;
