@@ -40,7 +40,7 @@ def parse():
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="X workspace (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=20.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--cpu-seconds", type=float, default=8.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
 

@@ -138,7 +138,8 @@ int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host
  *  9 algorithmic operand bytes read per sigma (operator blocks once per use + X write/read + psi/sigma)
  * 10 stage-1 tiles   11 stage-2 tiles   12 canonical flops (= key 1 without de-duplication)
  * 13 executed flops with every segment's K padded to whole 16-wide pipeline stages
- * 14 the same with M and N padded to whole tiles as well                                           */
+ * 14 the same with M and N padded to whole tiles as well; 15 ... padded to each tile's most loaded warp
+ *                                           */
 double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
 
 /* ---------------------------------------------------------------------------------------------

@@ -24,7 +24,7 @@ assert SECTOR_DT.itemsize == 12 and OP_DT.itemsize == 40 and BLOCK_DT.itemsize =
 assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
 
 STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
-             "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops")
+             "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops")
 
 EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_destroy",
            "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",

@@ -434,14 +434,28 @@ constexpr size_t smem_bytes(int nst) {
 }
 
 // variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, producer warps, register cap, double-buffered fragments>
-// Every variant but V1 uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step) with double-buffered fragments.
-#define V0 grouped_gemm_kernel<64, 64, 2, 2, 3, 1, 128, true>      // general blocks, 3 CTAs/SM
+// Every variant uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step).  V0 was tuned on the B200 (macros kept
+// for re-tuning): 2 stages x 96 registers -> 4 CTAs/SM beat 3 stages x 128 registers with double-buffered
+// fragments -> 3 CTAs/SM by 0-7 % (cfg 5 / cfg 4); 4 stages (2 CTAs/SM) and a second producer warp both lost ~10 %.
+#ifndef V0_NST
+#define V0_NST 2
+#endif
+#ifndef V0_REG
+#define V0_REG 96
+#endif
+#ifndef V0_DBUF
+#define V0_DBUF false
+#endif
+#ifndef V0_NPW
+#define V0_NPW 1
+#endif
+#define V0 grouped_gemm_kernel<64, 64, 2, 2, V0_NST, V0_NPW, V0_REG, V0_DBUF>
 #define V1 grouped_gemm_kernel<128, 128, 4, 4, 4, 4, 96, false>    // large blocks, least operand traffic, 1 CTA/SM
 #define V2 grouped_gemm_kernel<128, 32, 4, 1, 3, 1, 128, true>     // skinny N (stage 1 with a small R' sector)
 #define V3 grouped_gemm_kernel<32, 128, 1, 4, 3, 1, 128, true>     // skinny M
 #define V4 grouped_gemm_kernel<32, 32, 1, 1, 4, 1, 128, true>      // tiny blocks: one consumer warp
-constexpr int V0_T = 160, V1_T = 640, V2_T = 160, V3_T = 160, V4_T = 64;
-constexpr size_t V0_S = smem_bytes<64, 64>(3), V1_S = smem_bytes<128, 128>(4), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
+constexpr int V0_T = 32 * (4 + V0_NPW), V1_T = 640, V2_T = 160, V3_T = 160, V4_T = 64;
+constexpr size_t V0_S = smem_bytes<64, 64>(V0_NST), V1_S = smem_bytes<128, 128>(4), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
                  V4_S = smem_bytes<32, 32>(4);
 
 }  // namespace

@@ -65,6 +65,18 @@ static void cut_dim(int d, int B, std::vector<std::pair<int, int>>& out) {
     for (int o = 0; o < d; o += B) out.push_back({o, std::min(B, d - o)});
 }
 
+// fragments a tile costs when every consumer warp is charged the load of the most loaded one (WM x WN warps)
+static inline double warp_area(const std::vector<std::pair<int, int>>& cm, const std::vector<std::pair<int, int>>& cn, int v) {
+    const int wm = kVariants[v].bm / 32, wn = kVariants[v].bn / 32;
+    double a = 0;
+    for (auto& m : cm)
+        for (auto& n : cn) {
+            const int fm = (m.second + 7) / 8, fn = (n.second + 7) / 8;
+            a += 64.0 * wm * wn * ((fm + wm - 1) / wm) * ((fn + wn - 1) / wn);
+        }
+    return a;
+}
+
 static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N + 7) / 8); }
 
 struct TileRec { Tile t; double cost; };
@@ -257,7 +269,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     std::vector<Tile> tiles;
     std::vector<std::vector<HdItem>> hd(nblk);
     std::vector<RedJob> reds;   // split-K reductions (stage 3)
-    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0;
+    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
     int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
 
     auto psi_vec2 = [&](const dmrg_psi_block& B) { return (B.offset % 2 == 0) && (B.dr % 2 == 0); };
@@ -342,6 +354,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
             padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
             stage_flops += 2.0 * frag_area(jb.M, jb.N) * 16.0 * jb.pad_;
+            warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * 16.0 * jb.pad_;
             tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * 16.0 * jb.pad_;
             s1_flops += 2.0 * rows * dRi * dRo;
             alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
@@ -423,13 +436,14 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 (ident ? ident_segs : gemm_segs).push_back(s);
                 if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
             }
+            cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
+            cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
             padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
             stage_flops += 2.0 * frag_area(OB.dl, OB.dr) * 16.0 * g.nst;
+            warp_flops += 2.0 * warp_area(cut_m, cut_n, g.variant) * 16.0 * g.nst;
             tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * 16.0 * g.nst;
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
-            cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
-            cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
                 for (auto& a : cut_m)
                     for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
@@ -490,6 +504,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     P->stats[ST_S2_FLOPS] = s2_flops;
     P->stats[ST_PADDED_FLOPS] = padded_flops;
     P->stats[ST_STAGE_FLOPS] = stage_flops;   // K padded to whole 16-wide stages per segment
+    P->stats[ST_WARP_FLOPS] = warp_flops;     // ... M, N padded to the most loaded warp of each tile
     P->stats[ST_TILE_FLOPS] = tile_flops;     // ... and M, N padded to whole tiles: what a fill-independent tile time costs
     P->stats[ST_S1_JOBS] = (double)s1_jobs;
     P->stats[ST_LAUNCHES] = (double)P->launches.size() + (double)std::count_if(P->groups.begin(), P->groups.end(), [](const PlanGroup& g) { return g.stage == 3; });
@@ -506,6 +521,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         hd_blocks[b].item_end = (int32_t)hd_items.size();
     }
     P->n_hd_blocks = nblk;
+    std::vector<HdTile> hd_tiles;
+    for (int64_t b = 0; b < nblk; b++)
+        for (int ti = 0; ti < (P->blocks[b].dl + 31) / 32; ti++)
+            for (int tj = 0; tj < (P->blocks[b].dr + 31) / 32; tj++) hd_tiles.push_back({(int32_t)b, (int16_t)ti, (int16_t)tj});
+    P->n_hd_tiles = (int64_t)hd_tiles.size();
 
     // ---- upload ---------------------------------------------------------------------------------------
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
@@ -525,6 +545,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     if ((rc = up((void**)&P->d_reds, reds.data(), reds.size() * sizeof(RedJob)))) return rc;
     if ((rc = up((void**)&P->d_hd_items, hd_items.data(), hd_items.size() * sizeof(HdItem)))) return rc;
     if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
+    if ((rc = up((void**)&P->d_hd_tiles, hd_tiles.data(), hd_tiles.size() * sizeof(HdTile)))) return rc;
     DMRG_CUDA(cudaMalloc(&P->d_xws, sizeof(double) * (size_t)P->xws_elems));
     for (int v = 0; v < NUM_VARIANTS; v++) {
         DMRG_CUDA(cudaStreamCreateWithFlags(&P->aux[v], cudaStreamNonBlocking));
@@ -548,21 +569,40 @@ __global__ void __launch_bounds__(256) splitk_reduce_kernel(const RedJob* __rest
     }
 }
 
-// Hd[blk][i][j] = sum_items alpha * (L ? L[i][i] : 1) * (R ? R[j][j] : 1)     one thread per element
-__global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ blocks, const HdItem* __restrict__ items,
-                                                    const double* __restrict__ ops, double* __restrict__ diag) {
-    const HdBlock b = blocks[blockIdx.y];
-    const int64_t n = (int64_t)b.dl * b.dr;
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
-        const int i = (int)(e / b.dr), j = (int)(e - (int64_t)i * b.dr);
-        double acc = 0.0;
-        for (int it = b.item_begin; it < b.item_end; it++) {
-            const HdItem h = items[it];
-            const double l = h.l_off >= 0 ? ops[h.l_off + (int64_t)i * h.ldl + i] : 1.0;
-            const double r = h.r_off >= 0 ? ops[h.r_off + (int64_t)j * h.ldr + j] : 1.0;
-            acc = fma(h.alpha, l * r, acc);
+// Hd[blk][i][j] = sum_items alpha * (L ? L[i][i] : 1) * (R ? R[j][j] : 1), items in plan order.
+// One CTA per 32 x 32 tile of a block: the diagonals of 32 items at a time are staged in shared memory
+// (2 x 32 values per item instead of two global reads per element and item), then every thread
+// accumulates its 4 elements -- a rank-(number of items) update, deterministic.
+__global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ blocks, const HdTile* __restrict__ tiles,
+                                                    const HdItem* __restrict__ items, const double* __restrict__ ops,
+                                                    double* __restrict__ diag) {
+    __shared__ double sl[32][33], sr[32][33], sa[32];
+    const HdTile t = tiles[blockIdx.x];
+    const HdBlock b = blocks[t.blk];
+    const int i0 = t.ti * 32, j0 = t.tj * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;   // ty 0..7
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int base = b.item_begin; base < b.item_end; base += 32) {
+        const int nit = min(32, b.item_end - base);
+        __syncthreads();
+        for (int q = ty; q < nit; q += 8) {   // item q: lane tx fetches L[i0+tx][i0+tx] and R[j0+tx][j0+tx]
+            const HdItem h = items[base + q];
+            const int i = i0 + tx, j = j0 + tx;
+            sl[q][tx] = (h.l_off >= 0 && i < b.dl) ? ops[h.l_off + (int64_t)i * h.ldl + i] : 1.0;
+            sr[q][tx] = (h.r_off >= 0 && j < b.dr) ? ops[h.r_off + (int64_t)j * h.ldr + j] : 1.0;
+            if (tx == 0) sa[q] = h.alpha;
         }
-        diag[b.offset + e] = acc;
+        __syncthreads();
+        for (int q = 0; q < nit; q++) {
+            const double r = sa[q] * sr[q][tx];
+#pragma unroll
+            for (int u = 0; u < 4; u++) acc[u] = fma(sl[q][ty + 8 * u], r, acc[u]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < 4; u++) {
+        const int i = i0 + ty + 8 * u, j = j0 + tx;
+        if (i < b.dl && j < b.dr) diag[b.offset + (int64_t)i * b.dr + j] = acc[u];
     }
 }
 
@@ -602,7 +642,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_reds);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds);
     for (auto e : P->ev) cudaEventDestroy(e);
     for (int v = 0; v < NUM_VARIANTS; v++) {
         if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
@@ -715,11 +755,8 @@ int dmrg_hdiag(dmrg_plan* P, double* diag, void* cuda_stream) {
     if (!P || !diag) { set_error("dmrg_hdiag: NULL argument"); return DMRG_EINVAL; }
     if (P->ops->structure_only) { set_error("dmrg_hdiag: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int64_t YB = 32768;
-    for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += YB) {
-        const unsigned ny = (unsigned)std::min<int64_t>(YB, P->n_hd_blocks - y0);
-        hdiag_kernel<<<dim3(16, ny), 256, 0, st>>>(P->d_hd_blocks + y0, P->d_hd_items, P->ops->d_values, diag);
-    }
+    if (P->n_hd_tiles > 0)
+        hdiag_kernel<<<(unsigned)P->n_hd_tiles, 256, 0, st>>>(P->d_hd_blocks, P->d_hd_tiles, P->d_hd_items, P->ops->d_values, diag);
     DMRG_CUDA(cudaGetLastError());
     return DMRG_OK;
 }

@@ -3,6 +3,7 @@
 #include "common.h"
 
 struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // offsets < 0: identity factor
+struct HdTile { int32_t blk; int16_t ti, tj; };   // 32 x 32 tile of a psi block
 struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; };
 
 struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
@@ -12,7 +13,7 @@ struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one
 
 enum {
     ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
-    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_COUNT
+    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_WARP_FLOPS, ST_COUNT
 };
 
 struct DavidsonWs;
@@ -34,6 +35,8 @@ struct dmrg_plan {
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
     int64_t n_hd_blocks = 0;
+    HdTile* d_hd_tiles = nullptr;
+    int64_t n_hd_tiles = 0;
     double stats[ST_COUNT] = {0};
     // optional per-stage timing
     bool timing = false;
