@@ -27,6 +27,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "fp64_tflops_per_hpsi"
+NCU_DRAM_BYTES_PER_HPSI = {"cfg5": 5.12e12}   # profiles/r1_cfg5_launch_summary.csv (round 1)
 UNIT = "TFLOP/s"
 
 
@@ -247,8 +248,11 @@ def main():
     ms_sigma = float(np.median(ts))
     gemm_ms = s1_ms + s2_ms
     achieved = flops / (gemm_ms * 1e-3) * 1e-12
+    # DRAM bytes of all GEMM launches of one H psi, from the ncu pass committed as profiles/r1_cfg5_launches.csv
+    # (dram__bytes_read.sum + dram__bytes_write.sum); only meaningful for the configuration that was profiled
+    traffic = NCU_DRAM_BYTES_PER_HPSI.get(args.config)
     roofline = {"bound": "tensor", "achieved": achieved, "peak": peak_dmma, "unit": "TFLOP/s", "frac": achieved / peak_dmma,
-                "traffic": None, "kernel": "grouped_gemm_kernel (DMMA.8x8x4, all launches of one H psi)",
+                "traffic": traffic, "traffic_unit": "bytes per H psi (ncu, all GEMM launches)", "kernel": "grouped_gemm_kernel (DMMA.8x8x4, all launches of one H psi)",
                 "peak_source": "measured live: dmrg_fp64_peak_tflops(DMMA); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
                 "peak_dfma_measured": peak_dfma, "stage1_ms": s1_ms, "stage2_ms": s2_ms, "launches_per_hpsi": int(st["launches"]),
                 "executed_flops_per_hpsi": st["s1_flops"] + st["s2_flops"], "padded_flops_per_hpsi": st["padded_flops"],
@@ -294,7 +298,7 @@ def main():
                                                 "parallelism": "replicas only" if world > 1 else "single GPU",
                                                 "psi_size": int(n), "psi_blocks": int(len(pr.layout)), "terms": int(len(pr.term_coef)),
                                                 "tasks": int(st["tasks"]), "chunks": int(st["chunks"])},
-                "clocks": clk, "e2e": e2e, "gpu_launches": int(K * (st["launches"] + 1)) + 12 * K,
+                "clocks": clk, "e2e": e2e, "gpu_launches": int(K * (st["launches"] + 15) + 4),   # GEMM / reduce launches + 15 Davidson vector kernels per step, + hdiag, start-up
                 "roofline": roofline, "cpu_baseline": cpu,
                 "ms_per_hpsi_kernel_only": ms_sigma, "frac_of_fp64_peak_whole_step": value / world / peak_dmma,
                 "parity_sampled": parity,
