@@ -92,7 +92,7 @@ struct GemmLaunch {       // one launch of one kernel variant
     int64_t ntiles;
 };
 
-int launch_grouped_gemm(int variant, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+int launch_grouped_gemm(int variant, int cluster, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
                         const double* ops, double* xws, const double* psi, double* sigma, cudaStream_t st);
 int gemm_init();   // sets shared-memory attributes once
 

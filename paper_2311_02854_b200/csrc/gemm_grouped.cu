@@ -335,6 +335,7 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     const Tile tile = tiles[blockIdx.x];
+    if (tile.job < 0) return;   // padding of a thread-block cluster (whole CTA leaves before any barrier)
     const Job job = jobs[tile.job];
     const int m0 = tile.m0, n0 = tile.n0;
     const int m_lim = tile.rows, n_lim = tile.cols;   // <= BM, BN and inside the matrix (planner)
@@ -472,19 +473,42 @@ int gemm_init() {
     return DMRG_OK;
 }
 
-int launch_grouped_gemm(int variant, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+template <typename K>
+static cudaError_t launch_one(K kernel, unsigned grid, int threads, size_t smem, int cluster, cudaStream_t st, const Job* jobs, const Seg* segs,
+                              const Tile* tiles, const double* ops, double* xws, const double* psi, double* sigma) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    if (cluster > 1) {
+        // sibling tiles of one output block (they share A row panels / B column panels) are launched as one
+        // thread-block cluster: co-scheduled, they walk the same K-loop in step and meet in L2
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = cluster;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+    }
+    return cudaLaunchKernelEx(&cfg, kernel, jobs, segs, tiles, ops, xws, psi, sigma);
+}
+
+int launch_grouped_gemm(int variant, int cluster, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
                         const double* ops, double* xws, const double* psi, double* sigma, cudaStream_t st) {
     if (ntiles <= 0) return DMRG_OK;
     const unsigned g = (unsigned)ntiles;
+    cudaError_t e;
     switch (variant) {
-        case 0: V0<<<g, V0_T, V0_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 1: V1<<<g, V1_T, V1_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 2: V2<<<g, V2_T, V2_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 3: V3<<<g, V3_T, V3_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 4: V4<<<g, V4_T, V4_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 0: e = launch_one(V0, g, V0_T, V0_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 1: e = launch_one(V1, g, V1_T, V1_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 2: e = launch_one(V2, g, V2_T, V2_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 3: e = launch_one(V3, g, V3_T, V3_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 4: e = launch_one(V4, g, V4_T, V4_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
-    DMRG_CUDA(cudaGetLastError());
+    if (e != cudaSuccess) { set_error("launch_grouped_gemm: variant %d, %lld tiles, cluster %d: %s", variant, (long long)ntiles, cluster, cudaGetErrorString(e)); return DMRG_ECUDA; }
     return DMRG_OK;
 }
 

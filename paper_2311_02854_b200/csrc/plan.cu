@@ -82,9 +82,13 @@ static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N
 struct TileRec { Tile t; double cost; };
 
 // split-K policy of stage 2 (see the comment at its use)
-constexpr double kCtaSlots = 148.0 * 3;     // resident 64x64 CTAs on a B200
-constexpr double kSplitWaves = 8.0;
-constexpr double kMinSplitStages = 32.0;    // K = 512
+constexpr double kCtaSlots = 148.0 * 4;     // resident 64x64 CTAs on a B200
+static const double kSplitWaves = [] { const char* e = getenv("DMRG_SPLIT_WAVES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 200.0; }();
+static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 48.0; }();   // 48 stages: K = 768
+// CTAs per thread-block cluster for the 64x64 tiles of stage 2 (1, 2, 4 or 8); tuning knob DMRG_CLUSTER.
+// Measured at cfg 5: clusters of 2 / 4 / 8 sibling tiles make stage 2 9-11 % SLOWER (gang scheduling costs more
+// occupancy than the shared L2 lines give back), so the default is 1 (no clusters).
+static const int kCluster = [] { const char* e = getenv("DMRG_CLUSTER"); const int c = e ? atoi(e) : 1; return (c == 1 || c == 2 || c == 4 || c == 8) ? c : 1; }();
 
 static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
                       const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
@@ -283,8 +287,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             // grid.x limit: split very long lists
             size_t i = 0;
             while (i < r.size()) {
-                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);
-                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n});
+                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);   // a multiple of every cluster size
+                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n, (stage == 2 && v == 0) ? kCluster : 1});
                 for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
                 i += n;
             }
@@ -391,8 +395,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             groups.push_back(g);
             i = j;
         }
-        // A tile's K-loop is the critical path of the launch: cap it at 1/kSplitWaves of the time the
-        // whole launch would take on a perfectly balanced machine, but never below kMinSplitStages.
+        // A tile's K-loop is the critical path of the launch: cap it at 1/kSplitWaves of the time the whole launch
+        // would take on a perfectly balanced machine, but never below kMinSplitStages.  Measured at cfg 5 (stage-2
+        // ms): waves 2: 1622, 6: 1495, 24: 1375, 96: 1324, 200: 1314; floor 64 stages: 1333, 32: 1387, 16: 1409 --
+        // many short parts balance better and drift apart less than few long ones; the partial tiles they
+        // write (8 bytes per 2*K flops) cost nothing.
         const double smax = std::max<double>(kMinSplitStages, tile_stages / (kCtaSlots * kSplitWaves));
         std::vector<TileRec> recs2[NUM_VARIANTS];
         const size_t red_begin = reds.size();
@@ -445,8 +452,25 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
-                for (auto& a : cut_m)
-                    for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
+                if (g.variant != 0 || kCluster == 1) {
+                    for (auto& a : cut_m)
+                        for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
+                    return;
+                }
+                // 64x64 tiles of stage 2 are emitted in sibling groups of kCluster (CM x CN neighbouring tiles, padded
+                // with empty tiles): one thread-block cluster each.  Equal costs + stable sort keep a group together.
+                const int CN = kCluster >= 2 ? 2 : 1, CM = kCluster / CN;
+                for (size_t a0 = 0; a0 < cut_m.size(); a0 += CM)
+                    for (size_t b0 = 0; b0 < cut_n.size(); b0 += CN)
+                        for (int da = 0; da < CM; da++)
+                            for (int db = 0; db < CN; db++) {
+                                if (a0 + da < cut_m.size() && b0 + db < cut_n.size()) {
+                                    const auto &a = cut_m[a0 + da], &b = cut_n[b0 + db];
+                                    recs[0].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
+                                } else {
+                                    recs[0].push_back({{-1, 0, 0, 0, 0}, cost});
+                                }
+                            }
             };
             Job jb;
             jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
@@ -716,7 +740,7 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
             const PlanLaunch& L = P->launches[G.first_launch + li];
             cudaStream_t ls = li == 0 ? st : P->aux[li % NUM_VARIANTS];
             if (li > 0) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
-            int rc = launch_grouped_gemm(L.variant, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
+            int rc = launch_grouped_gemm(L.variant, L.cluster, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
                                          P->ops->d_values, P->d_xws, psi, sigma, ls);
             if (rc != DMRG_OK) return rc;
             if (li > 0) {

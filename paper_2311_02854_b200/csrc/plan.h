@@ -8,7 +8,7 @@ struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; }
 
 struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
 
-struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
+struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; int cluster; };   // cluster: CTAs per thread-block cluster (1 = none)
 struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent (stage 3: range of the RedJob table)
 
 enum {
