@@ -69,6 +69,40 @@ def make_config(name, **over):
     return make_blocked_problem(**kw) if gen == "blocked" else make_direct_problem(**kw)
 
 
+def term_subset_problem(pr, term_ids):
+    """The same bond restricted to a subset of the operator-pair terms (a bounded SAMPLE of the workload for
+    timing the oracle): stored operators are shared (no copy), linear-combination operators that no sampled
+    term refers to are dropped and the rest renumbered.  No contraction arithmetic here."""
+    import copy
+    term_ids = np.asarray(term_ids, dtype=np.int64)
+    q = copy.copy(pr)
+    ti = np.array(pr.term_idx[term_ids], dtype=np.int32)
+    ops = np.asarray(pr.ops)
+    is_lin = ops[:, 1] == 7
+    used = sorted({int(o) for o in ti[:, [0, 4]].ravel() if o >= 0 and is_lin[o]})
+    keep = [i for i in range(len(ops)) if not is_lin[i]] + used
+    remap = {old: new for new, old in enumerate(keep)}
+    new_ops = ops[keep].copy()
+    lin_ptr, lin_op, lin_coef = [0], [], []
+    for new, old in enumerate(keep):
+        if is_lin[old]:
+            j = int(ops[old, 2])
+            a, b = int(pr.lin_ptr[j]), int(pr.lin_ptr[j + 1])
+            new_ops[new, 2] = len(lin_ptr) - 1
+            lin_op += [remap[int(o)] for o in pr.lin_op[a:b]]
+            lin_coef += list(pr.lin_coef[a:b])
+            lin_ptr.append(len(lin_op))
+    for col in (0, 4):
+        ti[:, col] = [remap[int(o)] if o >= 0 else -1 for o in ti[:, col]]
+    q.ops = new_ops
+    q.lin_ptr = np.array(lin_ptr, dtype=np.int64)
+    q.lin_op = np.array(lin_op, dtype=np.int32)
+    q.lin_coef = np.array(lin_coef, dtype=np.float64)
+    q.term_idx = ti
+    q.term_coef = np.array(pr.term_coef[term_ids], dtype=np.float64)
+    return q
+
+
 def determinant_map(pr):
     """For tracked tiny problems: list over psi blocks of (dets, E) with
     psi_block = E^T-projected determinant coefficients; E = kron(E_L, E_R) per block.

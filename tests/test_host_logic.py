@@ -139,3 +139,14 @@ def test_direct_fill_problem_is_hermitian_and_seeded():
     _fill_normal(x1, 7, nthreads=1)
     _fill_normal(x2, 7, nthreads=4)
     assert np.array_equal(x1, x2)
+
+
+def test_term_subset_sampler_partitions_sigma():
+    """bench.py --impl reference times the oracle on every stride-th term: the subsets must partition H."""
+    from dmrg_workload.problem import term_subset_problem
+    pr = make_direct_problem(12, 5, 12, 0, D=60, seed=4)
+    psi = random_psi(pr.psi_size, 3)
+    full = oracle.opair_sigma(pr, psi)
+    n = len(pr.term_coef)
+    acc = sum(oracle.opair_sigma(term_subset_problem(pr, np.arange(k, n, 4)), psi) for k in range(4))
+    assert np.abs(acc - full).max() <= 1e-12 * np.linalg.norm(full)
