@@ -84,7 +84,10 @@ static_assert(sizeof(Tile) == 16, "Tile layout");
 struct TileShape { int bm, bn; };
 constexpr int NUM_VARIANTS = 5;
 extern const TileShape kVariants[NUM_VARIANTS];
-constexpr int GEMM_BK = 16;
+#ifndef DMRG_GEMM_BK
+#define DMRG_GEMM_BK 16
+#endif
+constexpr int GEMM_BK = DMRG_GEMM_BK;   // k-columns per pipeline stage (8, 16 or 32)
 
 struct GemmLaunch {       // one launch of one kernel variant
     int     variant;
