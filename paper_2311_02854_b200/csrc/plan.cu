@@ -634,6 +634,9 @@ __global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ 
 
 using namespace dmrg;
 
+// tuning knob: DMRG_NO_FORK=1 runs the launches of a group back to back on the caller's stream
+static const bool kNoFork = [] { const char* e = getenv("DMRG_NO_FORK"); return e && atoi(e) != 0; }();
+
 extern "C" {
 
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms, const double* site_ops,
@@ -738,12 +741,12 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         if (G.nlaunch > 1) DMRG_CUDA(cudaEventRecord(P->ev_fork, st));
         for (int li = 0; li < G.nlaunch; li++) {
             const PlanLaunch& L = P->launches[G.first_launch + li];
-            cudaStream_t ls = li == 0 ? st : P->aux[li % NUM_VARIANTS];
-            if (li > 0) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
+            cudaStream_t ls = (li == 0 || kNoFork) ? st : P->aux[li % NUM_VARIANTS];
+            if (li > 0 && !kNoFork) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
             int rc = launch_grouped_gemm(L.variant, L.cluster, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
                                          P->ops->d_values, P->d_xws, psi, sigma, ls);
             if (rc != DMRG_OK) return rc;
-            if (li > 0) {
+            if (li > 0 && !kNoFork) {
                 DMRG_CUDA(cudaEventRecord(P->ev_join[li % NUM_VARIANTS], ls));
                 DMRG_CUDA(cudaStreamWaitEvent(st, P->ev_join[li % NUM_VARIANTS], 0));
             }
