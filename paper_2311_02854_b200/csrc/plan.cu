@@ -79,7 +79,12 @@ static inline double warp_area(const std::vector<std::pair<int, int>>& cm, const
 
 static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N + 7) / 8); }
 
+__global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops, double* __restrict__ pack);
+
 struct TileRec { Tile t; double cost; };
+
+constexpr int64_t kMaxMergedCols = 4096;          // widest N-merged stage-1 GEMM
+constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are offsets into the packed R store
 
 // split-K policy of stage 2 (see the comment at its use)
 constexpr double kCtaSlots = 148.0 * 4;     // resident 64x64 CTAs on a B200
@@ -273,6 +278,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     std::vector<Tile> tiles;
     std::vector<std::vector<HdItem>> hd(nblk);
     std::vector<RedJob> reds;   // split-K reductions (stage 3)
+    std::vector<PackDesc> packs;   // packed R store (stage-1 B operands), filled on the device after upload
+    std::vector<size_t> pack_segs;  // segments whose b_off is relative to the packed store
+    int64_t pack_top = 0;
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
     int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
 
@@ -322,50 +330,113 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         std::vector<TileRec> recs1[NUM_VARIANTS];
         std::vector<std::pair<int, int>> cut_m, cut_n;
         int64_t xtop = 0;
+        // runs: one R block (normal or transposed use) applied to a run of consecutive psi blocks of its input panel
+        struct Run { size_t i, j; int64_t rows; };
+        std::vector<Run> runs;
         for (size_t i = 0; i < req.size();) {
             size_t j = i + 1;
             while (j < req.size() && req[j].r_off == req[i].r_off && req[j].r_trans == req[i].r_trans &&
                    req[j].in_blk == req[j - 1].in_blk + 1 && P->blocks[req[j].in_blk].ir == P->blocks[req[i].in_blk].ir)
                 j++;
-            const dmrg_psi_block& B0 = P->blocks[req[i].in_blk];
-            const int dRi = B0.dr, dRo = req[i].dRo, ldx = (int)round_up2(dRo);
             int64_t rows = 0;
-            bool v2 = psi_vec2(B0);
-            for (size_t q = i; q < j; q++) {
-                xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rows * ldx, ldx};
-                rows += P->blocks[req[q].in_blk].dl;
-            }
+            for (size_t q = i; q < j; q++) rows += P->blocks[req[q].in_blk].dl;
             DMRG_REQUIRE(rows < (int64_t(1) << 31), "dmrg_plan_create: merged stage-1 panel too tall");
-            Seg s;
-            s.a_off = B0.offset; s.lda = dRi;
-            s.b_off = req[i].r_off; s.ldb = (int)round_up2(req[i].r_trans ? dRo : dRi);
-            s.K = dRi; s.alpha = 1.0;
-            s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | (v2 ? SEG_A_VEC2 : 0) |
-                      (req[i].r_trans ? 0 : SEG_B_KCONTIG);
-            Job jb;
-            jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = dRo;
-            jb.seg_begin = (int32_t)segs.size(); jb.seg_end = jb.seg_begin + 1;
-            jb.flags = (SP_X << JOB_C_SPACE_SHIFT);
-            jb.pad_ = (dRi + GEMM_BK - 1) / GEMM_BK;
-            segs.push_back(s);
-            const int v = choose_variant(jb.M, jb.N);
-            const int bm = kVariants[v].bm, bn = kVariants[v].bn;
-            const double kpad4 = 4.0 * ((dRi + 3) / 4);
-            cut_dim(jb.M, bm, cut_m);
-            cut_dim(jb.N, bn, cut_n);
-            for (auto& a : cut_m)
-                for (auto& b : cut_n)
-                    recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
-            padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
-            stage_flops += 2.0 * frag_area(jb.M, jb.N) * 16.0 * jb.pad_;
-            warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * 16.0 * jb.pad_;
-            tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * 16.0 * jb.pad_;
-            s1_flops += 2.0 * rows * dRi * dRo;
-            alg_bytes += 8.0 * (rows * dRi + (double)dRi * dRo + rows * dRo);
-            jobs.push_back(jb);
-            s1_jobs++;
-            xtop += rows * ldx;
+            runs.push_back({i, j, rows});
             i = j;
+        }
+        // N-merge: R blocks that are applied to exactly the same runs of psi rows (same "signature") are stacked
+        // along N in the plan's packed store, K-contiguous, each block once per chunk (h.c. uses transposed while
+        // packing).  Every run of the signature is then ONE GEMM against the whole stack: one pass over those psi
+        // rows serves hundreds of R blocks, tiles are full but for one remainder per stack, and sectors of dimension
+        // 1..32 stop being skinny GEMMs.
+        // `runs` is ordered by (R block, first psi block): the runs of one R block are consecutive.
+        struct RBlk { size_t r0, r1; };   // range in runs[]
+        std::vector<RBlk> rblks;
+        for (size_t r = 0; r < runs.size();) {
+            size_t e = r + 1;
+            while (e < runs.size() && req[runs[e].i].r_off == req[runs[r].i].r_off && req[runs[e].i].r_trans == req[runs[r].i].r_trans) e++;
+            rblks.push_back({r, e});
+            r = e;
+        }
+        auto sig_less = [&](const RBlk& x, const RBlk& y) {   // lexicographic on the list of (first block, length)
+            const size_t nx = x.r1 - x.r0, ny = y.r1 - y.r0;
+            for (size_t t = 0; t < std::min(nx, ny); t++) {
+                const Run &a = runs[x.r0 + t], &b = runs[y.r0 + t];
+                if (req[a.i].in_blk != req[b.i].in_blk) return req[a.i].in_blk < req[b.i].in_blk;
+                if (a.j - a.i != b.j - b.i) return (a.j - a.i) < (b.j - b.i);
+            }
+            return nx < ny;
+        };
+        std::stable_sort(rblks.begin(), rblks.end(), sig_less);
+        for (size_t c0 = 0; c0 < rblks.size();) {
+            // class [c0, c1): same signature, stack width capped
+            const dmrg_psi_block& B0 = P->blocks[req[runs[rblks[c0].r0].i].in_blk];
+            const int dRi = B0.dr, ldp = (int)round_up2(dRi);
+            size_t c1 = c0;
+            int64_t ncols = 0;
+            while (c1 < rblks.size() && !sig_less(rblks[c0], rblks[c1]) && !sig_less(rblks[c1], rblks[c0]) &&
+                   (c1 == c0 || ncols + round_up2(req[runs[rblks[c1].r0].i].dRo) <= kMaxMergedCols)) {
+                ncols += round_up2(req[runs[rblks[c1].r0].i].dRo);
+                c1++;
+            }
+            const int ldx = (int)ncols;   // even by construction
+            // pack the stack once
+            std::vector<int64_t> col0s;
+            int64_t col0 = 0;
+            for (size_t c = c0; c < c1; c++) {
+                const XReq& r0 = req[runs[rblks[c].r0].i];
+                packs.push_back({r0.r_off, pack_top + col0 * ldp, r0.dRo, dRi, (int32_t)round_up2(r0.r_trans ? r0.dRo : dRi), r0.r_trans, ldp, 0});
+                col0s.push_back(col0);
+                col0 += round_up2(r0.dRo);
+                alg_bytes += 8.0 * (double)dRi * r0.dRo;
+            }
+            // one GEMM per run of the signature
+            const size_t nruns = rblks[c0].r1 - rblks[c0].r0;
+            for (size_t t = 0; t < nruns; t++) {
+                const Run& R0 = runs[rblks[c0].r0 + t];
+                const dmrg_psi_block& Bt = P->blocks[req[R0.i].in_blk];
+                const int64_t rows = R0.rows;
+                for (size_t c = c0; c < c1; c++) {
+                    const Run& Rc = runs[rblks[c].r0 + t];
+                    int64_t rr = 0;
+                    for (size_t q = Rc.i; q < Rc.j; q++) {
+                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx};
+                        rr += P->blocks[req[q].in_blk].dl;
+                    }
+                    s1_flops += 2.0 * rows * dRi * req[Rc.i].dRo;
+                    alg_bytes += 8.0 * rows * req[Rc.i].dRo;
+                }
+                alg_bytes += 8.0 * rows * dRi;
+                Seg s;
+                s.a_off = Bt.offset; s.lda = dRi;
+                s.b_off = kPackBase + pack_top; s.ldb = ldp;   // resolved to an offset from the operator store at upload
+                s.K = dRi; s.alpha = 1.0;
+                s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | (psi_vec2(Bt) ? SEG_A_VEC2 : 0) | SEG_B_KCONTIG;
+                pack_segs.push_back(segs.size());
+                Job jb;
+                jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = (int)ncols;
+                jb.seg_begin = (int32_t)segs.size(); jb.seg_end = jb.seg_begin + 1;
+                jb.flags = (SP_X << JOB_C_SPACE_SHIFT);
+                jb.pad_ = (dRi + GEMM_BK - 1) / GEMM_BK;
+                segs.push_back(s);
+                const int v = choose_variant(jb.M, jb.N);
+                const int bm = kVariants[v].bm, bn = kVariants[v].bn;
+                const double kpad4 = 4.0 * ((dRi + 3) / 4);
+                cut_dim(jb.M, bm, cut_m);
+                cut_dim(jb.N, bn, cut_n);
+                for (auto& a : cut_m)
+                    for (auto& b : cut_n)
+                        recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
+                padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
+                stage_flops += 2.0 * frag_area(jb.M, jb.N) * 16.0 * jb.pad_;
+                warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * 16.0 * jb.pad_;
+                tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * 16.0 * jb.pad_;
+                jobs.push_back(jb);
+                s1_jobs++;
+                xtop += rows * ldx;
+            }
+            pack_top += ncols * ldp;
+            c0 = c1;
         }
         ws_peak = std::max(ws_peak, xtop);
         emit_tiles(recs1, 1);
@@ -554,13 +625,19 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     // ---- upload ---------------------------------------------------------------------------------------
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
     P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
-                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems);
+                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems + 8.0 * pack_top);
     if (S->structure_only) return DMRG_OK;
     auto up = [&](void** dptr, const void* src, size_t bytes) -> int {
         DMRG_CUDA(cudaMalloc(dptr, std::max<size_t>(bytes, 16)));
         if (bytes) DMRG_CUDA(cudaMemcpy(*dptr, src, bytes, cudaMemcpyHostToDevice));
         return DMRG_OK;
     };
+    DMRG_CUDA(cudaMalloc(&P->d_pack, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
+    DMRG_CUDA(cudaMemset(P->d_pack, 0, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
+    {   // the GEMM kernel addresses the packed store relative to the operator store (one flat device address space)
+        const int64_t delta = (int64_t)(P->d_pack - S->d_values);
+        for (size_t q : pack_segs) segs[q].b_off += delta - kPackBase;
+    }
     for (Seg& sg : segs) sg.flags |= sg.alpha == 1.0 ? SEG_ALPHA_ONE : (sg.alpha == -1.0 ? SEG_ALPHA_NEG : 0u);
     int rc;
     if ((rc = up((void**)&P->d_jobs, jobs.data(), jobs.size() * sizeof(Job)))) return rc;
@@ -576,7 +653,34 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_join[v], cudaEventDisableTiming));
     }
     DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
+    if (!packs.empty()) {
+        PackDesc* d_packs = nullptr;
+        DMRG_CUDA(cudaMalloc(&d_packs, packs.size() * sizeof(PackDesc)));
+        DMRG_CUDA(cudaMemcpy(d_packs, packs.data(), packs.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));
+        for (size_t y0 = 0; y0 < packs.size(); y0 += 32768) {
+            const unsigned ny = (unsigned)std::min<size_t>(32768, packs.size() - y0);
+            pack_r_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, S->d_values, P->d_pack);
+        }
+        DMRG_CUDA(cudaGetLastError());
+        DMRG_CUDA(cudaDeviceSynchronize());
+        cudaFree(d_packs);
+    }
     return gemm_init();
+}
+
+// packed[n * ldp + k] = R block element (n, k) of the operator as USED: the stored block for a normal use, its
+// transpose for an h.c. use.  Run once per plan.     grid (chunks of elements, blocks)
+__global__ void __launch_bounds__(256) pack_r_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops,
+                                                     double* __restrict__ pack) {
+    const PackDesc d = descs[blockIdx.y];
+    const int64_t n_el = (int64_t)d.dRo * d.dRi;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_el; e += (int64_t)gridDim.x * blockDim.x) {
+        int n, k;
+        if (d.trans) { k = (int)(e / d.dRo); n = (int)(e - (int64_t)k * d.dRo); }   // coalesced read of the stored rows
+        else { n = (int)(e / d.dRi); k = (int)(e - (int64_t)n * d.dRi); }
+        const double v = d.trans ? ops[d.src + (int64_t)k * d.src_ld + n] : ops[d.src + (int64_t)n * d.src_ld + k];
+        pack[d.dst + (int64_t)n * d.ldp + k] = v;
+    }
 }
 
 // sigma_blk += sum_p partial_p, parts added in order (the deterministic end of split-K)     grid (chunks, jobs)
@@ -669,7 +773,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack);
     for (auto e : P->ev) cudaEventDestroy(e);
     for (int v = 0; v < NUM_VARIANTS; v++) {
         if (P->aux[v]) cudaStreamDestroy(P->aux[v]);

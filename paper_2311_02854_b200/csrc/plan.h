@@ -8,6 +8,8 @@ struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; }
 
 struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
 
+struct PackDesc { int64_t src, dst; int32_t dRo, dRi, src_ld, trans, ldp, pad_; };   // one R block copied into the packed stage-1 store
+
 struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; int cluster; };   // cluster: CTAs per thread-block cluster (1 = none)
 struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent (stage 3: range of the RedJob table)
 
@@ -32,6 +34,7 @@ struct dmrg_plan {
     cudaStream_t aux[dmrg::NUM_VARIANTS] = {nullptr};   // side streams: independent launches of a group overlap
     cudaEvent_t ev_fork = nullptr, ev_join[dmrg::NUM_VARIANTS] = {nullptr};
     RedJob* d_reds = nullptr;
+    double* d_pack = nullptr;   // packed, N-merged, K-contiguous copies of the R blocks (stage-1 B operands)
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
     int64_t n_hd_blocks = 0;
