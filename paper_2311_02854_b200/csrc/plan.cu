@@ -284,7 +284,14 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
     int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
 
-    auto psi_vec2 = [&](const dmrg_psi_block& B) { return (B.offset % 2 == 0) && (B.dr % 2 == 0); };
+    // The GEMM kernels read psi from a padded copy (rows padded to an even length, refreshed at the start of every
+    // dmrg_sigma): every psi operand is then 16-byte aligned; consecutive blocks of a panel stay contiguous.
+    std::vector<int64_t> ppad(nblk);
+    {
+        int64_t o = 0;
+        for (int64_t b = 0; b < nblk; b++) { ppad[b] = o; o += (int64_t)P->blocks[b].dl * round_up2(P->blocks[b].dr); }
+        P->psi_pad_elems = std::max<int64_t>(o, 2);
+    }
 
     auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
         PlanGroup grp{stage, (int)P->launches.size(), 0};
@@ -408,10 +415,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 }
                 alg_bytes += 8.0 * rows * dRi;
                 Seg s;
-                s.a_off = Bt.offset; s.lda = dRi;
+                s.a_off = ppad[req[R0.i].in_blk]; s.lda = ldp;
                 s.b_off = kPackBase + pack_top; s.ldb = ldp;   // resolved to an offset from the operator store at upload
                 s.K = dRi; s.alpha = 1.0;
-                s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | (psi_vec2(Bt) ? SEG_A_VEC2 : 0) | SEG_B_KCONTIG;
+                s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | SEG_A_VEC2 | SEG_B_KCONTIG;
                 pack_segs.push_back(segs.size());
                 Job jb;
                 jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = (int)ncols;
@@ -496,8 +503,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 }
                 if (k.r_off < 0) {
                     const dmrg_psi_block& IB = P->blocks[k.in_blk];
-                    s.b_off = IB.offset; s.ldb = IB.dr;
-                    s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | (psi_vec2(IB) ? SEG_B_VEC2 : 0);
+                    s.b_off = ppad[k.in_blk]; s.ldb = (int)round_up2(IB.dr);
+                    s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
                     if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
                 } else {
                     const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
@@ -611,7 +618,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     std::vector<HdItem> hd_items;
     std::vector<HdBlock> hd_blocks(nblk);
     for (int64_t b = 0; b < nblk; b++) {
-        hd_blocks[b] = {P->blocks[b].offset, P->blocks[b].dl, P->blocks[b].dr, (int32_t)hd_items.size(), 0};
+        hd_blocks[b] = {P->blocks[b].offset, P->blocks[b].dl, P->blocks[b].dr, (int32_t)hd_items.size(), 0, ppad[b]};
         hd_items.insert(hd_items.end(), hd[b].begin(), hd[b].end());
         hd_blocks[b].item_end = (int32_t)hd_items.size();
     }
@@ -632,6 +639,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         if (bytes) DMRG_CUDA(cudaMemcpy(*dptr, src, bytes, cudaMemcpyHostToDevice));
         return DMRG_OK;
     };
+    DMRG_CUDA(cudaMalloc(&P->d_psi_pad, sizeof(double) * (size_t)P->psi_pad_elems));
     DMRG_CUDA(cudaMalloc(&P->d_pack, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     DMRG_CUDA(cudaMemset(P->d_pack, 0, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     {   // the GEMM kernel addresses the packed store relative to the operator store (one flat device address space)
@@ -680,6 +688,18 @@ __global__ void __launch_bounds__(256) pack_r_kernel(const PackDesc* __restrict_
         else { n = (int)(e / d.dRi); k = (int)(e - (int64_t)n * d.dRi); }
         const double v = d.trans ? ops[d.src + (int64_t)k * d.src_ld + n] : ops[d.src + (int64_t)n * d.src_ld + k];
         pack[d.dst + (int64_t)n * d.ldp + k] = v;
+    }
+}
+
+// padded psi copy: block rows get an even length (zero pad)     grid (chunks, blocks)
+__global__ void __launch_bounds__(256) pad_psi_kernel(const HdBlock* __restrict__ blocks, const double* __restrict__ psi,
+                                                      double* __restrict__ pad) {
+    const HdBlock b = blocks[blockIdx.y];
+    const int ld = (b.dr + 1) & ~1;
+    const int64_t n = (int64_t)b.dl * ld;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / ld), j = (int)(e - (int64_t)i * ld);
+        pad[b.pad_off + e] = j < b.dr ? psi[b.offset + (int64_t)i * b.dr + j] : 0.0;
     }
 }
 
@@ -773,7 +793,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad);
     for (auto e : P->ev) cudaEventDestroy(e);
     for (int v = 0; v < NUM_VARIANTS; v++) {
         if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
@@ -828,6 +848,11 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
     const size_t ng = P->groups.size();
     if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * ng], st));
     DMRG_CUDA(cudaMemsetAsync(sigma, 0, sizeof(double) * (size_t)P->psi_size, st));
+    for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += 32768) {
+        const unsigned ny = (unsigned)std::min<int64_t>(32768, P->n_hd_blocks - y0);
+        pad_psi_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_hd_blocks + y0, psi, P->d_psi_pad);
+    }
+    DMRG_CUDA(cudaGetLastError());
     for (size_t gi = 0; gi < ng; gi++) {
         const PlanGroup& G = P->groups[gi];
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi], st));
@@ -848,7 +873,7 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
             cudaStream_t ls = (li == 0 || kNoFork) ? st : P->aux[li % NUM_VARIANTS];
             if (li > 0 && !kNoFork) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
             int rc = launch_grouped_gemm(L.variant, L.cluster, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
-                                         P->ops->d_values, P->d_xws, psi, sigma, ls);
+                                         P->ops->d_values, P->d_xws, P->d_psi_pad, sigma, ls);
             if (rc != DMRG_OK) return rc;
             if (li > 0 && !kNoFork) {
                 DMRG_CUDA(cudaEventRecord(P->ev_join[li % NUM_VARIANTS], ls));

@@ -4,7 +4,7 @@
 
 struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // offsets < 0: identity factor
 struct HdTile { int32_t blk; int16_t ti, tj; };   // 32 x 32 tile of a psi block
-struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; };
+struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; int64_t pad_off; };   // pad_off: block in the padded psi copy
 
 struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
 
@@ -34,6 +34,8 @@ struct dmrg_plan {
     cudaStream_t aux[dmrg::NUM_VARIANTS] = {nullptr};   // side streams: independent launches of a group overlap
     cudaEvent_t ev_fork = nullptr, ev_join[dmrg::NUM_VARIANTS] = {nullptr};
     RedJob* d_reds = nullptr;
+    double* d_psi_pad = nullptr;   // psi re-laid with even leading dimensions (16-byte cp.async for every operand)
+    int64_t psi_pad_elems = 0;
     double* d_pack = nullptr;   // packed, N-merged, K-contiguous copies of the R blocks (stage-1 B operands)
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
