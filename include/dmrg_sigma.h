@@ -117,6 +117,9 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *   n_total, two_sz_total: target quantum numbers of psi
  *   workspace_bytes: HBM the plan may use for the X intermediates (0 = default 8 GiB, clamped to
  *              what one term needs); terms are processed in chunks that fit it.
+ *              Besides the workspace the plan owns a packed copy of the R-side blocks as stage 1 uses them
+ *              (about the size of the R half of the store, twice where a block is used both ways) and a
+ *              padded copy of psi; dmrg_plan_stat(8) reports the total.
  * Fails with DMRG_ECHARGE if a term does not conserve (N, 2Sz).  The plan borrows `ops`
  * (which must outlive it) and owns its descriptors and workspace.  Synchronous.
  */

@@ -4,9 +4,10 @@
 // combination of symmetry blocks becomes a GEMM pair (Eq. 14).  Differences from the paper's design
 // (cublasDgemmBatched per equal-shape group on many streams), chosen for one B200:
 //   * stage-1 products X = psi_blk * (O^R_blk)^T are de-duplicated (X depends only on the R block and
-//     the psi block, and one-index R operators recur in many terms) and, because psi is laid out
-//     with all blocks of one R sector back to back, consecutive psi blocks are merged into one tall
-//     GEMM per R block;
+//     the psi block, and one-index R operators recur in many terms); because psi is laid out with all
+//     blocks of one R sector back to back, consecutive psi blocks are merged along M; and R blocks applied
+//     to the same psi rows are merged along N through a plan-owned packed copy (K-contiguous, h.c. uses
+//     transposed), so one tall-and-wide GEMM replaces hundreds of small ones;
 //   * all contributions to one sigma block are concatenated along K into ONE GEMM whose K-loop walks
 //     the (term, input block) pairs in a fixed order -- this is Eq. (13) without a separate reduction
 //     kernel and without atomics;

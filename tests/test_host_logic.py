@@ -150,3 +150,15 @@ def test_term_subset_sampler_partitions_sigma():
     n = len(pr.term_coef)
     acc = sum(oracle.opair_sigma(term_subset_problem(pr, np.arange(k, n, 4)), psi) for k in range(4))
     assert np.abs(acc - full).max() <= 1e-12 * np.linalg.norm(full)
+
+
+def test_stage1_is_n_merged():
+    """Stage 1 is planned as a few tall-and-wide GEMMs (R blocks stacked along N), not one GEMM per R block."""
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr, structure_only=True)
+    s = plan.stats()
+    n_rblocks_used = len({(int(t[4]), int(t[5])) for t in pr.term_idx if t[4] >= 0})   # (R op, trans) pairs
+    assert s["s1_jobs"] < 0.25 * n_rblocks_used * len(pr.secR)      # far fewer GEMMs than (op, sector) pairs
+    assert s["s1_flops"] > 0 and s["padded_flops"] / (s["s1_flops"] + s["s2_flops"]) < 1.5
+    plan.destroy()
+    ops.free()
