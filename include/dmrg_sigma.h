@@ -150,6 +150,8 @@ double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
  * alias; sigma is OVERWRITTEN.  Work is enqueued on `cuda_stream` (a cudaStream_t, NULL = default
  * stream) and the call returns without synchronising.  Bitwise reproducible run to run: every
  * sigma element is accumulated by one thread block in plan order, no floating-point atomics.
+ * A plan owns one X workspace and one padded copy of psi: calls on the same plan must be ordered (same stream,
+ * or externally synchronised); use one plan per concurrent stream.
  */
 int dmrg_sigma(dmrg_plan* plan, const double* psi, double* sigma, void* cuda_stream);
 

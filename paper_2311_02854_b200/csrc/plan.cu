@@ -84,7 +84,8 @@ __global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* 
 
 struct TileRec { Tile t; double cost; };
 
-constexpr int64_t kMaxMergedCols = 4096;          // widest N-merged stage-1 GEMM
+// widest N-merged stage-1 GEMM (tuning knob DMRG_MAX_MERGED_COLS)
+static const int64_t kMaxMergedCols = [] { const char* e = getenv("DMRG_MAX_MERGED_COLS"); const long v = e ? atol(e) : 0; return v >= 64 ? (int64_t)(v & ~1L) : int64_t(4096); }();
 constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are offsets into the packed R store
 
 // split-K policy of stage 2 (see the comment at its use)
