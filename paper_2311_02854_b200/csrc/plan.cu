@@ -795,7 +795,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io);
     for (auto e : P->ev) cudaEventDestroy(e);
     for (int v = 0; v < NUM_VARIANTS; v++) {
         if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
@@ -891,21 +891,16 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
 int dmrg_sigma_host(dmrg_plan* P, const double* psi_host, double* sigma_host, void* cuda_stream) {
     if (!P || !psi_host || !sigma_host) { set_error("dmrg_sigma_host: NULL argument"); return DMRG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    double* d = nullptr;
     const size_t bytes = sizeof(double) * (size_t)P->psi_size;
     const size_t pad = (bytes + 255) & ~size_t(255);
-    DMRG_CUDA(cudaMalloc(&d, 2 * pad));
+    if (!P->d_host_io) DMRG_CUDA(cudaMalloc(&P->d_host_io, 2 * pad));   // staging vectors, kept for later calls
+    double* d = P->d_host_io;
     double* d_sig = (double*)((char*)d + pad);
-    int rc = DMRG_OK;
-    cudaError_t e = cudaMemcpyAsync(d, psi_host, bytes, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) {
-        rc = dmrg_sigma(P, d, d_sig, cuda_stream);
-        if (rc == DMRG_OK) e = cudaMemcpyAsync(sigma_host, d_sig, bytes, cudaMemcpyDeviceToHost, st);
-    }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    cudaFree(d);
+    DMRG_CUDA(cudaMemcpyAsync(d, psi_host, bytes, cudaMemcpyHostToDevice, st));
+    int rc = dmrg_sigma(P, d, d_sig, cuda_stream);
     if (rc != DMRG_OK) return rc;
-    if (e != cudaSuccess) { set_error("dmrg_sigma_host: %s", cudaGetErrorString(e)); return DMRG_ECUDA; }
+    DMRG_CUDA(cudaMemcpyAsync(sigma_host, d_sig, bytes, cudaMemcpyDeviceToHost, st));
+    DMRG_CUDA(cudaStreamSynchronize(st));
     return DMRG_OK;
 }
 

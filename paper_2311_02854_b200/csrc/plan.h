@@ -36,6 +36,7 @@ struct dmrg_plan {
     RedJob* d_reds = nullptr;
     double* d_psi_pad = nullptr;   // psi re-laid with even leading dimensions (16-byte cp.async for every operand)
     int64_t psi_pad_elems = 0;
+    double* d_host_io = nullptr;   // device staging of dmrg_sigma_host (psi, sigma), allocated on first use
     double* d_pack = nullptr;   // packed, N-merged, K-contiguous copies of the R blocks (stage-1 B operands)
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;
