@@ -84,7 +84,7 @@ static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N
 
 __global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops, double* __restrict__ pack);
 
-struct TileRec { Tile t; double cost; };
+struct TileRec { Tile t; double cost; int64_t key = 0; };   // key: secondary launch order inside a cost bucket
 
 // widest N-merged stage-1 GEMM (tuning knob DMRG_MAX_MERGED_COLS)
 static const int64_t kMaxMergedCols = [] { const char* e = getenv("DMRG_MAX_MERGED_COLS"); const long v = e ? atol(e) : 0; return v >= 64 ? (int64_t)(v & ~1L) : int64_t(4096); }();
@@ -94,6 +94,7 @@ constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are
 constexpr double kCtaSlots = 148.0 * 4;     // resident 64x64 CTAs on a B200
 static const double kSplitWaves = [] { const char* e = getenv("DMRG_SPLIT_WAVES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 200.0; }();
 static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 48.0; }();   // 48 stages: K = 768
+static const bool kTileOrder = [] { const char* e = getenv("DMRG_TILE_ORDER"); return !e || atoi(e) != 0; }();   // knob: 0 = pure cost order
 // CTAs per thread-block cluster for the 64x64 tiles of stage 2 (1, 2, 4 or 8); tuning knob DMRG_CLUSTER.
 // Measured at cfg 5: clusters of 2 / 4 / 8 sibling tiles make stage 2 9-11 % SLOWER (gang scheduling costs more
 // occupancy than the shared L2 lines give back), so the default is 1 (no clusters).
@@ -302,7 +303,17 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         for (int v = 0; v < NUM_VARIANTS; v++) {
             auto& r = recs[v];
             if (r.empty()) continue;
-            std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
+            // longest first (LPT through the hardware block scheduler); inside a sqrt(2)-wide cost bucket, stage-2
+            // tiles follow `key` = (L sector of the sigma block, split-K part): sigma blocks of one L-sector row walk
+            // the same L operator blocks, so launching them together lets them share those blocks in L2
+            if (kTileOrder)
+                std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) {
+                    const int ba = (int)std::floor(2.0 * std::log2(a.cost)), bb = (int)std::floor(2.0 * std::log2(b.cost));
+                    if (ba != bb) return ba > bb;
+                    return a.key < b.key;
+                });
+            else
+                std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
             // grid.x limit: split very long lists
             size_t i = 0;
             while (i < r.size()) {
@@ -533,10 +544,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * 16.0 * g.nst;
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
+            int part_no = 0;
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
+                const int64_t key = (int64_t)OB.il * 65536 + part_no++;
                 if (g.variant != 0 || kCluster == 1) {
                     for (auto& a : cut_m)
-                        for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
+                        for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
                     return;
                 }
                 // 64x64 tiles of stage 2 are emitted in sibling groups of kCluster (CM x CN neighbouring tiles, padded
@@ -548,9 +561,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                             for (int db = 0; db < CN; db++) {
                                 if (a0 + da < cut_m.size() && b0 + db < cut_n.size()) {
                                     const auto &a = cut_m[a0 + da], &b = cut_n[b0 + db];
-                                    recs[0].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost});
+                                    recs[0].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
                                 } else {
-                                    recs[0].push_back({{-1, 0, 0, 0, 0}, cost});
+                                    recs[0].push_back({{-1, 0, 0, 0, 0}, cost, key});
                                 }
                             }
             };
