@@ -100,21 +100,65 @@ template <int BMN, int NT>
 __device__ __forceinline__ void load_operand(uint32_t sdst, const double* __restrict__ g, int ld, bool kcontig, bool vec2,
                                              int mn_lim, int k_lim, int tid) {
     const int mn_end = (mn_lim + 7) & ~7, k_end = (k_lim + 3) & ~3;
-    if (kcontig) {
-        if (vec2) {
-            constexpr int RPI = NT / (BK / 2), ITERS = BMN / RPI;   // rows per pass
+    if (vec2 && mn_lim >= BMN && k_lim >= BK) {
+        // interior stage (full tile, full K slab): no predicates, no zero-fill -- a copy is the LDGSTS and a 64-bit
+        // add.  The producer warp is on the critical path; this is the common case.
+        if (kcontig) {
+            constexpr int RPI = NT / (BK / 2), ITERS = BMN / RPI;
             const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
-            const int kb = k + 1 < k_lim ? 16 : (k < k_lim ? 8 : 0);
-            const bool lane_on = k < k_end;
             const double* src = g + (int64_t)r0 * ld + k;
             const int64_t step = (int64_t)RPI * ld;
             const uint32_t dst = sdst + (r0 * KPAD + k) * 8;
 #pragma unroll
             for (int i = 0; i < ITERS; i++) {
-                const int row = r0 + RPI * i;
-                const bool in = row < mn_lim;
-                cp_async16_if(dst + i * RPI * KPAD * 8, in ? src : g, in ? kb : 0, lane_on && row < mn_end);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + i * RPI * KPAD * 8), "l"(src) : "memory");
                 src += step;
+            }
+        } else {
+            constexpr int MPAD = BMN + 4;
+            constexpr int PR = BMN / 2;
+            constexpr int SEGS = PR > NT ? PR / NT : 1;
+            constexpr int KPI = PR > NT ? 1 : NT / PR;
+            const int k0 = tid / PR, mn0 = (tid % PR) * 2;
+#pragma unroll
+            for (int sg = 0; sg < SEGS; sg++) {
+                const int mn = mn0 + sg * NT * 2;
+                const double* src = g + (int64_t)k0 * ld + mn;
+                const int64_t step = (int64_t)KPI * ld;
+                const uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
+#pragma unroll
+                for (int i = 0; i < BK / KPI; i++) {
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst + i * KPI * MPAD * 8), "l"(src) : "memory");
+                    src += step;
+                }
+            }
+        }
+        return;
+    }
+    if (kcontig) {
+        if (vec2) {
+            // ragged stage: this lane's rows r0, r0+RPI, ...: full copies (kb bytes of the row's K slab) while the row
+            // is inside the matrix, then zero-fill up to the next multiple of 8 rows; loops are bounded by the row
+            // counts, so a ragged tile costs the producer in proportion to its rows
+            constexpr int RPI = NT / (BK / 2);
+            const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
+            const int kb = k + 1 < k_lim ? 16 : (k < k_lim ? 8 : 0);
+            if (k < k_end) {
+                const int n_in = mn_lim > r0 ? (mn_lim - r0 + RPI - 1) / RPI : 0;
+                const int n_all = mn_end > r0 ? (mn_end - r0 + RPI - 1) / RPI : 0;
+                const double* src = g + (int64_t)r0 * ld + k;
+                const int64_t step = (int64_t)RPI * ld;
+                uint32_t dst = sdst + (r0 * KPAD + k) * 8;
+#pragma unroll 4
+                for (int i = 0; i < n_in; i++) {
+                    cp_async16(dst, src, kb);
+                    src += step;
+                    dst += RPI * KPAD * 8;
+                }
+                for (int i = n_in; i < n_all; i++) {
+                    cp_async16(dst, g, 0);
+                    dst += RPI * KPAD * 8;
+                }
             }
         } else {
             constexpr int RPI = NT / BK, ITERS = BMN / RPI;
@@ -139,20 +183,25 @@ __device__ __forceinline__ void load_operand(uint32_t sdst, const double* __rest
             constexpr int SEGS = PR > NT ? PR / NT : 1;              // passes needed to cover one k-row
             constexpr int KPI = PR > NT ? 1 : NT / PR;               // k-rows per pass
             const int k0 = tid / PR, mn0 = (tid % PR) * 2;
+            const int n_in = k_lim > k0 ? min(BK / KPI, (k_lim - k0 + KPI - 1) / KPI) : 0;      // k-rows inside the segment
+            const int n_all = k_end > k0 ? min(BK / KPI, (k_end - k0 + KPI - 1) / KPI) : 0;     // ... up to the next multiple of 4
 #pragma unroll
             for (int sg = 0; sg < SEGS; sg++) {
                 const int mn = mn0 + sg * NT * 2;
+                if (mn >= mn_end) continue;
                 const int mb = mn + 1 < mn_lim ? 16 : (mn < mn_lim ? 8 : 0);
-                const bool lane_on = mn < mn_end;
                 const double* src = g + (int64_t)k0 * ld + mn;
                 const int64_t step = (int64_t)KPI * ld;
-                const uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
-#pragma unroll
-                for (int i = 0; i < BK / KPI; i++) {
-                    const int k = k0 + KPI * i;
-                    const bool in = k < k_lim;
-                    cp_async16_if(dst + i * KPI * MPAD * 8, in ? src : g, in ? mb : 0, lane_on && k < k_end);
+                uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
+#pragma unroll 4
+                for (int i = 0; i < n_in; i++) {
+                    cp_async16(dst, mb ? src : g, mb);
                     src += step;
+                    dst += KPI * MPAD * 8;
+                }
+                for (int i = n_in; i < n_all; i++) {
+                    cp_async16(dst, g, 0);
+                    dst += KPI * MPAD * 8;
                 }
             }
         } else {
