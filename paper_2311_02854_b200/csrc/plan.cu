@@ -98,6 +98,7 @@ static const bool kTileOrder = [] { const char* e = getenv("DMRG_TILE_ORDER"); r
 // CTAs per thread-block cluster for the 64x64 tiles of stage 2 (1, 2, 4 or 8); tuning knob DMRG_CLUSTER.
 // Measured at cfg 5: clusters of 2 / 4 / 8 sibling tiles make stage 2 9-11 % SLOWER (gang scheduling costs more
 // occupancy than the shared L2 lines give back), so the default is 1 (no clusters).
+static const int kSplitSmall = [] { const char* e = getenv("DMRG_SPLIT_SMALL"); const int d = e ? atoi(e) : 0; return d > 0 ? d : 0; }();   // measurement knob, see emit_tiles
 static const int kCluster = [] { const char* e = getenv("DMRG_CLUSTER"); const int c = e ? atoi(e) : 1; return (c == 1 || c == 2 || c == 4 || c == 8) ? c : 1; }();
 
 static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
@@ -314,8 +315,24 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 });
             else
                 std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
+            // measurement knob: tiles of small-block jobs (min(M, N) < kSplitSmall) move, in order, to the end of the
+            // list and get a launch of their own, so that ncu reports the small-block batch (HBM-bound) apart from the
+            // large-block one (FP64-pipe bound).  Same kernel, same tiles, same results; default off.
+            size_t nbig = r.size();
+            if (kSplitSmall > 0 && kCluster == 1)
+                nbig = std::stable_partition(r.begin(), r.end(), [&](const TileRec& a) {
+                           const Job& j = jobs[a.t.job];
+                           int d = std::min(j.M, j.N);
+                           if (j.seg_end - j.seg_begin == 1) d = std::min(d, segs[j.seg_begin].K);   // stage 1: K = d_R
+                           return d >= kSplitSmall;
+                       }) - r.begin();
             // grid.x limit: split very long lists
             size_t i = 0;
+            if (nbig > 0 && nbig < r.size()) {
+                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)nbig, (stage == 2 && v == 0) ? kCluster : 1});
+                for (size_t j = 0; j < nbig; j++) tiles.push_back(r[j].t);
+                i = nbig;
+            }
             while (i < r.size()) {
                 const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);   // a multiple of every cluster size
                 P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n, (stage == 2 && v == 0) ? kCluster : 1});
