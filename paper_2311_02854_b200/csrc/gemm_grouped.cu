@@ -39,6 +39,12 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ double lds64(uint32_t addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
+    return v;
+}
+
 struct StageMeta { double alpha; uint32_t flags; int32_t ksteps; };
 
 // ---- mbarrier helpers (shared::cta) ----------------------------------------------------------------
@@ -263,10 +269,18 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const do
             }
         }
     } else {
+        // 32-bit shared addresses advanced by a constant per k-step: the k-loop holds no address arithmetic beyond
+        // the fragment offsets (indexing by kk made ptxas rematerialise lane ids and reload spilled bases per k-step)
+        uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(pa), b_addr = (uint32_t)__cvta_generic_to_shared(pb);
+        const uint32_t a_rs = 64u * a_sm, b_rs = 64u * b_sn, a_ks = 32u * a_sk, b_ks = 32u * b_sk;
+        const uint32_t a_end = a_addr + ksteps * a_ks;
 #pragma unroll 1
-        for (int kk = 0; kk < ksteps; kk++) {
+        for (; a_addr != a_end; a_addr += a_ks, b_addr += b_ks) {
             double a0[FMe], b0[FNe];
-            load(a0, b0, kk);
+#pragma unroll
+            for (int i = 0; i < FMe; i++) a0[i] = lds64(a_addr + i * a_rs);
+#pragma unroll
+            for (int j = 0; j < FNe; j++) b0[j] = lds64(b_addr + j * b_rs);
             mma(a0, b0);
         }
     }
@@ -353,6 +367,12 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
             if (j >= fn_eff) continue;
             const int col = n0 + wn0 + 8 * j + 2 * lc;
             double* p = c + (int64_t)r * job.ldc + col;
+            if (col + 1 < n0 + cx.n_lim && ((uintptr_t)p & 15) == 0) {   // the lane's pair as one 16-byte access (X, even-ld sigma rows)
+                double2 v = make_double2(acc[i][j][0], acc[i][j][1]);
+                if (beta1) { const double2 o = *reinterpret_cast<const double2*>(p); v.x += o.x; v.y += o.y; }
+                *reinterpret_cast<double2*>(p) = v;
+                continue;
+            }
             if (col < n0 + cx.n_lim) p[0] = beta1 ? p[0] + acc[i][j][0] : acc[i][j][0];
             if (col + 1 < n0 + cx.n_lim) p[1] = beta1 ? p[1] + acc[i][j][1] : acc[i][j][1];
         }

@@ -162,3 +162,26 @@ def test_stage1_is_n_merged():
     assert s["s1_flops"] > 0 and s["padded_flops"] / (s["s1_flops"] + s["s2_flops"]) < 1.5
     plan.destroy()
     ops.free()
+
+
+def test_split_small_knob_only_regroups_launches():
+    """DMRG_SPLIT_SMALL (measurement knob for ncu) moves small-block tiles into launches of their own: same tiles,
+    same work, more launches.  The knob is read when the library is loaded, hence the subprocesses."""
+    import json
+    import subprocess
+    import sys
+    code = ("import json, paper_2311_02854_b200 as g\n"
+            "from dmrg_workload.problem import make_direct_problem\n"
+            "pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)\n"
+            "ops, plan = g.load_problem(pr, structure_only=True)\n"
+            "print(json.dumps(plan.stats()))\n")
+    out = []
+    for knob in ("0", "16"):
+        env = dict(os.environ, DMRG_SPLIT_SMALL=knob, PYTHONPATH=ROOT)
+        r = subprocess.run([sys.executable, "-c", code], env=env, cwd=ROOT, capture_output=True, text=True, timeout=300)
+        assert r.returncode == 0, r.stderr
+        out.append(json.loads(r.stdout.strip().splitlines()[-1]))
+    a, b = out
+    for k in ("s1_tiles", "s2_tiles", "s1_flops", "s2_flops", "padded_flops", "tasks", "chunks"):
+        assert a[k] == b[k], k
+    assert b["launches"] > a["launches"]
