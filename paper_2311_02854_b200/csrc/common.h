@@ -85,9 +85,9 @@ struct TileShape { int bm, bn; };
 constexpr int NUM_VARIANTS = 5;
 extern const TileShape kVariants[NUM_VARIANTS];
 #ifndef DMRG_GEMM_BK
-#define DMRG_GEMM_BK 16
+#define DMRG_GEMM_BK 32
 #endif
-constexpr int GEMM_BK = DMRG_GEMM_BK;   // k-columns per pipeline stage (8, 16 or 32)
+constexpr int GEMM_BK = DMRG_GEMM_BK;   // k-columns per pipeline stage (8, 16 or 32); 32 measured best at cfg 5 / cfg 3
 
 struct GemmLaunch {       // one launch of one kernel variant
     int     variant;

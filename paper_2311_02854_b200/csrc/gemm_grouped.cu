@@ -242,12 +242,6 @@ template <int FM, int FN, int FMe, int FNe, bool DBUF>
 __device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const double* __restrict__ pa, const double* __restrict__ pb,
                                               int a_sm, int a_sk, int b_sn, int b_sk, int ksteps, int mode, double alpha) {
     static_assert(FM <= 4 && FN <= 4, "ragged-tile dispatch covers up to 4 x 4 fragments per warp");
-    auto load = [&](double (&af)[FMe], double (&bf)[FNe], int kk) {
-#pragma unroll
-        for (int i = 0; i < FMe; i++) af[i] = pa[8 * i * a_sm + 4 * kk * a_sk];
-#pragma unroll
-        for (int j = 0; j < FNe; j++) bf[j] = pb[8 * j * b_sn + 4 * kk * b_sk];
-    };
     auto mma = [&](double (&af)[FMe], double (&bf)[FNe]) {
         if (mode != 0) scale_frags<FMe, FNe>(af, bf, mode, alpha);
 #pragma unroll
@@ -256,15 +250,25 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const do
             for (int j = 0; j < FNe; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     };
     if (DBUF) {
+        uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(pa), b_addr = (uint32_t)__cvta_generic_to_shared(pb);
+        const uint32_t a_rs = 64u * a_sm, b_rs = 64u * b_sn, a_ks = 32u * a_sk, b_ks = 32u * b_sk;
+        auto loadu = [&](double (&af)[FMe], double (&bf)[FNe]) {
+#pragma unroll
+            for (int i = 0; i < FMe; i++) af[i] = lds64(a_addr + i * a_rs);
+#pragma unroll
+            for (int j = 0; j < FNe; j++) bf[j] = lds64(b_addr + j * b_rs);
+            a_addr += a_ks;
+            b_addr += b_ks;
+        };
         double a0[FMe], b0[FNe], a1[FMe], b1[FNe];
-        load(a0, b0, 0);
+        loadu(a0, b0);
 #pragma unroll 1
         for (int kk = 0; kk < ksteps; kk += 2) {
             const bool two = kk + 1 < ksteps;
-            if (two) load(a1, b1, kk + 1);
+            if (two) loadu(a1, b1);
             mma(a0, b0);
             if (two) {
-                if (kk + 2 < ksteps) load(a0, b0, kk + 2);
+                if (kk + 2 < ksteps) loadu(a0, b0);
                 mma(a1, b1);
             }
         }
@@ -505,13 +509,15 @@ constexpr size_t smem_bytes(int nst) {
 
 // variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, producer warps, register cap, double-buffered fragments>
 // Every variant uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step).  V0 was tuned on the B200 (macros kept
-// for re-tuning): 2 stages x 96 registers -> 4 CTAs/SM beat 3 stages x 128 registers with double-buffered
-// fragments -> 3 CTAs/SM by 0-7 % (cfg 5 / cfg 4); 4 stages (2 CTAs/SM) and a second producer warp both lost ~10 %.
+// for re-tuning).  Default: BK = 32, 2 stages (72 KB), 128 registers, no spills -> 3 CTAs/SM: half the mbarrier
+// round trips per flop of BK = 16.  Measured against BK = 16 / 2 stages / 96 registers / 4 CTAs/SM: cfg 5 +1.7 %,
+// cfg 3 +1.0 %, cfg 4 -1.6 %, cfg 2 -2.2 %.  BK = 16 with 3 stages x 128 registers (3 CTAs/SM) lost 4-11 %, 4 stages
+// (2 CTAs/SM) and a second producer warp ~10 %, double-buffered fragments at BK = 32 1-5 %.
 #ifndef V0_NST
 #define V0_NST 2
 #endif
 #ifndef V0_REG
-#define V0_REG 96
+#define V0_REG 128
 #endif
 #ifndef V0_DBUF
 #define V0_DBUF false
@@ -519,13 +525,14 @@ constexpr size_t smem_bytes(int nst) {
 #ifndef V0_NPW
 #define V0_NPW 1
 #endif
+constexpr int V1_NST = BK >= 32 ? 2 : 4;   // 128x128 stages must fit 227 KB
 #define V0 grouped_gemm_kernel<64, 64, 2, 2, V0_NST, V0_NPW, V0_REG, V0_DBUF>
-#define V1 grouped_gemm_kernel<128, 128, 4, 4, 4, 4, 96, false>    // large blocks, least operand traffic, 1 CTA/SM
+#define V1 grouped_gemm_kernel<128, 128, 4, 4, V1_NST, 4, 96, false>    // large blocks, least operand traffic, 1 CTA/SM
 #define V2 grouped_gemm_kernel<128, 32, 4, 1, 3, 1, 128, true>     // skinny N (stage 1 with a small R' sector)
 #define V3 grouped_gemm_kernel<32, 128, 1, 4, 3, 1, 128, true>     // skinny M
 #define V4 grouped_gemm_kernel<32, 32, 1, 1, 4, 1, 128, true>      // tiny blocks: one consumer warp
 constexpr int V0_T = 32 * (4 + V0_NPW), V1_T = 640, V2_T = 160, V3_T = 160, V4_T = 64;
-constexpr size_t V0_S = smem_bytes<64, 64>(V0_NST), V1_S = smem_bytes<128, 128>(4), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
+constexpr size_t V0_S = smem_bytes<64, 64>(V0_NST), V1_S = smem_bytes<128, 128>(V1_NST), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
                  V4_S = smem_bytes<32, 32>(4);
 
 }  // namespace

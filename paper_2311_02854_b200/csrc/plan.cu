@@ -93,7 +93,7 @@ constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are
 // split-K policy of stage 2 (see the comment at its use)
 constexpr double kCtaSlots = 148.0 * 4;     // resident 64x64 CTAs on a B200
 static const double kSplitWaves = [] { const char* e = getenv("DMRG_SPLIT_WAVES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 200.0; }();
-static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 48.0; }();   // 48 stages: K = 768
+static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 768.0 / GEMM_BK; }();   // K = 768 per part at least
 static const bool kTileOrder = [] { const char* e = getenv("DMRG_TILE_ORDER"); return !e || atoi(e) != 0; }();   // knob: 0 = pure cost order
 // CTAs per thread-block cluster for the 64x64 tiles of stage 2 (1, 2, 4 or 8); tuning knob DMRG_CLUSTER.
 // Measured at cfg 5: clusters of 2 / 4 / 8 sibling tiles make stage 2 9-11 % SLOWER (gang scheduling costs more
