@@ -27,7 +27,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "fp64_tflops_per_hpsi"
-NCU_DRAM_BYTES_PER_HPSI = {"cfg5": 2.59e12}   # profiles/r1_cfg5_launch_summary.csv (round 1)
+NCU_DRAM_BYTES_PER_HPSI = {"cfg5": 1.53e12}   # 42 GEMM launches of one H psi in profiles/r1_cfg5_launches.csv (round 1, final kernel)
 UNIT = "TFLOP/s"
 
 
