@@ -67,7 +67,7 @@ struct Job {
     int32_t  ldc, M, N;
     int32_t  seg_begin, seg_end;
     uint32_t flags;
-    int32_t  pad_;
+    int32_t  nstages;   // pipeline stages of GEMM_BK k-columns over all non-identity segments (planner)
 };
 static_assert(sizeof(Job) == 40, "Job layout");
 

@@ -30,10 +30,6 @@ constexpr int KPAD = BK + 4;   // row stride of a k-contiguous tile (20 = 4 mod 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
 }
-__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src, int src_bytes) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
-}
-
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -86,10 +82,6 @@ __device__ __forceinline__ void scale_frags(double (&af)[FM], double (&bf)[FN], 
 }
 
 // predicated cp.async: no instruction is issued when `on` is false
-__device__ __forceinline__ void cp_async16_if(uint32_t dst, const void* src, int src_bytes, bool on) {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %3, 0;\n@p cp.async.cg.shared.global [%0], [%1], 16, %2;\n}\n" ::"r"(dst), "l"(src),
-                 "r"(src_bytes), "r"((int)on) : "memory");
-}
 __device__ __forceinline__ void cp_async8_if(uint32_t dst, const void* src, int src_bytes, bool on) {
     asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %3, 0;\n@p cp.async.ca.shared.global [%0], [%1], 8, %2;\n}\n" ::"r"(dst), "l"(src),
                  "r"(src_bytes), "r"((int)on) : "memory");
@@ -412,7 +404,7 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     const Job job = jobs[tile.job];
     const int m0 = tile.m0, n0 = tile.n0;
     const int m_lim = tile.rows, n_lim = tile.cols;   // <= BM, BN and inside the matrix (planner)
-    const int nstages = job.pad_;
+    const int nstages = job.nstages;
     auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
 
     const uint32_t full_u32 = (uint32_t)__cvta_generic_to_shared(bar_full);

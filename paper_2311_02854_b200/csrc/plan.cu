@@ -456,7 +456,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = (int)ncols;
                 jb.seg_begin = (int32_t)segs.size(); jb.seg_end = jb.seg_begin + 1;
                 jb.flags = (SP_X << JOB_C_SPACE_SHIFT);
-                jb.pad_ = (dRi + GEMM_BK - 1) / GEMM_BK;
+                jb.nstages = (dRi + GEMM_BK - 1) / GEMM_BK;
                 segs.push_back(s);
                 const int v = choose_variant(jb.M, jb.N);
                 const int bm = kVariants[v].bm, bn = kVariants[v].bn;
@@ -467,9 +467,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     for (auto& b : cut_n)
                         recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
                 padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
-                stage_flops += 2.0 * frag_area(jb.M, jb.N) * 16.0 * jb.pad_;
-                warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * 16.0 * jb.pad_;
-                tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * 16.0 * jb.pad_;
+                stage_flops += 2.0 * frag_area(jb.M, jb.N) * (double)GEMM_BK * jb.nstages;
+                warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * (double)GEMM_BK * jb.nstages;
+                tile_flops += 2.0 * (double)cut_m.size() * cut_n.size() * bm * bn * (double)GEMM_BK * jb.nstages;
                 jobs.push_back(jb);
                 s1_jobs++;
                 xtop += rows * ldx;
@@ -556,9 +556,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
             cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
             padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
-            stage_flops += 2.0 * frag_area(OB.dl, OB.dr) * 16.0 * g.nst;
-            warp_flops += 2.0 * warp_area(cut_m, cut_n, g.variant) * 16.0 * g.nst;
-            tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * 16.0 * g.nst;
+            stage_flops += 2.0 * frag_area(OB.dl, OB.dr) * (double)GEMM_BK * g.nst;
+            warp_flops += 2.0 * warp_area(cut_m, cut_n, g.variant) * (double)GEMM_BK * g.nst;
+            tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * (double)GEMM_BK * g.nst;
             alg_bytes += 16.0 * OB.dl * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
             int part_no = 0;
@@ -592,7 +592,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());
                 segs.insert(segs.end(), gemm_segs.begin(), gemm_segs.end());
                 jb.seg_end = (int32_t)segs.size();
-                jb.pad_ = g.nst;
+                jb.nstages = g.nst;
                 push_tiles(recs2, (int32_t)jobs.size(), g.nst + 1.0);
                 jobs.push_back(jb);
             } else {
@@ -618,7 +618,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     if (nparts == 0) segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());   // identity-L terms ride with part 0
                     segs.insert(segs.end(), gemm_segs.begin() + sbeg, gemm_segs.begin() + send);
                     pj.seg_end = (int32_t)segs.size();
-                    pj.pad_ = pst;
+                    pj.nstages = pst;
                     push_tiles(recs2, (int32_t)jobs.size(), pst + 1.0);
                     jobs.push_back(pj);
                     part_off.push_back(ptop);
