@@ -91,7 +91,7 @@ static const int64_t kMaxMergedCols = [] { const char* e = getenv("DMRG_MAX_MERG
 constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are offsets into the packed R store
 
 // split-K policy of stage 2 (see the comment at its use)
-constexpr double kCtaSlots = 148.0 * 4;     // resident 64x64 CTAs on a B200
+constexpr double kCtaSlots = 148.0 * 4;     // unit of the split-K wave count: 592 CTA slots (4 per SM with 16-column stages; the 32-column default keeps 3 resident -- the DMRG_SPLIT_WAVES sweep of DESIGN.md section 9 is in these units)
 static const double kSplitWaves = [] { const char* e = getenv("DMRG_SPLIT_WAVES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 200.0; }();
 static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 768.0 / GEMM_BK; }();   // K = 768 per part at least
 static const bool kTileOrder = [] { const char* e = getenv("DMRG_TILE_ORDER"); return !e || atoi(e) != 0; }();   // knob: 0 = pure cost order
