@@ -4,7 +4,8 @@
   x0 normalised; iteration k: w_k = H b_k; G_ik = b_i.w_k; lowest eigenpair (theta, y) of
   the m x m matrix G; x = sum y_i b_i; r = sum y_i w_i - theta x; stop if |r| <= tol;
   t = r * den/(den^2 + delta^2), den = theta - Hd, delta = 1e-3; orthogonalise t against
-  b_1..b_m by classical Gram-Schmidt applied twice; normalise -> b_{m+1}.
+  b_1..b_m by MODIFIED Gram-Schmidt (one basis vector at a time, each projection taken
+  from the already-updated t) applied twice; normalise -> b_{m+1}.
   When m reaches max_space the basis collapses to {x}.  One iteration = one H psi.
 """
 import numpy as np

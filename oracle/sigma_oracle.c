@@ -59,7 +59,8 @@ int oracle_num_threads(void) {
 #endif
 }
 
-static optab_t *build_optabs(const problem_t *P, double ***owned, int *nowned) {
+/* form_values = 0: structure only (which blocks exist); used by opair_count, which needs no arithmetic */
+static optab_t *build_optabs(const problem_t *P, double ***owned, int *nowned, int form_values) {
     optab_t *T = (optab_t *)calloc(P->nops, sizeof(optab_t));
     *owned = (double **)calloc(P->nops, sizeof(double *));
     *nowned = 0;
@@ -77,7 +78,7 @@ static optab_t *build_optabs(const problem_t *P, double ***owned, int *nowned) {
         if (kind != 7) {
             for (int64_t b = op[6]; b < op[6] + op[7]; b++) {
                 const int64_t *bd = P->blocks + 3 * b;
-                T[o].rowblk[bd[0]] = (double *)(P->values + bd[2]);
+                T[o].rowblk[bd[0]] = form_values ? (double *)(P->values + bd[2]) : (double *)P->values;   /* presence only */
             }
         }
     }
@@ -98,7 +99,7 @@ static optab_t *build_optabs(const problem_t *P, double ***owned, int *nowned) {
                 if (T[P->lin_op[i]].rowblk[r]) has = 1;
             if (has) total += (size_t)sec[3 * r + 2] * sec[3 * c + 2];
         }
-        double *buf = (double *)calloc(total ? total : 1, sizeof(double));
+        double *buf = (double *)calloc(form_values && total ? total : 1, sizeof(double));
         (*owned)[(*nowned)++] = buf;
         size_t off = 0;
         for (int r = 0; r < nsec; r++) {
@@ -110,10 +111,11 @@ static optab_t *build_optabs(const problem_t *P, double ***owned, int *nowned) {
                 const double *src = T[P->lin_op[i]].rowblk[r];
                 if (!src) continue;
                 has = 1;
+                if (!form_values) continue;
                 double cf = P->lin_coef[i];
                 for (size_t e = 0; e < n; e++) buf[off + e] += cf * src[e];
             }
-            if (has) { T[o].rowblk[r] = buf + off; off += n; }
+            if (has) { T[o].rowblk[r] = form_values ? buf + off : buf; off += n; }
         }
     }
     return T;
@@ -236,7 +238,7 @@ int64_t opair_sigma(const int32_t *secL, int nsecL, const int32_t *secR, int nse
     problem_t P = make_problem(secL, nsecL, secR, nsecR, ops, nops, blocks, values, lin_ptr, lin_op, lin_coef,
                                site_ops, site_parity, nsite, term_coef, term_idx, nterms, layout, npsiblk);
     double **owned; int nowned;
-    optab_t *T = build_optabs(&P, &owned, &nowned);
+    optab_t *T = build_optabs(&P, &owned, &nowned, 1);
     int64_t ntask;
     task_t *tasks = enumerate_tasks(&P, T, &ntask, 0);
     qsort(tasks, ntask, sizeof(task_t), cmp_task_out);
@@ -287,6 +289,43 @@ int64_t opair_sigma(const int32_t *secL, int nsecL, const int32_t *secR, int nse
     return done;
 }
 
+
+/* The cost measure alone (Table 1 caption: the FLOP count of a GEMM C = A B with shapes
+ * (M,K)(K,N) is 2MNK): the same (term, psi block, dot transition) expansion as opair_sigma, no arithmetic.
+ * flops_out = sum over tasks of 2 dLi dRi dRo (if the R factor is not the identity) + 2 dLo dLi dRo (if the
+ * L factor is not the identity).  values may be NULL (only block presence is used).  Returns the task count. */
+int64_t opair_count(const int32_t *secL, int nsecL, const int32_t *secR, int nsecR,
+    const int64_t *ops, int nops, const int64_t *blocks, const double *values,
+    const int64_t *lin_ptr, const int32_t *lin_op, const double *lin_coef,
+    const double *site_ops, const int32_t *site_parity, int nsite,
+    const double *term_coef, const int32_t *term_idx, int64_t nterms,
+    const int64_t *layout, int64_t npsiblk, int64_t psi_size,
+    const int32_t *only_out, int n_only, double *flops_out) {
+    static const double dummy = 0.0;
+    (void)psi_size;
+    problem_t P = make_problem(secL, nsecL, secR, nsecR, ops, nops, blocks, values ? values : &dummy, lin_ptr, lin_op, lin_coef,
+                               site_ops, site_parity, nsite, term_coef, term_idx, nterms, layout, npsiblk);
+    double **owned; int nowned;
+    optab_t *T = build_optabs(&P, &owned, &nowned, 0);
+    int64_t ntask;
+    task_t *tasks = enumerate_tasks(&P, T, &ntask, 0);
+    char *want = (char *)malloc(npsiblk);
+    memset(want, n_only > 0 ? 0 : 1, npsiblk);
+    for (int i = 0; i < n_only; i++) want[only_out[i]] = 1;
+    double flops = 0.0; int64_t done = 0;
+    for (int64_t k = 0; k < ntask; k++) {
+        const task_t *t = &tasks[k];
+        if (!want[t->out_blk]) continue;
+        if (t->Rm) flops += 2.0 * t->dLi * t->dRi * t->dRo;
+        if (t->Lm) flops += 2.0 * t->dLo * t->dLi * t->dRo;
+        done++;
+    }
+    if (flops_out) *flops_out = flops;
+    free(want); free(tasks);
+    free_optabs(T, nops, owned, nowned);
+    return done;
+}
+
 /* Diagonal of H in the psi layout: terms whose four factors are all block-diagonal. */
 int64_t opair_hdiag(const int32_t *secL, int nsecL, const int32_t *secR, int nsecR,
     const int64_t *ops, int nops, const int64_t *blocks, const double *values,
@@ -297,7 +336,7 @@ int64_t opair_hdiag(const int32_t *secL, int nsecL, const int32_t *secR, int nse
     problem_t P = make_problem(secL, nsecL, secR, nsecR, ops, nops, blocks, values, lin_ptr, lin_op, lin_coef,
                                site_ops, site_parity, nsite, term_coef, term_idx, nterms, layout, npsiblk);
     double **owned; int nowned;
-    optab_t *T = build_optabs(&P, &owned, &nowned);
+    optab_t *T = build_optabs(&P, &owned, &nowned, 1);
     int64_t ntask;
     task_t *tasks = enumerate_tasks(&P, T, &ntask, 1);
     memset(diag, 0, psi_size * sizeof(double));
