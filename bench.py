@@ -6,8 +6,11 @@
 A step is one Davidson iteration: one H psi (dmrg_sigma: stage-1 and stage-2 grouped GEMMs) plus the
 device-side Davidson vector work of that iteration (subspace dots, Ritz vector, residual,
 preconditioner, orthogonalisation); the per-bond H diagonal is computed once at the start of the timed
-region.  value = algorithmic FP64 TFLOP/s over the whole timed region (the paper's cost measure: 2 dL dR dR'
-+ 2 dL' dL dR' per term and symmetry-block combination), ms_per_step = ms per H psi.
+region.  value = EXECUTED FP64 TFLOP/s over the whole timed region: the flops of the GEMMs the plan runs (the
+paper's cost measure 2MNK per GEMM, PAPER.md:151, after the planner's de-duplication of X = psi R^T products;
+unpadded), ms_per_step = ms per H psi.  The canonical count (one GEMM pair per term and symmetry-block
+combination, no de-duplication) and the rate on it are printed beside it (`canonical_flops_per_hpsi`,
+`canonical_tflops`) so that a smarter plan cannot inflate the rate.
 Inputs are seeded synthetic (dmrg_workload), resident in HBM before the timed region starts.
 With N > 1 (torchrun) every rank runs an independent replica of the same bond ("replicas only":
 BASELINE.json fixes the path to one GPU with no sharding and no collectives).
@@ -27,7 +30,9 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "fp64_tflops_per_hpsi"
-NCU_DRAM_BYTES_PER_HPSI = {"cfg5": 1.53e12}   # 42 GEMM launches of one H psi in profiles/r1_cfg5_launches.csv (round 1, final kernel)
+# dram__bytes_read.sum + dram__bytes_write.sum of all GEMM launches of one H psi, from a committed ncu launch list
+# (NOT measured by this run): config -> (bytes, source)
+NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (1.53e12, "profiles/r1_cfg5_launches.csv (round 1 kernel)")}
 UNIT = "TFLOP/s"
 
 
@@ -42,7 +47,20 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
+                    help="dmrg_plan_options field (copy_mode, split_waves, min_split_stages, max_merged_cols, "
+                         "cost_order_only, split_small, release_r_store); repeatable")
+    ap.add_argument("--operators", default="default", choices=["default", "direct", "renorm"],
+                    help="cfg3-5 operator values: direct fill (seeded random blocks) or GPU renormalization (NEXT-1)")
     return ap.parse_args()
+
+
+def plan_options(args):
+    out = {}
+    for kv in args.opt:
+        k, v = kv.split("=", 1)
+        out[k] = float(v) if k == "split_waves" else int(v)
+    return out
 
 
 class ClockSampler:
@@ -144,12 +162,12 @@ def oracle_term_sample(pr, psi, total_flops, seconds, k=0):
 
 
 def dist_env():
-    from paper_2311_02854_b200 import replicas
-    return replicas.dist_env()
+    return (int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0")))
 
 
 def run_reference(args):
-    """--impl reference: for this tier the reference arm is the CPU oracle, timed as it stands."""
+    """--impl reference: for this tier the reference arm is the CPU oracle, timed as it stands.  It stands on
+    oracle/ and dmrg_workload/ alone: the product package is never imported here."""
     rank, world, _ = dist_env()
     if rank != 0:
         return
@@ -157,9 +175,8 @@ def run_reference(args):
     import oracle
     pr = make_config(args.config)
     psi = random_psi(pr.psi_size, 5)
-    import paper_2311_02854_b200 as g
-    ops, plan = g.load_problem(pr, structure_only=True)   # host planner only: flop count of the full workload
-    total = plan.stats()["canon_flops"]
+    total = oracle.opair_count(pr)["flops"]   # the oracle's own cost counter (pinned: tests/test_oracle_flopcount.py)
+    assert "paper_2311_02854_b200" not in sys.modules
     # Each step = the oracle, as it stands, on a bounded SAMPLE of the workload: every stride-th operator-pair term
     # (all sigma blocks), sized so that the whole run takes a few minutes.  (Sampling sigma blocks instead would
     # make every step pay the oracle's full term expansion and its 8 GB of intermediates, ~80 s at cfg 5.)
@@ -216,7 +233,8 @@ def main():
     free1, _ = torch.cuda.mem_get_info()
     ws = int(args.workspace_gib * 2 ** 30) if args.workspace_gib > 0 else int(min(24 * 2 ** 30, 0.25 * free1))
     t0 = time.perf_counter()
-    plan = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, ws)
+    popts = plan_options(args)
+    plan = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, ws, **popts)
     t_plan = time.perf_counter() - t0
     st = plan.stats()
     n = plan.psi_size
@@ -251,7 +269,8 @@ def main():
     clk = clocks.stop()
     ms_total = e0.elapsed_time(e1)
     assert res["iters"] == K
-    flops = st["canon_flops"]
+    flops_canon = st["canon_flops"]
+    flops = st["s1_flops"] + st["s2_flops"]       # executed: what the GEMM launches of one H psi compute (unpadded)
     thr, ms_step = replicas.job_throughput(flops, ms_total / K, world, "cuda")   # max over ranks
     value = thr * 1e-12
 
@@ -262,9 +281,9 @@ def main():
         a.record(stream); plan.sigma(x, sig, stream); b.record(stream); torch.cuda.synchronize()
         ts.append(a.elapsed_time(b))
     ms_sigma = float(np.median(ts))
-    # The GEMM kernel's launches of one H psi overlap on several streams (tile variants; stage 1 of the next chunk
-    # under stage 2 of this one), so "launch duration" is the device time of the whole dmrg_sigma call, which is
-    # > 99 % GEMM launches (profiles/).  A separate, serialised call gives the per-stage split.
+    # dmrg_sigma enqueues its launches back to back on the caller's stream (per chunk: stage 1, stage 2, split-K
+    # reduce); "launch duration" of the roofline is the device time of the whole call, which is > 99 % GEMM launches
+    # (profiles/).  A second call with the library's per-group events gives the per-stage split.
     plan.set_timing(True)
     plan.sigma(x, sig, stream)
     s1_ms, s2_ms, _ = plan.stage_ms()
@@ -273,13 +292,18 @@ def main():
     achieved = flops / (gemm_ms * 1e-3) * 1e-12
     # DRAM bytes of all GEMM launches of one H psi, from the ncu pass committed as profiles/r1_cfg5_launches.csv
     # (dram__bytes_read.sum + dram__bytes_write.sum); only meaningful for the configuration that was profiled
-    traffic = NCU_DRAM_BYTES_PER_HPSI.get(args.config)
+    traffic, traffic_src = NCU_DRAM_BYTES_PER_HPSI.get(args.config, (None, None))
     roofline = {"bound": "tensor", "achieved": achieved, "peak": peak_dmma, "unit": "TFLOP/s", "frac": achieved / peak_dmma,
-                "traffic": traffic, "traffic_unit": "bytes per H psi (ncu, all GEMM launches)", "kernel": "grouped_gemm_kernel (DMMA.8x8x4, all launches of one H psi)",
-                "peak_source": "measured live: dmrg_fp64_peak_tflops(DMMA); nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                "flops": "executed (s1_flops + s2_flops of the plan, unpadded)",
+                "traffic": traffic, "traffic_unit": "bytes per H psi (ncu, all GEMM launches)",
+                "traffic_source": f"NOT this run: {traffic_src}" if traffic else None,
+                "kernel": "grouped_gemm_kernel (DMMA.8x8x4, all launches of one H psi)",
+                "peak_source": "builder probe, measured live in this process: dmrg_fp64_peak_tflops(DMMA) (csrc/fp64_peak.cu); MEASURED_PEAKS.json "
+                               "has no FP64 entry; nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                "canonical_tflops": flops_canon / (gemm_ms * 1e-3) * 1e-12, "canonical_frac": flops_canon / (gemm_ms * 1e-3) * 1e-12 / peak_dmma,
                 "peak_dfma_measured": peak_dfma, "stage1_ms_serialised": s1_ms, "stage2_ms_serialised": s2_ms, "hpsi_ms": ms_sigma, "launches_per_hpsi": int(st["launches"]),
-                "executed_flops_per_hpsi": st["s1_flops"] + st["s2_flops"], "padded_flops_per_hpsi": st["padded_flops"],
-                "algorithmic_flops_per_hpsi": flops, "algorithmic_bytes_per_hpsi": st["alg_bytes"],
+                "executed_flops_per_hpsi": flops, "padded_flops_per_hpsi": st["padded_flops"],
+                "canonical_flops_per_hpsi": flops_canon, "algorithmic_bytes_per_hpsi": st["alg_bytes"],
                 "hbm_gbs_if_streamed": st["alg_bytes"] / (gemm_ms * 1e-3) * 1e-9}
 
     # ---- end to end through the C ABI with host buffers ---------------------------------------------
@@ -303,10 +327,10 @@ def main():
     cpu = None
     parity = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = oracle_term_sample(pr, psi_h, flops, args.cpu_seconds)
+        cpu = oracle_term_sample(pr, psi_h, flops_canon, args.cpu_seconds)
         # parity on sampled sigma blocks (all terms), in the launch configuration that was timed; the oracle's
         # fixed cost (full term expansion, all intermediates) dominates this call, so it is not the cpu_baseline
-        chk = oracle_sample(pr, psi_h, flops, 1.0)
+        chk = oracle_sample(pr, psi_h, flops_canon, 1.0)
         blocks, refs = chk["blocks"], chk["sigma"]
         got = sig.cpu().numpy()
         nrm = float(np.linalg.norm(got))
@@ -327,6 +351,8 @@ def main():
                 "clocks": clk, "e2e": e2e, "gpu_launches": int(K * (st["launches"] + 15) + 4),   # GEMM / reduce launches + 15 Davidson vector kernels per step, + hdiag, start-up
                 "roofline": roofline, "cpu_baseline": cpu,
                 "ms_per_hpsi_kernel_only": ms_sigma, "frac_of_fp64_peak_whole_step": value / world / peak_dmma,
+                "canonical_flops_per_hpsi": flops_canon, "canonical_tflops": world * flops_canon / (ms_step * 1e-3) * 1e-12,
+                "plan_options": popts,
                 "parity_sampled": parity,
                 "footprint_gb": {"operator_store": ops.device_bytes / 1e9, "plan_and_workspace": st["plan_device_bytes"] / 1e9,
                                  "davidson_vectors": (2 * max(W, K) + 3) * 8 * n / 1e9},

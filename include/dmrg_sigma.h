@@ -115,18 +115,54 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *   terms      [host] nterms operator-pair terms (all four slots; identity = op -1 / site op 0..)
  *   site_ops   [host] nsite row-major 4x4 dot matrices; site_parity[i] = fermion parity of site op i
  *   n_total, two_sz_total: target quantum numbers of psi
- *   workspace_bytes: HBM the plan may use for the X intermediates (0 = default 8 GiB, clamped to
- *              what one term needs); terms are processed in chunks that fit it.
+ *   workspace_bytes: HBM the plan may use for the X intermediates (0 = default 8 GiB, raised to
+ *              what the largest single term needs); terms are processed in chunks that fit it.
+ *              The limit covers the X intermediates only: the split-K partial sigma tiles of a chunk live
+ *              behind them in the same allocation (dmrg_plan_stat(16) = doubles actually allocated).
  *              Besides the workspace the plan owns a packed copy of the R-side blocks as stage 1 uses them
  *              (about the size of the R half of the store, twice where a block is used both ways) and a
  *              padded copy of psi; dmrg_plan_stat(8) reports the total.
  * Fails with DMRG_ECHARGE if a term does not conserve (N, 2Sz).  The plan borrows `ops`
  * (which must outlive it) and owns its descriptors and workspace.  Synchronous.
+ *
+ * dmrg_plan_create_opts: the same with every planner / kernel policy spelled out (there are no
+ * environment variables).  Zero-initialise the struct for the defaults; fields:
+ *   workspace_bytes    as above
+ *   copy_mode          how operand tiles are staged global -> shared by the GEMM kernel:
+ *                      0 = default (2); 1 = 16-byte cp.async (LDGSTS) issued by a 32-lane producer warp;
+ *                      2 = TMA: one cp.async.bulk.tensor.2d per operand and pipeline stage through per-matrix
+ *                      tensor maps the plan builds (the TMA unit zero-fills ragged tails)
+ *   split_waves        split-K granularity of stage 2: a sigma block's K-loop is cut into parts no longer than
+ *                      1/split_waves of the chunk's ideally balanced run time (0 = default 200)
+ *   min_split_stages   ... but never shorter than this many GEMM_BK-wide pipeline stages (0 = default 24)
+ *   max_merged_cols    widest N-merged stage-1 GEMM in columns (0 = default 4096)
+ *   cost_order_only    1 = launch tiles in pure cost order; 0 (default) = inside a cost bucket, stage-2 tiles
+ *                      follow (L sector of the sigma block, split-K part) so that they share L blocks in L2
+ *   split_small        measurement aid for ncu (default 0 = off): tiles of jobs with min(M, N, K) < split_small
+ *                      get a launch of their own (same tiles, same results, more launches)
+ *   release_r_store    1 = after packing, free the store's R-side blocks (the plan's packed copy is then the only
+ *                      one; the store can serve no further dmrg_plan_create); 0 = keep (default)
  */
+typedef struct {
+    int64_t workspace_bytes;
+    int32_t copy_mode;
+    int32_t min_split_stages;
+    double  split_waves;
+    int32_t max_merged_cols;
+    int32_t cost_order_only;
+    int32_t split_small;
+    int32_t release_r_store;
+    int32_t reserved[8];
+} dmrg_plan_options;
+
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,
                      const double* site_ops, const int32_t* site_parity, int32_t nsite,
                      int32_t n_total, int32_t two_sz_total, int64_t workspace_bytes,
                      dmrg_plan** out);
+int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,
+                          const double* site_ops, const int32_t* site_parity, int32_t nsite,
+                          int32_t n_total, int32_t two_sz_total, const dmrg_plan_options* options,
+                          dmrg_plan** out);
 void    dmrg_plan_destroy(dmrg_plan* plan);
 int64_t dmrg_plan_psi_size(const dmrg_plan* plan);            /* doubles in psi / sigma         */
 int64_t dmrg_plan_num_psi_blocks(const dmrg_plan* plan);
@@ -140,8 +176,9 @@ int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host
  *  7 kernel launches per sigma   8 device bytes held by the plan (descriptors + workspace)
  *  9 algorithmic operand bytes read per sigma (operator blocks once per use + X write/read + psi/sigma)
  * 10 stage-1 tiles   11 stage-2 tiles   12 canonical flops (= key 1 without de-duplication)
- * 13 executed flops with every segment's K padded to whole 16-wide pipeline stages
+ * 13 executed flops with every segment's K padded to whole GEMM_BK(= 32)-wide pipeline stages
  * 14 the same with M and N padded to whole tiles as well; 15 ... padded to each tile's most loaded warp
+ * 16 doubles allocated for the X workspace (X intermediates + split-K partial tiles of the largest chunk)
  *                                           */
 double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
 
@@ -169,7 +206,9 @@ int dmrg_hdiag(dmrg_plan* plan, double* diag, void* cuda_stream);
  *   iteration k: w_k = H b_k (dmrg_sigma); G_ik = b_i.w_k; (theta, y) = lowest eigenpair of G;
  *   x = sum y_i b_i; r = sum y_i w_i - theta x; stop if |r| <= tol; t = r den/(den^2+delta^2),
  *   den = theta - Hd, delta = 1e-3; orthogonalise t against b_1..b_m (classical Gram-Schmidt twice),
- *   normalise -> b_{m+1}.  At m = max_space the basis collapses to {x}.  One iteration = one H psi.
+ *   normalise -> b_{m+1}.  At m = max_space (>= 2) the basis collapses to {x} and H x is re-evaluated (that
+ *   H psi counts as an iteration, as in the oracle).  One iteration = one H psi.  A zero initial guess is
+ *   DMRG_EINVAL; a correction that vanishes after orthogonalisation ends the run (DMRG_ENOCONV, text says why).
  *   All vector work runs on the device; the host sees only O(m) scalars per iteration.
  *   thetas [host, may be NULL] receives theta_k for k < *iters (capacity max_iter).
  * Returns DMRG_OK if |r| <= tol, DMRG_ENOCONV if max_iter was reached (outputs still valid).

@@ -16,7 +16,8 @@
  *   Hamiltonian"), term by term.
  *
  * All arithmetic FP64, plain loops, no blocking, no reordering beyond the formula.
- * OpenMP only distributes independent output blocks over threads.
+ * OpenMP only distributes independent output blocks (or, for a handful of blocks, independent output rows) over
+ * threads; the summation order of every element is fixed.
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -249,7 +250,15 @@ int64_t opair_sigma(const int32_t *secL, int nsecL, const int32_t *secR, int nse
     { int64_t k = 0; for (int64_t b = 0; b <= npsiblk; b++) { while (k < ntask && tasks[k].out_blk < b) k++; start[b] = k; } }
     memset(sigma, 0, psi_size * sizeof(double));
     double flops = 0.0; int64_t done = 0;
-#pragma omp parallel for schedule(dynamic, 1) reduction(+ : flops, done)
+    /* Threads: whole output blocks are dealt to threads; when only a few blocks are asked for (fewer than threads),
+     * the rows i of each product are dealt to threads instead.  Either way every output element is summed by one
+     * thread in the same order (tasks in (term, input block) order, kk ascending): the result does not depend on
+     * the thread count or on which of the two modes ran. */
+    int rows_mode = 0;
+#ifdef _OPENMP
+    rows_mode = (n_only > 0 && n_only < omp_get_max_threads());
+#endif
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : flops, done) if (!rows_mode)
     for (int64_t ob = 0; ob < npsiblk; ob++) {
         if (!want[ob]) continue;
         double *out = sigma + layout[7 * ob + 6];
@@ -261,6 +270,7 @@ int64_t opair_sigma(const int32_t *secL, int nsecL, const int32_t *secR, int nse
             double *X = (double *)calloc((size_t)dLi * dRo, sizeof(double));
             if (!t->Rm) memcpy(X, x, sizeof(double) * dLi * dRi);
             else {
+#pragma omp parallel for schedule(static) if (rows_mode && (double)dLi * dRi * dRo > 2e5)
                 for (int i = 0; i < dLi; i++)
                     for (int kk = 0; kk < dRi; kk++) {
                         double a = x[(size_t)i * dRi + kk];
@@ -272,6 +282,7 @@ int64_t opair_sigma(const int32_t *secL, int nsecL, const int32_t *secR, int nse
             /* step 2 + reduction (Eqs. 12-13): sigma[i][j] += alpha * sum_k OL[i][k] X[k][j] */
             if (!t->Lm) { for (size_t e = 0; e < (size_t)dLo * dRo; e++) out[e] += t->alpha * X[e]; }
             else {
+#pragma omp parallel for schedule(static) if (rows_mode && (double)dLo * dLi * dRo > 2e5)
                 for (int i = 0; i < dLo; i++)
                     for (int kk = 0; kk < dLi; kk++) {
                         double a = t->alpha * (t->Lt ? t->Lm[(size_t)kk * dLo + i] : t->Lm[(size_t)i * dLi + kk]);

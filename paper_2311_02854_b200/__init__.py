@@ -23,10 +23,17 @@ PSIBLK_DT = np.dtype([("il", "<i4"), ("c1", "<i4"), ("c2", "<i4"), ("ir", "<i4")
 assert SECTOR_DT.itemsize == 12 and OP_DT.itemsize == 40 and BLOCK_DT.itemsize == 16
 assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
 
-STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
-             "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops")
+PLANOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("min_split_stages", "<i4"), ("split_waves", "<f8"),
+                       ("max_merged_cols", "<i4"), ("cost_order_only", "<i4"), ("split_small", "<i4"), ("release_r_store", "<i4"),
+                       ("reserved", "<i4", (8,))], align=True)
+assert PLANOPT_DT.itemsize == 72
+COPY_LDGSTS, COPY_TMA = 1, 2
 
-EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_destroy",
+STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
+             "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops",
+             "xws_elems")
+
+EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_create_opts", "dmrg_plan_destroy",
            "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",
            "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version")
@@ -57,6 +64,8 @@ def lib():
         L.dmrg_ops_device_bytes.restype = i64
         L.dmrg_plan_create.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, i64, C.POINTER(vp)]
         L.dmrg_plan_create.restype = C.c_int
+        L.dmrg_plan_create_opts.argtypes = [vp, vp, i64, vp, vp, i32, i32, i32, vp, C.POINTER(vp)]
+        L.dmrg_plan_create_opts.restype = C.c_int
         L.dmrg_plan_destroy.argtypes = [vp]
         L.dmrg_plan_destroy.restype = None
         L.dmrg_plan_psi_size.argtypes = [vp]
@@ -166,8 +175,10 @@ class OpsStore:
 class Plan:
     """dmrg_plan_create and the calls that take a plan (dmrg_sigma, dmrg_hdiag, dmrg_davidson)."""
 
-    def __init__(self, ops, term_coef, term_idx, site_ops, site_parity, n_total, two_sz_total, workspace_bytes=0):
-        """term_idx: int [nterms,6] (op_l, trans_l, dot1, dot2, op_r, trans_r)."""
+    def __init__(self, ops, term_coef, term_idx, site_ops, site_parity, n_total, two_sz_total, workspace_bytes=0, **options):
+        """term_idx: int [nterms,6] (op_l, trans_l, dot1, dot2, op_r, trans_r).
+        options: fields of dmrg_plan_options (copy_mode, split_waves, min_split_stages, max_merged_cols,
+        cost_order_only, split_small, release_r_store); passing any selects dmrg_plan_create_opts."""
         self._h = None
         self.ops = ops   # keep the store alive: the plan borrows it
         ti = np.asarray(term_idx).reshape(-1, 6)
@@ -178,8 +189,18 @@ class Plan:
         so = np.ascontiguousarray(site_ops, dtype=np.float64).reshape(-1, 16)
         sp = np.ascontiguousarray(site_parity, dtype=np.int32)
         h = C.c_void_p()
-        _check(lib().dmrg_plan_create(ops._h, _ptr(td), len(td), _ptr(so), _ptr(sp), len(so), int(n_total),
-                                      int(two_sz_total), int(workspace_bytes), C.byref(h)))
+        if options:
+            po = np.zeros(1, dtype=PLANOPT_DT)
+            po["workspace_bytes"] = int(workspace_bytes)
+            for k, v in options.items():
+                if k not in PLANOPT_DT.names or k == "reserved":
+                    raise TypeError(f"unknown plan option {k!r}")
+                po[k] = v
+            _check(lib().dmrg_plan_create_opts(ops._h, _ptr(td), len(td), _ptr(so), _ptr(sp), len(so), int(n_total),
+                                               int(two_sz_total), _ptr(po), C.byref(h)))
+        else:
+            _check(lib().dmrg_plan_create(ops._h, _ptr(td), len(td), _ptr(so), _ptr(sp), len(so), int(n_total),
+                                          int(two_sz_total), int(workspace_bytes), C.byref(h)))
         self._h = h
 
     @property
@@ -244,11 +265,11 @@ def fp64_peak_tflops(which, ms=200.0, stream=None):
     return v
 
 
-def load_problem(pr, workspace_bytes=0, values=None, structure_only=False):
+def load_problem(pr, workspace_bytes=0, values=None, structure_only=False, **options):
     """Convenience: OpsStore + Plan from a dmrg_workload Problem (array formats of dmrg_workload/store.py).
-    structure_only=True plans without a device (statistics / layout only)."""
+    structure_only=True plans without a device (statistics / layout only); options -> dmrg_plan_options."""
     ops = OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks,
                    None if structure_only else (pr.values if values is None else values),
                    pr.lin_ptr, pr.lin_op, pr.lin_coef)
-    plan = Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, workspace_bytes)
+    plan = Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, workspace_bytes, **options)
     return ops, plan

@@ -40,8 +40,7 @@ enum : uint32_t {
     SEG_A_MCONTIG = 1u << 0,   // A(m,k) at a_off + k*lda + m   (operator block used transposed)
     SEG_B_KCONTIG = 1u << 1,   // B(k,n) at b_off + n*ldb + k   (X = psi * O^T with O stored [n][k])
     SEG_A_IDENT   = 1u << 2,   // A is the identity: acc += alpha * B tile (no GEMM)
-    SEG_A_VEC2    = 1u << 3,   // A operand 16-byte loadable (even offset, even ld)
-    SEG_B_VEC2    = 1u << 4,
+    // (bits 3, 4 unused: every operand the planner emits is 16-byte aligned with an even leading dimension)
     SEG_ALPHA_ONE = 1u << 5,   // alpha == +1 (set by the planner before upload)
     SEG_ALPHA_NEG = 1u << 6,   // alpha == -1
     SEG_A_SPACE_SHIFT = 8,     // 2 bits
@@ -49,6 +48,9 @@ enum : uint32_t {
 };
 
 // One K-segment of a grouped GEMM job:  C += alpha * A(M x K) * B(K x N)
+// Operands are addressed twice: as (space, offset, ld) for the cp.async path and the identity-A prologue, and as
+// (tensor map, origin of the operand inside the mapped matrix) for the TMA path.  i0 / o0 are the origin along the
+// map's inner (contiguous) / outer dimension; the kernel adds the tile and K offsets.
 struct Seg {
     int64_t  a_off;
     int64_t  b_off;
@@ -56,8 +58,14 @@ struct Seg {
     int32_t  K;
     uint32_t flags;
     double   alpha;
+    int32_t  a_map, b_map;
+    int32_t  a_i0, a_o0, b_i0, b_o0;
 };
-static_assert(sizeof(Seg) == 40, "Seg layout");
+static_assert(sizeof(Seg) == 64, "Seg layout");
+
+// 128-byte CUtensorMap image (cuda.h is not included here; the planner encodes it through the driver entry point)
+struct alignas(64) TensorMap { uint64_t opaque[16]; };
+enum : int { COPY_LDGSTS = 1, COPY_TMA = 2 };
 
 enum : uint32_t { JOB_BETA1 = 1u << 0, JOB_C_SPACE_SHIFT = 8 };
 
@@ -82,7 +90,7 @@ static_assert(sizeof(Tile) == 16, "Tile layout");
 
 // tile-shape variants of the grouped GEMM kernel
 struct TileShape { int bm, bn; };
-constexpr int NUM_VARIANTS = 5;
+constexpr int NUM_VARIANTS = 1;
 extern const TileShape kVariants[NUM_VARIANTS];
 #ifndef DMRG_GEMM_BK
 #define DMRG_GEMM_BK 32
@@ -95,8 +103,8 @@ struct GemmLaunch {       // one launch of one kernel variant
     int64_t ntiles;
 };
 
-int launch_grouped_gemm(int variant, int cluster, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
-                        const double* ops, double* xws, const double* psi, double* sigma, cudaStream_t st);
+int launch_grouped_gemm(int variant, int copy_mode, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+                        const double* ops, double* xws, const double* psi, double* sigma, const TensorMap* tmaps, cudaStream_t st);
 int gemm_init();   // sets shared-memory attributes once
 
 }  // namespace dmrg

@@ -153,17 +153,23 @@ static int ws_ensure(dmrg_plan* P, int max_space) {
     if (P->dav) { davidson_ws_free(P->dav); P->dav = nullptr; }
     DavidsonWs* ws = new (std::nothrow) DavidsonWs();
     if (!ws) { set_error("dmrg_davidson: out of host memory"); return DMRG_ENOMEM; }
-    P->dav = ws;
     ws->n = n; ws->stride = round_up2(n); ws->max_space = max_space;
     const size_t vb = sizeof(double) * (size_t)ws->stride;
-    DMRG_CUDA(cudaMalloc(&ws->B, vb * max_space));
-    DMRG_CUDA(cudaMalloc(&ws->W, vb * max_space));
-    DMRG_CUDA(cudaMalloc(&ws->x, vb));
-    DMRG_CUDA(cudaMalloc(&ws->r, vb));
-    DMRG_CUDA(cudaMalloc(&ws->hd, vb));
-    DMRG_CUDA(cudaMalloc(&ws->partial, sizeof(double) * (size_t)(max_space + 2) * RED_GRID));
-    DMRG_CUDA(cudaMalloc(&ws->scal, sizeof(double) * (size_t)(max_space + 8)));
-    DMRG_CUDA(cudaMalloc(&ws->y, sizeof(double) * (size_t)(max_space + 8)));
+    // the workspace is attached to the plan only once every allocation has succeeded
+    auto alloc_all = [&]() -> int {
+        DMRG_CUDA(cudaMalloc(&ws->B, vb * max_space));
+        DMRG_CUDA(cudaMalloc(&ws->W, vb * max_space));
+        DMRG_CUDA(cudaMalloc(&ws->x, vb));
+        DMRG_CUDA(cudaMalloc(&ws->r, vb));
+        DMRG_CUDA(cudaMalloc(&ws->hd, vb));
+        DMRG_CUDA(cudaMalloc(&ws->partial, sizeof(double) * (size_t)(max_space + 2) * RED_GRID));
+        DMRG_CUDA(cudaMalloc(&ws->scal, sizeof(double) * (size_t)(max_space + 8)));
+        DMRG_CUDA(cudaMalloc(&ws->y, sizeof(double) * (size_t)(max_space + 8)));
+        return DMRG_OK;
+    };
+    const int rc = alloc_all();
+    if (rc != DMRG_OK) { davidson_ws_free(ws); return rc; }
+    P->dav = ws;
     return DMRG_OK;
 }
 
@@ -188,6 +194,12 @@ static int davidson_impl(dmrg_plan* P, double* x_io, int max_iter, int max_space
     if ((rc = dmrg_hdiag(P, ws->hd, st))) return rc;
     // b_0 = x0 / |x0|
     if ((rc = dots(ws, x_io, 1, x_io, s_misc, st))) return rc;
+    {
+        double n2 = 0.0;
+        DMRG_CUDA(cudaMemcpyAsync(&n2, s_misc, sizeof(double), cudaMemcpyDeviceToHost, st));
+        DMRG_CUDA(cudaStreamSynchronize(st));
+        if (!(n2 > 0.0) || !std::isfinite(n2)) { set_error("dmrg_davidson: the initial guess has norm^2 = %g", n2); return DMRG_EINVAL; }
+    }
     normalize_kernel<<<EW_GRID, 256, 0, st>>>(ws->B, x_io, s_misc, n);
     int m = 1, it = 0;
     double theta = 0.0, rn = 0.0;
@@ -228,6 +240,16 @@ static int davidson_impl(dmrg_plan* P, double* x_io, int max_iter, int max_space
             project_out_kernel<<<EW_GRID, 256, 0, st>>>(ws->r, ws->B, ld, m, s_dots, n);
         }
         if ((rc = dots(ws, ws->r, 1, ws->r, s_misc, st))) return rc;
+        {   // a correction vector that vanishes after orthogonalisation (exact eigenvector inside the space) cannot
+            // extend the basis: report it instead of dividing by zero (rn > tol here, so this is a breakdown)
+            double t2 = 0.0;
+            DMRG_CUDA(cudaMemcpyAsync(&t2, s_misc, sizeof(double), cudaMemcpyDeviceToHost, st));
+            DMRG_CUDA(cudaStreamSynchronize(st));
+            if (!(t2 > 1e-300) || !std::isfinite(t2)) {
+                set_error("dmrg_davidson: the new direction has norm^2 = %g after orthogonalisation (iteration %d)", t2, it);
+                break;
+            }
+        }
         normalize_kernel<<<EW_GRID, 256, 0, st>>>(ws->B + (int64_t)m * ld, ws->r, s_misc, n);
         DMRG_CUDA(cudaGetLastError());
         m++;
@@ -249,7 +271,9 @@ static int davidson_impl(dmrg_plan* P, double* x_io, int max_iter, int max_space
 
 extern "C" int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_space, double tol, double* energy,
                              double* resid_norm, int32_t* iters, double* thetas, void* cuda_stream) {
-    if (!plan || !x || max_iter < 1 || max_space < 1) { dmrg::set_error("dmrg_davidson: bad argument"); return DMRG_EINVAL; }
+    if (!plan || !x || max_iter < 1) { dmrg::set_error("dmrg_davidson: bad argument"); return DMRG_EINVAL; }
+    if (max_space < 2 && max_iter > 1) { dmrg::set_error("dmrg_davidson: max_space must be >= 2 (a space of one vector can never be extended)"); return DMRG_EINVAL; }
+    if (max_space < 1) { dmrg::set_error("dmrg_davidson: max_space must be >= 1"); return DMRG_EINVAL; }
     if (plan->ops->structure_only) { dmrg::set_error("dmrg_davidson: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     if ((uintptr_t)x & 15) { dmrg::set_error("dmrg_davidson: x must be 16-byte aligned"); return DMRG_EINVAL; }
     try {

@@ -6,26 +6,38 @@
 // bitwise reproducible and needs no atomics.  Both steps of the paper's GEMM pair map onto it:
 //   stage 1 (Eq. 11):      X = psi_panel * (O^R)^T           one segment, beta = 0
 //   stage 2 + reduction (Eqs. 12-13):   sigma_blk += sum_mu alpha_mu O^L_mu X_mu   many segments, beta = 1
-// (the paper runs Eq. 13 as a separate batched GEMV; here it is the K-loop itself).
+// (the paper runs Eq. 13 as a separate batched GEMV; here it is the K-loop itself), and so does
+// the renormalization pair of Eqs. 16-17 with the site tensor in psi's place.
 //
 // Arithmetic: DMMA.8x8x4 (PTX mma.sync.aligned.m8n8k4.f64).  tcgen05 has no FP64 kind, so the
 // warp-level DMMA is the FP64 tensor path of sm_100a; measured it issues at the full FP64 pipe rate
 // (148 SMs x 64 FMA/clk) while needing 4x fewer shared-memory operands than a DFMA register tile.
-// Operands are staged global -> shared with cp.async (16-byte when the planner proved alignment,
-// 8-byte otherwise) through an NST-deep ring; zero-fill (src-size 0) pads ragged M, N, K tails.
-// Either operand may be read transposed: the shared-memory tile keeps the global orientation and
-// only the fragment addressing changes, both orientations being bank-conflict free
-// (row strides = 4 mod 16 doubles).
+//
+// Staging global -> shared (plan option copy_mode):
+//   * TMA (default): every operand matrix has a 2-D tensor map (cuTensorMapEncodeTiled, FP64 elements) built by the
+//     planner; one elected producer lane issues ONE cp.async.bulk.tensor.2d (SASS UTMALDG) per operand and stage,
+//     completion counted in bytes on the stage's "full" mbarrier (expect_tx).  The box is 36 x BM (k-contiguous
+//     operand) or (BM+4) x 32 (m/n-contiguous): the inner box dimension carries the 4 padding columns that make
+//     the fragment loads bank-conflict free, so TMA itself writes the padded shared-memory layout.  Elements
+//     outside the operand matrix are zero-filled by the TMA unit (ragged M, N, K tails cost nothing); rows or
+//     columns that belong to a neighbouring sub-matrix (X slices, psi runs) only feed accumulator rows / columns
+//     that are never stored, and the K tail of such slices is masked in registers (compute_stage).
+//   * 16-byte cp.async (LDGSTS) with zero-fill (src-size 0) by all 32 producer lanes: the round-1 path, kept as a
+//     selectable alternative (it needs no tensor maps).
+// Every operand the planner emits is 16-byte aligned with an even leading dimension (operator blocks and the
+// packed R store by construction, psi through the plan's padded copy, X by its even column offsets).
+// Either operand may be read transposed: the shared-memory tile keeps the global orientation and only the
+// fragment addressing changes, both orientations being bank-conflict free (row strides = 4 mod 16 doubles).
 #include "common.h"
 
 namespace dmrg {
 
-const TileShape kVariants[NUM_VARIANTS] = {{64, 64}, {128, 128}, {128, 32}, {32, 128}, {32, 32}};
+const TileShape kVariants[NUM_VARIANTS] = {{64, 64}};
 
 namespace {
 
 constexpr int BK = GEMM_BK;
-constexpr int KPAD = BK + 4;   // row stride of a k-contiguous tile (20 = 4 mod 16)
+constexpr int KPAD = BK + 4;   // row stride of a k-contiguous tile (36 = 4 mod 16)
 
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, int src_bytes) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
@@ -34,14 +46,13 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
-
 __device__ __forceinline__ double lds64(uint32_t addr) {
     double v;
     asm volatile("ld.shared.f64 %0, [%1];\n" : "=d"(v) : "r"(addr));
     return v;
 }
 
-struct StageMeta { double alpha; uint32_t flags; int32_t ksteps; };
+struct StageMeta { double alpha; uint32_t flags; int32_t kvalid; };   // kvalid: k-columns of this stage inside the segment
 
 // ---- mbarrier helpers (shared::cta) ----------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -49,6 +60,10 @@ __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+// arrive and add `bytes` to the transaction count the phase waits for (bulk copies complete_tx against it)
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
 }
 // arrive on `bar` once all cp.async issued so far by this thread have landed (counts against the init count)
 __device__ __forceinline__ void mbar_arrive_cp_async(uint32_t bar) {
@@ -64,6 +79,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
         "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// one box of a 2-D tensor map -> shared (dst 128-byte aligned); completion = box bytes on `bar`
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n" ::"r"(dst),
+                 "l"(tmap), "r"(c0), "r"(c1), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
+    asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");
 }
 
 // fold alpha into the smaller fragment set; |alpha| = 1 flips the sign bit on the integer pipe
@@ -81,26 +104,18 @@ __device__ __forceinline__ void scale_frags(double (&af)[FM], double (&bf)[FN], 
     }
 }
 
-// predicated cp.async: no instruction is issued when `on` is false
-__device__ __forceinline__ void cp_async8_if(uint32_t dst, const void* src, int src_bytes, bool on) {
-    asm volatile("{\n.reg .pred p;\nsetp.ne.b32 p, %3, 0;\n@p cp.async.ca.shared.global [%0], [%1], 8, %2;\n}\n" ::"r"(dst), "l"(src),
-                 "r"(src_bytes), "r"((int)on) : "memory");
-}
-
-// Stage one operand tile (MN x BK) of a segment into shared memory with NT producer threads.
-//   kcontig: global (mn,k) at g + mn*ld + k, shared at mn*KPAD + k
-//   else   : global (mn,k) at g + k*ld + mn, shared at k*(BMN+4) + mn
+// ---- producer, cp.async path ----------------------------------------------------------------------------
+// Stage one operand tile (MN x BK) of a segment into shared memory with the 32 producer lanes, 16 bytes per copy.
 // Elements outside [0, mn_lim) x [0, k_lim) are zero-filled (src-size 0); rows >= round_up(mn_lim, 8) and
-// k >= round_up(k_lim, 4) are never read by a fragment and are not copied at all.  Each thread keeps one fixed
-// position along the contiguous direction and walks the other with a constant pointer stride, so a copy costs
-// a 64-bit add, two compares and the LDGSTS -- the producer warp must not be the bottleneck.
-template <int BMN, int NT>
-__device__ __forceinline__ void load_operand(uint32_t sdst, const double* __restrict__ g, int ld, bool kcontig, bool vec2,
-                                             int mn_lim, int k_lim, int tid) {
+// k >= round_up(k_lim, 4) are never read by a fragment and are not copied at all.  Each lane keeps one fixed
+// position along the contiguous direction and walks the other with a constant pointer stride.
+template <int BMN>
+__device__ __forceinline__ void ldgsts_operand(uint32_t sdst, const double* __restrict__ g, int ld, bool kcontig, int mn_lim, int k_lim,
+                                               int tid) {
+    constexpr int NT = 32;
     const int mn_end = (mn_lim + 7) & ~7, k_end = (k_lim + 3) & ~3;
-    if (vec2 && mn_lim >= BMN && k_lim >= BK) {
-        // interior stage (full tile, full K slab): no predicates, no zero-fill -- a copy is the LDGSTS and a 64-bit
-        // add.  The producer warp is on the critical path; this is the common case.
+    if (mn_lim >= BMN && k_lim >= BK) {
+        // interior stage (full tile, full K slab): no predicates, no zero-fill
         if (kcontig) {
             constexpr int RPI = NT / (BK / 2), ITERS = BMN / RPI;
             const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
@@ -134,106 +149,66 @@ __device__ __forceinline__ void load_operand(uint32_t sdst, const double* __rest
         return;
     }
     if (kcontig) {
-        if (vec2) {
-            // ragged stage: this lane's rows r0, r0+RPI, ...: full copies (kb bytes of the row's K slab) while the row
-            // is inside the matrix, then zero-fill up to the next multiple of 8 rows; loops are bounded by the row
-            // counts, so a ragged tile costs the producer in proportion to its rows
-            constexpr int RPI = NT / (BK / 2);
-            const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
-            const int kb = k + 1 < k_lim ? 16 : (k < k_lim ? 8 : 0);
-            if (k < k_end) {
-                const int n_in = mn_lim > r0 ? (mn_lim - r0 + RPI - 1) / RPI : 0;
-                const int n_all = mn_end > r0 ? (mn_end - r0 + RPI - 1) / RPI : 0;
-                const double* src = g + (int64_t)r0 * ld + k;
-                const int64_t step = (int64_t)RPI * ld;
-                uint32_t dst = sdst + (r0 * KPAD + k) * 8;
-#pragma unroll 4
-                for (int i = 0; i < n_in; i++) {
-                    cp_async16(dst, src, kb);
-                    src += step;
-                    dst += RPI * KPAD * 8;
-                }
-                for (int i = n_in; i < n_all; i++) {
-                    cp_async16(dst, g, 0);
-                    dst += RPI * KPAD * 8;
-                }
-            }
-        } else {
-            constexpr int RPI = NT / BK, ITERS = BMN / RPI;
-            const int r0 = tid / BK, k = tid % BK;
-            const int kb = k < k_lim ? 8 : 0;
-            const bool lane_on = k < k_end;
+        // ragged stage: this lane's rows r0, r0+RPI, ...: full copies (kb bytes of the row's K slab) while the row
+        // is inside the matrix, then zero-fill up to the next multiple of 8 rows; loops are bounded by the row
+        // counts, so a ragged tile costs the producer in proportion to its rows
+        constexpr int RPI = NT / (BK / 2);
+        const int r0 = tid / (BK / 2), k = (tid % (BK / 2)) * 2;
+        const int kb = k + 1 < k_lim ? 16 : (k < k_lim ? 8 : 0);
+        if (k < k_end) {
+            const int n_in = mn_lim > r0 ? (mn_lim - r0 + RPI - 1) / RPI : 0;
+            const int n_all = mn_end > r0 ? (mn_end - r0 + RPI - 1) / RPI : 0;
             const double* src = g + (int64_t)r0 * ld + k;
             const int64_t step = (int64_t)RPI * ld;
-            const uint32_t dst = sdst + (r0 * KPAD + k) * 8;
-#pragma unroll
-            for (int i = 0; i < ITERS; i++) {
-                const int row = r0 + RPI * i;
-                const bool in = row < mn_lim;
-                cp_async8_if(dst + i * RPI * KPAD * 8, in ? src : g, in ? kb : 0, lane_on && row < mn_end);
+            uint32_t dst = sdst + (r0 * KPAD + k) * 8;
+#pragma unroll 4
+            for (int i = 0; i < n_in; i++) {
+                cp_async16(dst, src, kb);
                 src += step;
+                dst += RPI * KPAD * 8;
+            }
+            for (int i = n_in; i < n_all; i++) {
+                cp_async16(dst, g, 0);
+                dst += RPI * KPAD * 8;
             }
         }
     } else {
         constexpr int MPAD = BMN + 4;
-        if (vec2) {
-            constexpr int PR = BMN / 2;                              // 16-byte pairs per k-row
-            constexpr int SEGS = PR > NT ? PR / NT : 1;              // passes needed to cover one k-row
-            constexpr int KPI = PR > NT ? 1 : NT / PR;               // k-rows per pass
-            const int k0 = tid / PR, mn0 = (tid % PR) * 2;
-            const int n_in = k_lim > k0 ? min(BK / KPI, (k_lim - k0 + KPI - 1) / KPI) : 0;      // k-rows inside the segment
-            const int n_all = k_end > k0 ? min(BK / KPI, (k_end - k0 + KPI - 1) / KPI) : 0;     // ... up to the next multiple of 4
+        constexpr int PR = BMN / 2;                              // 16-byte pairs per k-row
+        constexpr int SEGS = PR > NT ? PR / NT : 1;              // passes needed to cover one k-row
+        constexpr int KPI = PR > NT ? 1 : NT / PR;               // k-rows per pass
+        const int k0 = tid / PR, mn0 = (tid % PR) * 2;
+        const int n_in = k_lim > k0 ? min(BK / KPI, (k_lim - k0 + KPI - 1) / KPI) : 0;      // k-rows inside the segment
+        const int n_all = k_end > k0 ? min(BK / KPI, (k_end - k0 + KPI - 1) / KPI) : 0;     // ... up to the next multiple of 4
 #pragma unroll
-            for (int sg = 0; sg < SEGS; sg++) {
-                const int mn = mn0 + sg * NT * 2;
-                if (mn >= mn_end) continue;
-                const int mb = mn + 1 < mn_lim ? 16 : (mn < mn_lim ? 8 : 0);
-                const double* src = g + (int64_t)k0 * ld + mn;
-                const int64_t step = (int64_t)KPI * ld;
-                uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
+        for (int sg = 0; sg < SEGS; sg++) {
+            const int mn = mn0 + sg * NT * 2;
+            if (mn >= mn_end) continue;
+            const int mb = mn + 1 < mn_lim ? 16 : (mn < mn_lim ? 8 : 0);
+            const double* src = g + (int64_t)k0 * ld + mn;
+            const int64_t step = (int64_t)KPI * ld;
+            uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
 #pragma unroll 4
-                for (int i = 0; i < n_in; i++) {
-                    cp_async16(dst, mb ? src : g, mb);
-                    src += step;
-                    dst += KPI * MPAD * 8;
-                }
-                for (int i = n_in; i < n_all; i++) {
-                    cp_async16(dst, g, 0);
-                    dst += KPI * MPAD * 8;
-                }
+            for (int i = 0; i < n_in; i++) {
+                cp_async16(dst, mb ? src : g, mb);
+                src += step;
+                dst += KPI * MPAD * 8;
             }
-        } else {
-            constexpr int PR = BMN;
-            constexpr int SEGS = PR > NT ? PR / NT : 1;
-            constexpr int KPI = PR > NT ? 1 : NT / PR;
-            const int k0 = tid / PR, mn0 = tid % PR;
-#pragma unroll
-            for (int sg = 0; sg < SEGS; sg++) {
-                const int mn = mn0 + sg * NT;
-                const int mb = mn < mn_lim ? 8 : 0;
-                const bool lane_on = mn < mn_end;
-                const double* src = g + (int64_t)k0 * ld + mn;
-                const int64_t step = (int64_t)KPI * ld;
-                const uint32_t dst = sdst + (k0 * MPAD + mn) * 8;
-#pragma unroll
-                for (int i = 0; i < BK / KPI; i++) {
-                    const int k = k0 + KPI * i;
-                    const bool in = k < k_lim;
-                    cp_async8_if(dst + i * KPI * MPAD * 8, in ? src : g, in ? mb : 0, lane_on && k < k_end);
-                    src += step;
-                }
+            for (int i = n_in; i < n_all; i++) {
+                cp_async16(dst, g, 0);
+                dst += KPI * MPAD * 8;
             }
         }
     }
 }
 
-// One pipeline stage of one consumer warp: up to BK/4 k-steps of FMe x FNe DMMA fragments (the top-left part of
-// the warp's FM x FN accumulator grid).  With DBUF the fragments of k-step kk+1 are fetched while the DMMAs of
-// k-step kk issue (two k-steps per loop trip, so the buffer index is static).
-template <int FM, int FN, int FMe, int FNe, bool DBUF>
-__device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const double* __restrict__ pa, const double* __restrict__ pb,
-                                              int a_sm, int a_sk, int b_sn, int b_sk, int ksteps, int mode, double alpha) {
-    static_assert(FM <= 4 && FN <= 4, "ragged-tile dispatch covers up to 4 x 4 fragments per warp");
+// One pipeline stage of one consumer warp: the k-steps of FMe x FNe DMMA fragments covering `kvalid` k-columns.
+// The fragments of the last k-step are masked in registers beyond kvalid (lane lc holds k = 4 kk + lc), so the
+// shared-memory tile needs no zero K padding.
+template <int FMe, int FNe>
+__device__ __forceinline__ void compute_stage(double (&acc)[FMe][FNe][2], uint32_t a_addr, uint32_t b_addr, uint32_t a_rs, uint32_t b_rs,
+                                              uint32_t a_ks, uint32_t b_ks, int kvalid, int lc, int mode, double alpha) {
+    static_assert(FMe <= 4 && FNe <= 4, "ragged-tile dispatch covers up to 4 x 4 fragments per warp");
     auto mma = [&](double (&af)[FMe], double (&bf)[FNe]) {
         if (mode != 0) scale_frags<FMe, FNe>(af, bf, mode, alpha);
 #pragma unroll
@@ -241,58 +216,42 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FM][FN][2], const do
 #pragma unroll
             for (int j = 0; j < FNe; j++) dmma884(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
     };
-    if (DBUF) {
-        uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(pa), b_addr = (uint32_t)__cvta_generic_to_shared(pb);
-        const uint32_t a_rs = 64u * a_sm, b_rs = 64u * b_sn, a_ks = 32u * a_sk, b_ks = 32u * b_sk;
-        auto loadu = [&](double (&af)[FMe], double (&bf)[FNe]) {
-#pragma unroll
-            for (int i = 0; i < FMe; i++) af[i] = lds64(a_addr + i * a_rs);
-#pragma unroll
-            for (int j = 0; j < FNe; j++) bf[j] = lds64(b_addr + j * b_rs);
-            a_addr += a_ks;
-            b_addr += b_ks;
-        };
-        double a0[FMe], b0[FNe], a1[FMe], b1[FNe];
-        loadu(a0, b0);
+    // 32-bit shared addresses advanced by a constant per k-step: the k-loop holds no address arithmetic beyond
+    // the fragment offsets (indexing by kk made ptxas rematerialise lane ids and reload spilled bases per k-step)
+    const int ksteps = (kvalid + 3) >> 2;
+    const int tail = kvalid - 4 * (ksteps - 1);            // valid k-columns of the last k-step: 1..4
+    const uint32_t a_end = a_addr + (uint32_t)(tail == 4 ? ksteps : ksteps - 1) * a_ks;
 #pragma unroll 1
-        for (int kk = 0; kk < ksteps; kk += 2) {
-            const bool two = kk + 1 < ksteps;
-            if (two) loadu(a1, b1);
-            mma(a0, b0);
-            if (two) {
-                if (kk + 2 < ksteps) loadu(a0, b0);
-                mma(a1, b1);
-            }
-        }
-    } else {
-        // 32-bit shared addresses advanced by a constant per k-step: the k-loop holds no address arithmetic beyond
-        // the fragment offsets (indexing by kk made ptxas rematerialise lane ids and reload spilled bases per k-step)
-        uint32_t a_addr = (uint32_t)__cvta_generic_to_shared(pa), b_addr = (uint32_t)__cvta_generic_to_shared(pb);
-        const uint32_t a_rs = 64u * a_sm, b_rs = 64u * b_sn, a_ks = 32u * a_sk, b_ks = 32u * b_sk;
-        const uint32_t a_end = a_addr + ksteps * a_ks;
-#pragma unroll 1
-        for (; a_addr != a_end; a_addr += a_ks, b_addr += b_ks) {
-            double a0[FMe], b0[FNe];
+    for (; a_addr != a_end; a_addr += a_ks, b_addr += b_ks) {
+        double a0[FMe], b0[FNe];
 #pragma unroll
-            for (int i = 0; i < FMe; i++) a0[i] = lds64(a_addr + i * a_rs);
+        for (int i = 0; i < FMe; i++) a0[i] = lds64(a_addr + i * a_rs);
 #pragma unroll
-            for (int j = 0; j < FNe; j++) b0[j] = lds64(b_addr + j * b_rs);
-            mma(a0, b0);
-        }
+        for (int j = 0; j < FNe; j++) b0[j] = lds64(b_addr + j * b_rs);
+        mma(a0, b0);
+    }
+    if (tail != 4) {
+        double a0[FMe], b0[FNe];
+        const bool keep = lc < tail;
+#pragma unroll
+        for (int i = 0; i < FMe; i++) { const double v = lds64(a_addr + i * a_rs); a0[i] = keep ? v : 0.0; }
+#pragma unroll
+        for (int j = 0; j < FNe; j++) { const double v = lds64(b_addr + j * b_rs); b0[j] = keep ? v : 0.0; }
+        mma(a0, b0);
     }
 }
 
 struct ConsumerCtx {
     const Job* job; const Seg* segs; const double* ops; double* xws; const double* psi; double* sigma;
-    const double* smem; const StageMeta* meta; uint32_t full_u32, empty_u32;
+    uint32_t smem_u32; const StageMeta* meta; uint32_t full_u32, empty_u32;
     int m0, n0, m_lim, n_lim, nstages, lane, wm0, wn0, fm_eff, fn_eff;
 };
 
 // Everything one consumer warp does for one tile, with FMe x FNe accumulator fragments (<= the 4 x 4 of a 32x32
 // warp tile): identity-A segments, the mbarrier-paced main loop, the epilogue.  Fragments (i, j) with
 // i >= fm_eff or j >= fn_eff (a warp ragged in both directions keeps all its columns) are computed on
-// zero-filled or neighbouring data and never stored.
-template <int BM, int BN, int NST, int FMe, int FNe, bool DBUF>
+// stale or neighbouring data and never stored.
+template <int BM, int BN, int NST, int FMe, int FNe>
 __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
     constexpr int A_ELEMS = (BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4);
     constexpr int B_ELEMS = (BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4);
@@ -334,18 +293,18 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
         const int slot = it % NST;
         mbar_wait(cx.full_u32 + 8 * slot, (it / NST) & 1);
         if (any_frag) {
-            const double* sa = cx.smem + slot * STAGE_ELEMS;
-            const double* sb = sa + A_ELEMS;
+            const uint32_t sa = cx.smem_u32 + (uint32_t)slot * (STAGE_ELEMS * 8);
+            const uint32_t sb = sa + A_ELEMS * 8;
             const StageMeta mt = cx.meta[slot];
             const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
             const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
             // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
             const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
             const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
-            const double* pa = sa + (wm0 + lr) * a_sm + lc * a_sk;
-            const double* pb = sb + (wn0 + lr) * b_sn + lc * b_sk;
+            const uint32_t pa = sa + 8u * (uint32_t)((wm0 + lr) * a_sm + lc * a_sk);
+            const uint32_t pb = sb + 8u * (uint32_t)((wn0 + lr) * b_sn + lc * b_sk);
             const int mode = (mt.flags & SEG_ALPHA_ONE) ? 0 : ((mt.flags & SEG_ALPHA_NEG) ? 1 : 2);   // integer test: no FP64-pipe DSETP
-            compute_stage<FMe, FNe, FMe, FNe, DBUF>(acc, pa, pb, a_sm, a_sk, b_sn, b_sk, mt.ksteps, mode, mt.alpha);
+            compute_stage<FMe, FNe>(acc, pa, pb, 64u * a_sm, 64u * b_sn, 32u * a_sk, 32u * b_sk, mt.kvalid, lc, mode, mt.alpha);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(cx.empty_u32 + 8 * slot);
@@ -376,15 +335,16 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
 }
 
 // Warp-specialised kernel.  Warps 0 .. WM*WN-1 are CONSUMERS (LDS + DMMA only, one TM x TN warp tile
-// each); the last warp is the PRODUCER, which walks the job's segment list and issues every cp.async.
-// The two sides meet only through per-stage mbarriers (full: 32 cp.async-completion arrivals + 1
-// release arrival that publishes the stage metadata; empty: one arrival per consumer warp), so there
-// is no CTA-wide barrier in the main loop and the consumer warps drift freely against each other.
-template <int BM, int BN, int WM, int WN, int NST, int NPW, int MAXREG, bool DBUF>
-__global__ void __launch_bounds__(32 * (WM * WN + NPW)) __maxnreg__(MAXREG)
+// each); the last warp is the PRODUCER, which walks the job's segment list and stages every operand tile.
+// The two sides meet only through per-stage mbarriers (full: one expect_tx arrival of the elected lane + the
+// byte counts of the two TMA copies -- or, on the cp.async path, 32 cp.async-completion arrivals + 1 release
+// arrival; either way the arrival publishes the stage metadata; empty: one arrival per consumer warp), so
+// there is no CTA-wide barrier in the main loop and the consumer warps drift freely against each other.
+template <int BM, int BN, int WM, int WN, int NST, int MAXREG>
+__global__ void __launch_bounds__(32 * (WM * WN + 1)) __maxnreg__(MAXREG)
 grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, const Tile* __restrict__ tiles,
                     const double* __restrict__ ops, double* __restrict__ xws, const double* __restrict__ psi,
-                    double* __restrict__ sigma) {
+                    double* __restrict__ sigma, const TensorMap* __restrict__ tmaps, int copy_mode) {
     constexpr int NCW = WM * WN;   // consumer warps
     constexpr int TM = BM / WM, TN = BN / WN;
     constexpr int FM = TM / 8, FN = TN / 8;
@@ -393,14 +353,13 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     constexpr int STAGE_ELEMS = A_ELEMS + B_ELEMS;
     static_assert(FM >= 1 && FN >= 1, "warp tile must be a multiple of 8x8");
 
-    extern __shared__ __align__(16) double smem[];
+    extern __shared__ __align__(128) double smem[];   // TMA destinations: every stage buffer is a multiple of 128 bytes
     __shared__ StageMeta meta[NST];
     __shared__ __align__(8) uint64_t bar_full[NST], bar_empty[NST];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     const Tile tile = tiles[blockIdx.x];
-    if (tile.job < 0) return;   // padding of a thread-block cluster (whole CTA leaves before any barrier)
     const Job job = jobs[tile.job];
     const int m0 = tile.m0, n0 = tile.n0;
     const int m_lim = tile.rows, n_lim = tile.cols;   // <= BM, BN and inside the matrix (planner)
@@ -409,30 +368,63 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
 
     const uint32_t full_u32 = (uint32_t)__cvta_generic_to_shared(bar_full);
     const uint32_t empty_u32 = (uint32_t)__cvta_generic_to_shared(bar_empty);
+    const uint32_t smem_u32 = (uint32_t)__cvta_generic_to_shared(smem);
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < NST; s++) {
-            mbar_init(full_u32 + 8 * s, 32 * NPW + 1);
+            mbar_init(full_u32 + 8 * s, copy_mode == COPY_TMA ? 1 : 32 + 1);
             mbar_init(empty_u32 + 8 * s, NCW);
         }
     }
     __syncthreads();   // the only CTA-wide barrier
 
     if (warp >= NCW) {
-        // =============================== producer warp(s) ============================================
-        // NPW == 1: one warp stages A and B; NPW == 2 / 4: the first half of the producer warps stages A, the second half B
-        const int pw = warp - NCW;
+        // =============================== producer warp ==============================================
         int lseg = job.seg_begin;
         while (lseg < job.seg_end && (segs[lseg].flags & SEG_A_IDENT)) lseg++;   // identity segments need no staging
         if (lseg >= job.seg_end) return;
         Seg ls = segs[lseg];
         int lk0 = 0;
-        const uint32_t smem_u32 = (uint32_t)__cvta_generic_to_shared(smem);
+        if (copy_mode == COPY_TMA) {
+            // ---- TMA: one elected lane, two tensor copies per stage ------------------------------------
+            if (lane != 0) return;
+            constexpr uint32_t A_KC_BYTES = KPAD * BM * 8, A_MC_BYTES = (BM + 4) * BK * 8;
+            constexpr uint32_t B_KC_BYTES = KPAD * BN * 8, B_MC_BYTES = (BN + 4) * BK * 8;
+            for (int it = 0; it < nstages; it++) {
+                const int slot = it % NST;
+                if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
+                const uint32_t sa = smem_u32 + (uint32_t)slot * (STAGE_ELEMS * 8);
+                const uint32_t sb = sa + A_ELEMS * 8;
+                const uint32_t bar = full_u32 + 8 * slot;
+                const bool a_kc = !(ls.flags & SEG_A_MCONTIG);
+                const bool b_kc = (ls.flags & SEG_B_KCONTIG) != 0;
+                meta[slot].alpha = ls.alpha;
+                meta[slot].flags = ls.flags;
+                meta[slot].kvalid = min(ls.K - lk0, BK);
+                mbar_arrive_expect_tx(bar, (a_kc ? A_KC_BYTES : A_MC_BYTES) + (b_kc ? B_KC_BYTES : B_MC_BYTES));   // release: publishes meta[slot]
+                tma_load_2d(sa, tmaps + ls.a_map, a_kc ? ls.a_i0 + lk0 : ls.a_i0 + m0, a_kc ? ls.a_o0 + m0 : ls.a_o0 + lk0, bar);
+                tma_load_2d(sb, tmaps + ls.b_map, b_kc ? ls.b_i0 + lk0 : ls.b_i0 + n0, b_kc ? ls.b_o0 + n0 : ls.b_o0 + lk0, bar);
+                lk0 += BK;
+                if (lk0 >= ls.K) {
+                    lk0 = 0;
+                    lseg++;
+                    if (lseg < job.seg_end) {
+                        ls = segs[lseg];
+                        if (lseg + 1 < job.seg_end) {   // descriptor of the segment after this one: hide its fetch latency
+                            tma_prefetch_desc(tmaps + segs[lseg + 1].a_map);
+                            tma_prefetch_desc(tmaps + segs[lseg + 1].b_map);
+                        }
+                    }
+                }
+            }
+            return;
+        }
         for (int it = 0; it < nstages; it++) {
             const int slot = it % NST;
             if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
-            const uint32_t sa = smem_u32 + slot * STAGE_ELEMS * 8;
+            const uint32_t sa = smem_u32 + (uint32_t)slot * (STAGE_ELEMS * 8);
             const uint32_t sb = sa + A_ELEMS * 8;
+            const uint32_t bar = full_u32 + 8 * slot;
             const int k_lim = ls.K - lk0;
             const bool a_kc = !(ls.flags & SEG_A_MCONTIG);
             const bool b_kc = (ls.flags & SEG_B_KCONTIG) != 0;
@@ -440,16 +432,14 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
                                (a_kc ? (int64_t)m0 * ls.lda + lk0 : (int64_t)lk0 * ls.lda + m0);
             const double* gb = space_r((ls.flags >> SEG_B_SPACE_SHIFT) & 3u) + ls.b_off +
                                (b_kc ? (int64_t)n0 * ls.ldb + lk0 : (int64_t)lk0 * ls.ldb + n0);
-            constexpr int HP = NPW > 1 ? NPW / 2 : 1;   // producer warps per operand
-            const int ptid = (pw % HP) * 32 + lane;
-            if (NPW == 1 || pw < HP) load_operand<BM, 32 * HP>(sa, ga, ls.lda, a_kc, (ls.flags & SEG_A_VEC2) != 0, m_lim, k_lim, ptid);
-            if (NPW == 1 || pw >= HP) load_operand<BN, 32 * HP>(sb, gb, ls.ldb, b_kc, (ls.flags & SEG_B_VEC2) != 0, n_lim, k_lim, ptid);
-            mbar_arrive_cp_async(full_u32 + 8 * slot);
-            if (pw == 0 && lane == 0) {
+            ldgsts_operand<BM>(sa, ga, ls.lda, a_kc, m_lim, k_lim, lane);
+            ldgsts_operand<BN>(sb, gb, ls.ldb, b_kc, n_lim, k_lim, lane);
+            mbar_arrive_cp_async(bar);
+            if (lane == 0) {
                 meta[slot].alpha = ls.alpha;
                 meta[slot].flags = ls.flags;
-                meta[slot].ksteps = (min(k_lim, BK) + 3) >> 2;
-                mbar_arrive(full_u32 + 8 * slot);   // release: publishes meta[slot]
+                meta[slot].kvalid = min(k_lim, BK);
+                mbar_arrive(bar);   // release: publishes meta[slot]
             }
             lk0 += BK;
             if (lk0 >= ls.K) {
@@ -467,7 +457,7 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     // the pace of its most loaded warp.
     ConsumerCtx cx;
     cx.job = &job; cx.segs = segs; cx.ops = ops; cx.xws = xws; cx.psi = psi; cx.sigma = sigma;
-    cx.smem = smem; cx.meta = meta; cx.full_u32 = full_u32; cx.empty_u32 = empty_u32;
+    cx.smem_u32 = smem_u32; cx.meta = meta; cx.full_u32 = full_u32; cx.empty_u32 = empty_u32;
     cx.m0 = m0; cx.n0 = n0; cx.m_lim = m_lim; cx.n_lim = n_lim; cx.nstages = nstages; cx.lane = lane;
     const int fr_m = (m_lim + 7) >> 3, fr_n = (n_lim + 7) >> 3;
     const int per_m = (fr_m + WM - 1) / WM, per_n = (fr_n + WN - 1) / WN;
@@ -479,16 +469,16 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     // both counts at once made ptxas spill; a warp ragged in both directions pads its columns to the warp tile.)
     if (cx.fm_eff == FM || cx.fm_eff == 0) {
         switch (cx.fn_eff) {
-            case 1: consumer_body<BM, BN, NST, FM, 1, DBUF>(cx); break;
-            case 2: if constexpr (FN >= 2) consumer_body<BM, BN, NST, FM, 2, DBUF>(cx); break;
-            case 3: if constexpr (FN >= 3) consumer_body<BM, BN, NST, FM, 3, DBUF>(cx); break;
-            default: consumer_body<BM, BN, NST, FM, FN, DBUF>(cx); break;   // full warp tile, or a warp with no fragment
+            case 1: consumer_body<BM, BN, NST, FM, 1>(cx); break;
+            case 2: if constexpr (FN >= 2) consumer_body<BM, BN, NST, FM, 2>(cx); break;
+            case 3: if constexpr (FN >= 3) consumer_body<BM, BN, NST, FM, 3>(cx); break;
+            default: consumer_body<BM, BN, NST, FM, FN>(cx); break;   // full warp tile, or a warp with no fragment
         }
     } else {
         switch (cx.fm_eff) {
-            case 1: consumer_body<BM, BN, NST, 1, FN, DBUF>(cx); break;
-            case 2: if constexpr (FM >= 2) consumer_body<BM, BN, NST, 2, FN, DBUF>(cx); break;
-            default: if constexpr (FM >= 3) consumer_body<BM, BN, NST, 3, FN, DBUF>(cx); break;
+            case 1: consumer_body<BM, BN, NST, 1, FN>(cx); break;
+            case 2: if constexpr (FM >= 2) consumer_body<BM, BN, NST, 2, FN>(cx); break;
+            default: if constexpr (FM >= 3) consumer_body<BM, BN, NST, 3, FN>(cx); break;
         }
     }
 }
@@ -499,33 +489,14 @@ constexpr size_t smem_bytes(int nst) {
            (((BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4)) + ((BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4)));
 }
 
-// variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, producer warps, register cap, double-buffered fragments>
-// Every variant uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step).  V0 was tuned on the B200 (macros kept
-// for re-tuning).  Default: BK = 32, 2 stages (72 KB), 128 registers, no spills -> 3 CTAs/SM: half the mbarrier
-// round trips per flop of BK = 16.  Measured against BK = 16 / 2 stages / 96 registers / 4 CTAs/SM: cfg 5 +1.7 %,
-// cfg 3 +1.0 %, cfg 4 -1.6 %, cfg 2 -2.2 %.  BK = 16 with 3 stages x 128 registers (3 CTAs/SM) lost 4-11 %, 4 stages
-// (2 CTAs/SM) and a second producer warp ~10 %, double-buffered fragments at BK = 32 1-5 %.
-#ifndef V0_NST
-#define V0_NST 2
-#endif
-#ifndef V0_REG
-#define V0_REG 128
-#endif
-#ifndef V0_DBUF
-#define V0_DBUF false
-#endif
-#ifndef V0_NPW
-#define V0_NPW 1
-#endif
-constexpr int V1_NST = BK >= 32 ? 2 : 4;   // 128x128 stages must fit 227 KB
-#define V0 grouped_gemm_kernel<64, 64, 2, 2, V0_NST, V0_NPW, V0_REG, V0_DBUF>
-#define V1 grouped_gemm_kernel<128, 128, 4, 4, V1_NST, 4, 96, false>    // large blocks, least operand traffic, 1 CTA/SM
-#define V2 grouped_gemm_kernel<128, 32, 4, 1, 3, 1, 128, true>     // skinny N (stage 1 with a small R' sector)
-#define V3 grouped_gemm_kernel<32, 128, 1, 4, 3, 1, 128, true>     // skinny M
-#define V4 grouped_gemm_kernel<32, 32, 1, 1, 4, 1, 128, true>      // tiny blocks: one consumer warp
-constexpr int V0_T = 32 * (4 + V0_NPW), V1_T = 640, V2_T = 160, V3_T = 160, V4_T = 64;
-constexpr size_t V0_S = smem_bytes<64, 64>(V0_NST), V1_S = smem_bytes<128, 128>(V1_NST), V2_S = smem_bytes<128, 32>(3), V3_S = smem_bytes<32, 128>(3),
-                 V4_S = smem_bytes<32, 32>(4);
+// variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, register cap>
+// Every variant uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step).
+//   V0 64x64, 2x2 consumer warps, BK = 32, 2 stages (72 KB), 128 registers, no spills -> 3 CTAs/SM.  Measured
+//      against BK = 16 / 2 stages / 96 registers / 4 CTAs/SM: cfg 5 +1.7 %, cfg 3 +1.0 %, cfg 4 -1.6 %, cfg 2 -2.2 %;
+//      3 stages x BK = 16, 4 stages, a second producer warp, double-buffered fragments: all slower.
+#define V0 grouped_gemm_kernel<64, 64, 2, 2, 2, 128>
+constexpr int V0_T = 32 * 5;
+constexpr size_t V0_S = smem_bytes<64, 64>(2);
 
 }  // namespace
 
@@ -533,50 +504,20 @@ int gemm_init() {
     static bool done = false;
     if (done) return DMRG_OK;
     DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
-    DMRG_CUDA(cudaFuncSetAttribute(V1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V1_S));
-    DMRG_CUDA(cudaFuncSetAttribute(V2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V2_S));
-    DMRG_CUDA(cudaFuncSetAttribute(V3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V3_S));
-    DMRG_CUDA(cudaFuncSetAttribute(V4, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V4_S));
     done = true;
     return DMRG_OK;
 }
 
-template <typename K>
-static cudaError_t launch_one(K kernel, unsigned grid, int threads, size_t smem, int cluster, cudaStream_t st, const Job* jobs, const Seg* segs,
-                              const Tile* tiles, const double* ops, double* xws, const double* psi, double* sigma) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid);
-    cfg.blockDim = dim3(threads);
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    if (cluster > 1) {
-        // sibling tiles of one output block (they share A row panels / B column panels) are launched as one
-        // thread-block cluster: co-scheduled, they walk the same K-loop in step and meet in L2
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = cluster;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-    }
-    return cudaLaunchKernelEx(&cfg, kernel, jobs, segs, tiles, ops, xws, psi, sigma);
-}
-
-int launch_grouped_gemm(int variant, int cluster, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
-                        const double* ops, double* xws, const double* psi, double* sigma, cudaStream_t st) {
+int launch_grouped_gemm(int variant, int copy_mode, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+                        const double* ops, double* xws, const double* psi, double* sigma, const TensorMap* tmaps, cudaStream_t st) {
     if (ntiles <= 0) return DMRG_OK;
     const unsigned g = (unsigned)ntiles;
-    cudaError_t e;
     switch (variant) {
-        case 0: e = launch_one(V0, g, V0_T, V0_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 1: e = launch_one(V1, g, V1_T, V1_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 2: e = launch_one(V2, g, V2_T, V2_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 3: e = launch_one(V3, g, V3_T, V3_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
-        case 4: e = launch_one(V4, g, V4_T, V4_S, cluster, st, jobs, segs, tiles, ops, xws, psi, sigma); break;
+        case 0: V0<<<g, V0_T, V0_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
-    if (e != cudaSuccess) { set_error("launch_grouped_gemm: variant %d, %lld tiles, cluster %d: %s", variant, (long long)ntiles, cluster, cudaGetErrorString(e)); return DMRG_ECUDA; }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { set_error("launch_grouped_gemm: variant %d, %lld tiles: %s", variant, (long long)ntiles, cudaGetErrorString(e)); return DMRG_ECUDA; }
     return DMRG_OK;
 }
 

@@ -19,6 +19,8 @@
 #include <new>
 #include <unordered_map>
 
+#include <cuda.h>   // CUtensorMap types only; the encoder is reached through cudaGetDriverEntryPoint (no libcuda link)
+
 #include "plan.h"
 
 namespace dmrg {
@@ -34,32 +36,16 @@ struct Task {
     double alpha;
 };
 
-struct XLoc { int64_t off; int32_t ld; };
+struct XLoc { int64_t off; int32_t ld; int64_t job_off; int32_t job_rows, r0, c0; };   // X of one task: a slice of a stage-1 job's output matrix
 
 static inline int64_t xkey(int64_t r_off, int r_trans, int in_blk, int64_t nblk) {
     return (r_off * 2 + r_trans) * nblk + in_blk;
 }
 
-// Tile variant for an M x N output.  With fragment skipping every variant executes the same
-// ceil(M/8)*ceil(N/8) DMMA fragments per k-step, so the choice is about occupancy and operand traffic:
-// skinny outputs get skinny tiles (all warps busy), everything else the 64x64 tile at 3 CTAs/SM; the
-// 128x128 tile (half the operand traffic, but one CTA per SM, so ragged edges idle its warps) is used
-// only when enabled and the output fills its tiles.
-// Tuning knob: DMRG_VARIANT_MASK = bit mask of allowed variants.  Default 0b00001: the 64x64 tile only -- since its
-// consumer body is specialised on the warp's fragment counts it also handles skinny and tiny outputs better than the
-// dedicated 128x32 / 32x128 / 32x32 tiles did (cfg 5: 2338 -> 2274 ms, cfg 4: 159 -> 148 ms per H psi).
-static int choose_variant(int M, int N) {
-    static const int mask = [] { const char* e = getenv("DMRG_VARIANT_MASK"); const int m = e ? atoi(e) : 0; return (m & 31) ? (m & 31) | 1 : 1; }();
-    auto ok = [&](int v) { return (mask >> v) & 1; };
-    if (ok(4) && M <= 32 && N <= 32) return 4;
-    if (ok(2) && N <= 32 && M > 32) return 2;
-    if (ok(3) && M <= 32 && N > 32) return 3;
-    if (ok(1)) {
-        const double util = (double)M * N / (std::ceil(M / 128.0) * std::ceil(N / 128.0) * 16384.0);
-        if (util >= 0.75) return 1;
-    }
-    return 0;
-}
+// Tile variant for an M x N output: one variant today (64x64 tile, 2 x 2 consumer warps).  Since its consumer
+// body is specialised on the warp's fragment counts it also handled skinny and tiny outputs better than the
+// dedicated 128x32 / 32x128 / 32x32 / 128x128 tiles of round 1 did, which are gone.
+static int choose_variant(int /*M*/, int /*N*/) { return 0; }
 
 // cut a dimension d into full pieces of B plus the remainder.  (Equal-sized pieces were tried and lost: they
 // push every tile onto the kernel's ragged path, and the full-tile path is the fast one.)
@@ -86,24 +72,97 @@ __global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* 
 
 struct TileRec { Tile t; double cost; int64_t key = 0; };   // key: secondary launch order inside a cost bucket
 
-// widest N-merged stage-1 GEMM (tuning knob DMRG_MAX_MERGED_COLS)
-static const int64_t kMaxMergedCols = [] { const char* e = getenv("DMRG_MAX_MERGED_COLS"); const long v = e ? atol(e) : 0; return v >= 64 ? (int64_t)(v & ~1L) : int64_t(4096); }();
 constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are offsets into the packed R store
 
-// split-K policy of stage 2 (see the comment at its use)
-constexpr double kCtaSlots = 148.0 * 4;     // unit of the split-K wave count: 592 CTA slots (4 per SM with 16-column stages; the 32-column default keeps 3 resident -- the DMRG_SPLIT_WAVES sweep of DESIGN.md section 9 is in these units)
-static const double kSplitWaves = [] { const char* e = getenv("DMRG_SPLIT_WAVES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 200.0; }();
-static const double kMinSplitStages = [] { const char* e = getenv("DMRG_MIN_SPLIT_STAGES"); const double w = e ? atof(e) : 0; return w > 0 ? w : 768.0 / GEMM_BK; }();   // K = 768 per part at least
-static const bool kTileOrder = [] { const char* e = getenv("DMRG_TILE_ORDER"); return !e || atoi(e) != 0; }();   // knob: 0 = pure cost order
-// CTAs per thread-block cluster for the 64x64 tiles of stage 2 (1, 2, 4 or 8); tuning knob DMRG_CLUSTER.
-// Measured at cfg 5: clusters of 2 / 4 / 8 sibling tiles make stage 2 9-11 % SLOWER (gang scheduling costs more
-// occupancy than the shared L2 lines give back), so the default is 1 (no clusters).
-static const int kSplitSmall = [] { const char* e = getenv("DMRG_SPLIT_SMALL"); const int d = e ? atoi(e) : 0; return d > 0 ? d : 0; }();   // measurement knob, see emit_tiles
-static const int kCluster = [] { const char* e = getenv("DMRG_CLUSTER"); const int c = e ? atoi(e) : 1; return (c == 1 || c == 2 || c == 4 || c == 8) ? c : 1; }();
+// split-K policy of stage 2 (see the comment at its use): the wave count is in units of 592 CTA slots (the sweep of
+// DESIGN.md section 9 was taken with 4 resident CTAs per SM; the BK = 32 kernel keeps 3, the unit is kept so that the
+// recorded numbers stay comparable)
+constexpr double kCtaSlots = 148.0 * 4;
+
+struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
+    int64_t workspace_bytes;
+    int copy_mode;
+    double split_waves, min_split_stages;
+    int64_t max_merged_cols;
+    bool tile_order;
+    int split_small;
+    bool release_r_store;
+};
+
+static PlanPolicy make_policy(const dmrg_plan_options* o) {
+    PlanPolicy p;
+    p.workspace_bytes = (o && o->workspace_bytes > 0) ? o->workspace_bytes : (int64_t(8) << 30);
+    p.copy_mode = (o && (o->copy_mode == COPY_LDGSTS || o->copy_mode == COPY_TMA)) ? o->copy_mode : COPY_TMA;
+    p.split_waves = (o && o->split_waves > 0) ? o->split_waves : 200.0;
+    p.min_split_stages = (o && o->min_split_stages > 0) ? (double)o->min_split_stages : 768.0 / GEMM_BK;   // K = 768 per part at least
+    p.max_merged_cols = (o && o->max_merged_cols >= 64) ? (int64_t)(o->max_merged_cols & ~1) : int64_t(4096);
+    p.tile_order = !(o && o->cost_order_only);
+    p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
+    p.release_r_store = o && o->release_r_store;
+    return p;
+}
+
+// ---- tensor maps of the TMA path -----------------------------------------------------------------------------
+// One 2-D FP64 tensor map per operand matrix and orientation.  kind 0: the operand is read k-contiguous (box =
+// (GEMM_BK + 4) x tile rows), kind 1: m/n-contiguous (box = (tile + 4) x GEMM_BK): the 4 extra inner columns are the
+// bank-conflict padding of the shared-memory tile, written by the TMA unit itself.  Elements outside the matrix
+// (inner, outer) are zero-filled by the hardware.
+enum MapSpace : uint32_t { MS_OPS = 0, MS_X = 1, MS_PSI = 2, MS_PACK = 3 };
+struct MapDesc { uint32_t space; int32_t kind; int64_t off; int32_t inner, outer, ld; };
+
+struct MapTable {
+    std::vector<MapDesc> descs;
+    std::unordered_map<uint64_t, int32_t> index;
+    int32_t get(uint32_t space, int64_t off, int kind, int inner, int64_t outer, int ld) {
+        const uint64_t key = ((uint64_t)off << 3) | (space << 1) | (uint32_t)kind;
+        auto it = index.find(key);
+        if (it != index.end()) return it->second;
+        const int32_t id = (int32_t)descs.size();
+        descs.push_back({space, kind, off, inner, (int32_t)outer, ld});
+        index.emplace(key, id);
+        return id;
+    }
+};
+
+static int encode_tensor_maps(const std::vector<MapDesc>& descs, double* const base[4], std::vector<TensorMap>& out) {
+    static_assert(sizeof(TensorMap) == sizeof(CUtensorMap), "TensorMap must be the size of a CUtensorMap");
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    void* fp = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    DMRG_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fp, cudaEnableDefault, &qres));
+    if (!fp || qres != cudaDriverEntryPointSuccess) { set_error("dmrg_plan_create: cuTensorMapEncodeTiled is not available in this driver"); return DMRG_ECUDA; }
+    EncodeFn encode = (EncodeFn)fp;
+    out.resize(descs.size());
+    const int bm = kVariants[0].bm;
+    for (size_t i = 0; i < descs.size(); i++) {
+        const MapDesc& d = descs[i];
+        const cuuint64_t gdim[2] = {(cuuint64_t)d.inner, (cuuint64_t)d.outer};
+        const cuuint64_t gstride[1] = {(cuuint64_t)d.ld * 8};
+        const cuuint32_t box[2] = {(cuuint32_t)(d.kind == 0 ? GEMM_BK + 4 : bm + 4), (cuuint32_t)(d.kind == 0 ? bm : GEMM_BK)};
+        const cuuint32_t estride[2] = {1, 1};
+        const CUresult r = encode((CUtensorMap*)&out[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)(base[d.space] + d.off), gdim, gstride, box,
+                                  estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            set_error("dmrg_plan_create: cuTensorMapEncodeTiled failed (%d) for map %zu: space %u off %lld inner %d outer %d ld %d kind %d", (int)r, i,
+                      d.space, (long long)d.off, d.inner, d.outer, d.ld, d.kind);
+            return DMRG_ECUDA;
+        }
+    }
+    return DMRG_OK;
+}
 
 static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
                       const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
-                      int64_t workspace_bytes) {
+                      const PlanPolicy& pol) {
+    const int64_t workspace_bytes = pol.workspace_bytes;
+    const int64_t kMaxMergedCols = pol.max_merged_cols;
+    const double kSplitWaves = pol.split_waves, kMinSplitStages = pol.min_split_stages;
+    const bool kTileOrder = pol.tile_order;
+    const int kSplitSmall = pol.split_small;
+    P->copy_mode = pol.copy_mode;
     const dmrg_ops* S = P->ops;
     const auto& secL = S->sec[0];
     const auto& secR = S->sec[1];
@@ -230,7 +289,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
 
     // ---- chunk the (ordered) terms by X workspace --------------------------------------------------
     auto x_elems = [](const Task& k) { return (int64_t)k.dLi * round_up2(k.dRo); };
-    int64_t ws_elems = (workspace_bytes > 0 ? workspace_bytes : (int64_t(8) << 30)) / 8;
+    int64_t ws_elems = workspace_bytes / 8;
     {
         int64_t max_term = 0;
         std::unordered_map<int64_t, char> seen;
@@ -298,6 +357,14 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         for (int64_t b = 0; b < nblk; b++) { ppad[b] = o; o += (int64_t)P->blocks[b].dl * round_up2(P->blocks[b].dr); }
         P->psi_pad_elems = std::max<int64_t>(o, 2);
     }
+    // psi panels (all blocks of one R sector, contiguous in the padded copy): the matrices of the stage-1 A tensor maps
+    std::vector<int64_t> panel_first(nR, -1), panel_rows(nR, 0);
+    for (int64_t b = 0; b < nblk; b++) {
+        const int ir = P->blocks[b].ir;
+        if (panel_first[ir] < 0) panel_first[ir] = b;
+        panel_rows[ir] += P->blocks[b].dl;
+    }
+    MapTable maps;
 
     auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
         PlanGroup grp{stage, (int)P->launches.size(), 0};
@@ -319,7 +386,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             // list and get a launch of their own, so that ncu reports the small-block batch (HBM-bound) apart from the
             // large-block one (FP64-pipe bound).  Same kernel, same tiles, same results; default off.
             size_t nbig = r.size();
-            if (kSplitSmall > 0 && kCluster == 1)
+            if (kSplitSmall > 0)
                 nbig = std::stable_partition(r.begin(), r.end(), [&](const TileRec& a) {
                            const Job& j = jobs[a.t.job];
                            int d = std::min(j.M, j.N);
@@ -329,13 +396,13 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             // grid.x limit: split very long lists
             size_t i = 0;
             if (nbig > 0 && nbig < r.size()) {
-                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)nbig, (stage == 2 && v == 0) ? kCluster : 1});
+                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)nbig});
                 for (size_t j = 0; j < nbig; j++) tiles.push_back(r[j].t);
                 i = nbig;
             }
             while (i < r.size()) {
-                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);   // a multiple of every cluster size
-                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n, (stage == 2 && v == 0) ? kCluster : 1});
+                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);
+                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n});
                 for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
                 i += n;
             }
@@ -439,7 +506,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     const Run& Rc = runs[rblks[c].r0 + t];
                     int64_t rr = 0;
                     for (size_t q = Rc.i; q < Rc.j; q++) {
-                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx};
+                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx, xtop, (int32_t)rows, (int32_t)rr, (int32_t)col0s[c - c0]};
                         rr += P->blocks[req[q].in_blk].dl;
                     }
                     s1_flops += 2.0 * rows * dRi * req[Rc.i].dRo;
@@ -450,7 +517,14 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 s.a_off = ppad[req[R0.i].in_blk]; s.lda = ldp;
                 s.b_off = kPackBase + pack_top; s.ldb = ldp;   // resolved to an offset from the operator store at upload
                 s.K = dRi; s.alpha = 1.0;
-                s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_VEC2 | SEG_A_VEC2 | SEG_B_KCONTIG;
+                s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_KCONTIG;
+                {
+                    const int64_t pf = panel_first[Bt.ir];
+                    s.a_map = maps.get(MS_PSI, ppad[pf], 0, dRi, panel_rows[Bt.ir], ldp);
+                    s.a_i0 = 0; s.a_o0 = (int32_t)((ppad[req[R0.i].in_blk] - ppad[pf]) / ldp);
+                    s.b_map = maps.get(MS_PACK, pack_top, 0, dRi, ncols, ldp);
+                    s.b_i0 = 0; s.b_o0 = 0;
+                }
                 pack_segs.push_back(segs.size());
                 Job jb;
                 jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = (int)ncols;
@@ -528,20 +602,24 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 s.alpha = k.alpha;
                 s.K = k.dLi;
                 s.flags = 0;
+                s.a_map = s.b_map = 0; s.a_i0 = s.a_o0 = s.b_i0 = s.b_o0 = 0;
                 if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
                 else {
                     s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
-                    s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | SEG_A_VEC2 | (k.l_trans ? SEG_A_MCONTIG : 0);
+                    s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | (k.l_trans ? SEG_A_MCONTIG : 0);
+                    s.a_map = k.l_trans ? maps.get(MS_OPS, k.l_off, 1, k.dLo, k.dLi, s.lda) : maps.get(MS_OPS, k.l_off, 0, k.dLi, k.dLo, s.lda);
                 }
                 if (k.r_off < 0) {
                     const dmrg_psi_block& IB = P->blocks[k.in_blk];
                     s.b_off = ppad[k.in_blk]; s.ldb = (int)round_up2(IB.dr);
-                    s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
+                    s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT);
                     if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
+                    else s.b_map = maps.get(MS_PSI, ppad[k.in_blk], 1, IB.dr, IB.dl, s.ldb);
                 } else {
                     const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
                     s.b_off = xl.off; s.ldb = xl.ld;
-                    s.flags |= (SP_X << SEG_B_SPACE_SHIFT) | SEG_B_VEC2;
+                    s.flags |= (SP_X << SEG_B_SPACE_SHIFT);
+                    if (!ident) { s.b_map = maps.get(MS_X, xl.job_off, 1, xl.ld, xl.job_rows, xl.ld); s.b_i0 = xl.c0; s.b_o0 = xl.r0; }
                     alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
                 }
                 if (!ident) {
@@ -564,25 +642,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             int part_no = 0;
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
                 const int64_t key = (int64_t)OB.il * 65536 + part_no++;
-                if (g.variant != 0 || kCluster == 1) {
-                    for (auto& a : cut_m)
-                        for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
-                    return;
-                }
-                // 64x64 tiles of stage 2 are emitted in sibling groups of kCluster (CM x CN neighbouring tiles, padded
-                // with empty tiles): one thread-block cluster each.  Equal costs + stable sort keep a group together.
-                const int CN = kCluster >= 2 ? 2 : 1, CM = kCluster / CN;
-                for (size_t a0 = 0; a0 < cut_m.size(); a0 += CM)
-                    for (size_t b0 = 0; b0 < cut_n.size(); b0 += CN)
-                        for (int da = 0; da < CM; da++)
-                            for (int db = 0; db < CN; db++) {
-                                if (a0 + da < cut_m.size() && b0 + db < cut_n.size()) {
-                                    const auto &a = cut_m[a0 + da], &b = cut_n[b0 + db];
-                                    recs[0].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
-                                } else {
-                                    recs[0].push_back({{-1, 0, 0, 0, 0}, cost, key});
-                                }
-                            }
+                for (auto& a : cut_m)
+                    for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
             };
             Job jb;
             jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
@@ -639,7 +700,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     P->stats[ST_S1_FLOPS] = s1_flops;
     P->stats[ST_S2_FLOPS] = s2_flops;
     P->stats[ST_PADDED_FLOPS] = padded_flops;
-    P->stats[ST_STAGE_FLOPS] = stage_flops;   // K padded to whole 16-wide stages per segment
+    P->stats[ST_STAGE_FLOPS] = stage_flops;   // K padded to whole GEMM_BK-wide stages per segment
     P->stats[ST_WARP_FLOPS] = warp_flops;     // ... M, N padded to the most loaded warp of each tile
     P->stats[ST_TILE_FLOPS] = tile_flops;     // ... and M, N padded to whole tiles: what a fill-independent tile time costs
     P->stats[ST_S1_JOBS] = (double)s1_jobs;
@@ -665,8 +726,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
 
     // ---- upload ---------------------------------------------------------------------------------------
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
+    P->stats[ST_XWS_ELEMS] = (double)P->xws_elems;
     P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
-                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + 8.0 * P->xws_elems + 8.0 * pack_top);
+                                         hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +
+                                         8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems);
     if (S->structure_only) return DMRG_OK;
     auto up = [&](void** dptr, const void* src, size_t bytes) -> int {
         DMRG_CUDA(cudaMalloc(dptr, std::max<size_t>(bytes, 16)));
@@ -690,11 +753,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
     if ((rc = up((void**)&P->d_hd_tiles, hd_tiles.data(), hd_tiles.size() * sizeof(HdTile)))) return rc;
     DMRG_CUDA(cudaMalloc(&P->d_xws, sizeof(double) * (size_t)P->xws_elems));
-    for (int v = 0; v < NUM_VARIANTS; v++) {
-        DMRG_CUDA(cudaStreamCreateWithFlags(&P->aux[v], cudaStreamNonBlocking));
-        DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_join[v], cudaEventDisableTiming));
+    {   // tensor maps hold absolute device addresses: encoded once every buffer they point into exists
+        double* const base[4] = {S->d_values, P->d_xws, P->d_psi_pad, P->d_pack};
+        std::vector<TensorMap> tm;
+        if ((rc = encode_tensor_maps(maps.descs, base, tm))) return rc;
+        if ((rc = up((void**)&P->d_tmaps, tm.data(), tm.size() * sizeof(TensorMap)))) return rc;
     }
-    DMRG_CUDA(cudaEventCreateWithFlags(&P->ev_fork, cudaEventDisableTiming));
     if (!packs.empty()) {
         PackDesc* d_packs = nullptr;
         DMRG_CUDA(cudaMalloc(&d_packs, packs.size() * sizeof(PackDesc)));
@@ -792,14 +856,19 @@ __global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ 
 
 using namespace dmrg;
 
-// tuning knob: DMRG_NO_FORK=1 runs the launches of a group back to back on the caller's stream
-static const bool kNoFork = [] { const char* e = getenv("DMRG_NO_FORK"); return e && atoi(e) != 0; }();
-
 extern "C" {
 
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms, const double* site_ops,
                      const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
                      int64_t workspace_bytes, dmrg_plan** out) {
+    dmrg_plan_options o = {};
+    o.workspace_bytes = workspace_bytes;
+    return dmrg_plan_create_opts(ops, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, &o, out);
+}
+
+int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms, const double* site_ops,
+                          const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
+                          const dmrg_plan_options* options, dmrg_plan** out) {
     if (!out) { set_error("dmrg_plan_create: out is NULL"); return DMRG_EINVAL; }
     *out = nullptr;
     if (!ops || nterms < 0 || (nterms > 0 && !terms) || !site_ops || !site_parity || nsite <= 0) {
@@ -811,7 +880,7 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
     P->ops = ops;
     int rc;
     try {
-        rc = plan_build(P, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, workspace_bytes);
+        rc = plan_build(P, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, make_policy(options));
     } catch (const std::bad_alloc&) {
         set_error("dmrg_plan_create: out of host memory");
         rc = DMRG_ENOMEM;
@@ -827,13 +896,8 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io); cudaFree(P->d_tmaps);
     for (auto e : P->ev) cudaEventDestroy(e);
-    for (int v = 0; v < NUM_VARIANTS; v++) {
-        if (P->aux[v]) cudaStreamDestroy(P->aux[v]);
-        if (P->ev_join[v]) cudaEventDestroy(P->ev_join[v]);
-    }
-    if (P->ev_fork) cudaEventDestroy(P->ev_fork);
     if (P->dav) davidson_ws_free(P->dav);
     delete P;
 }
@@ -890,8 +954,6 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
     for (size_t gi = 0; gi < ng; gi++) {
         const PlanGroup& G = P->groups[gi];
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi], st));
-        // the launches of a group (one per tile variant) are independent: the first runs on the caller's
-        // stream, the others on side streams forked from / joined to it, so their tails overlap
         if (G.stage == 3) {   // first_launch / nlaunch index the reduction table here
             for (int y0 = 0; y0 < G.nlaunch; y0 += 32768) {
                 const unsigned ny = (unsigned)std::min(32768, G.nlaunch - y0);
@@ -901,18 +963,11 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
             if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
             continue;
         }
-        if (G.nlaunch > 1) DMRG_CUDA(cudaEventRecord(P->ev_fork, st));
-        for (int li = 0; li < G.nlaunch; li++) {
+        for (int li = 0; li < G.nlaunch; li++) {   // more than one launch per group only with split_small (measurement aid)
             const PlanLaunch& L = P->launches[G.first_launch + li];
-            cudaStream_t ls = (li == 0 || kNoFork) ? st : P->aux[li % NUM_VARIANTS];
-            if (li > 0 && !kNoFork) DMRG_CUDA(cudaStreamWaitEvent(ls, P->ev_fork, 0));
-            int rc = launch_grouped_gemm(L.variant, L.cluster, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
-                                         P->ops->d_values, P->d_xws, P->d_psi_pad, sigma, ls);
+            int rc = launch_grouped_gemm(L.variant, P->copy_mode, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
+                                         P->ops->d_values, P->d_xws, P->d_psi_pad, sigma, P->d_tmaps, st);
             if (rc != DMRG_OK) return rc;
-            if (li > 0 && !kNoFork) {
-                DMRG_CUDA(cudaEventRecord(P->ev_join[li % NUM_VARIANTS], ls));
-                DMRG_CUDA(cudaStreamWaitEvent(st, P->ev_join[li % NUM_VARIANTS], 0));
-            }
         }
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
     }

@@ -10,12 +10,12 @@ struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, npa
 
 struct PackDesc { int64_t src, dst; int32_t dRo, dRi, src_ld, trans, ldp, pad_; };   // one R block copied into the packed stage-1 store
 
-struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; int cluster; };   // cluster: CTAs per thread-block cluster (1 = none)
+struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
 struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent (stage 3: range of the RedJob table)
 
 enum {
     ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
-    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_WARP_FLOPS, ST_COUNT
+    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_WARP_FLOPS, ST_XWS_ELEMS, ST_COUNT
 };
 
 struct DavidsonWs;
@@ -31,12 +31,12 @@ struct dmrg_plan {
     int64_t xws_elems = 0;
     std::vector<PlanLaunch> launches;
     std::vector<PlanGroup> groups;
-    cudaStream_t aux[dmrg::NUM_VARIANTS] = {nullptr};   // side streams: independent launches of a group overlap
-    cudaEvent_t ev_fork = nullptr, ev_join[dmrg::NUM_VARIANTS] = {nullptr};
+    int copy_mode = 2;   // operand staging of the GEMM kernel (dmrg_plan_options.copy_mode)
     RedJob* d_reds = nullptr;
     double* d_psi_pad = nullptr;   // psi re-laid with even leading dimensions (16-byte cp.async for every operand)
     int64_t psi_pad_elems = 0;
     double* d_host_io = nullptr;   // device staging of dmrg_sigma_host (psi, sigma), allocated on first use
+    dmrg::TensorMap* d_tmaps = nullptr;   // tensor maps of the TMA path (one per operand matrix and orientation)
     double* d_pack = nullptr;   // packed, N-merged, K-contiguous copies of the R blocks (stage-1 B operands)
     HdItem* d_hd_items = nullptr;
     HdBlock* d_hd_blocks = nullptr;

@@ -189,30 +189,34 @@ def test_error_paths():
     ops.free()
 
 
-def test_split_small_knob_gives_bitwise_same_sigma(tmp_path):
-    """DMRG_SPLIT_SMALL (the ncu measurement knob of profiles/r1_cfg5_final.md section 7) only regroups tiles into
-    launches: sigma must be bitwise the same with and without it.  The knob is read at library load: subprocesses."""
-    import os
-    import subprocess
-    import sys
-    _gpu()
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    code = ("import sys, numpy as np, torch\n"
-            "import paper_2311_02854_b200 as g\n"
-            "from dmrg_workload.problem import make_direct_problem, random_psi\n"
-            "pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)\n"
-            "ops, plan = g.load_problem(pr)\n"
-            "psi = torch.from_numpy(random_psi(pr.psi_size, 11)).cuda()\n"
-            "sig = torch.empty_like(psi)\n"
-            "plan.sigma(psi, sig, torch.cuda.current_stream()); torch.cuda.synchronize()\n"
-            "np.save(sys.argv[1], sig.cpu().numpy()); print(plan.stats()['launches'])\n")
-    launches, sig = [], []
-    for knob in ("0", "16"):
-        out = str(tmp_path / f"sigma_{knob}.npy")
-        env = dict(os.environ, DMRG_SPLIT_SMALL=knob, PYTHONPATH=root)
-        r = subprocess.run([sys.executable, "-c", code, out], env=env, cwd=root, capture_output=True, text=True, timeout=600)
-        assert r.returncode == 0, r.stderr
-        launches.append(float(r.stdout.strip().splitlines()[-1]))
-        sig.append(np.load(out))
-    assert launches[1] > launches[0]
-    assert np.linalg.norm(sig[0]) > 0 and np.array_equal(sig[0], sig[1])
+def test_plan_options_give_the_same_sigma():
+    """split_small only regroups tiles into launches and copy_mode only changes how operand tiles reach shared
+    memory (TMA tensor copies vs 16-byte cp.async): sigma must be BITWISE the same; split-K granularity, stack width
+    and tile order only change rounding order / launch order."""
+    g = _gpu()
+    from dmrg_workload.problem import make_direct_problem
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr)
+    psi = random_psi(pr.psi_size, 11)
+    ref = _sigma_gpu(plan, psi)
+    orc = oracle.opair_sigma(pr, psi)
+    assert np.abs(ref - orc).max() / np.linalg.norm(orc) <= TOL_SIGMA
+
+    def variant(**kw):
+        p2 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, **kw)
+        out = _sigma_gpu(p2, psi)
+        st = p2.stats()
+        p2.destroy()
+        return out, st
+
+    out, st = variant(split_small=16)
+    assert st["launches"] > plan.stats()["launches"] and np.array_equal(out, ref)
+    out, _ = variant(copy_mode=g.COPY_LDGSTS)
+    assert np.array_equal(out, ref)
+    out, _ = variant(copy_mode=g.COPY_TMA, cost_order_only=1)
+    assert np.array_equal(out, ref)
+    for kw in (dict(split_waves=4000.0, min_split_stages=1), dict(max_merged_cols=64), dict(workspace_bytes=1, copy_mode=g.COPY_LDGSTS)):
+        out, _ = variant(**kw)
+        assert np.abs(out - orc).max() / np.linalg.norm(orc) <= TOL_SIGMA, kw
+    plan.destroy()
+    ops.free()

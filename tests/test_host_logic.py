@@ -164,24 +164,37 @@ def test_stage1_is_n_merged():
     ops.free()
 
 
-def test_split_small_knob_only_regroups_launches():
-    """DMRG_SPLIT_SMALL (measurement knob for ncu) moves small-block tiles into launches of their own: same tiles,
-    same work, more launches.  The knob is read when the library is loaded, hence the subprocesses."""
-    import json
-    import subprocess
-    import sys
-    code = ("import json, paper_2311_02854_b200 as g\n"
-            "from dmrg_workload.problem import make_direct_problem\n"
-            "pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)\n"
-            "ops, plan = g.load_problem(pr, structure_only=True)\n"
-            "print(json.dumps(plan.stats()))\n")
-    out = []
-    for knob in ("0", "16"):
-        env = dict(os.environ, DMRG_SPLIT_SMALL=knob, PYTHONPATH=ROOT)
-        r = subprocess.run([sys.executable, "-c", code], env=env, cwd=ROOT, capture_output=True, text=True, timeout=300)
-        assert r.returncode == 0, r.stderr
-        out.append(json.loads(r.stdout.strip().splitlines()[-1]))
-    a, b = out
+def test_split_small_option_only_regroups_launches():
+    """dmrg_plan_options.split_small (measurement aid for ncu) moves small-block tiles into launches of their own:
+    same tiles, same work, more launches."""
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr, structure_only=True)
+    plan16 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, split_small=16)
+    a, b = plan.stats(), plan16.stats()
     for k in ("s1_tiles", "s2_tiles", "s1_flops", "s2_flops", "padded_flops", "tasks", "chunks"):
         assert a[k] == b[k], k
     assert b["launches"] > a["launches"]
+    plan16.destroy()
+    plan.destroy()
+    ops.free()
+
+
+def test_plan_options_are_validated_and_structural():
+    """Every policy of the planner is an explicit dmrg_plan_options field (no environment variables): split-K
+    granularity and merged-stack width change the number of tiles / jobs but never the executed flops of stage 2."""
+    import subprocess
+    src = open(os.path.join(ROOT, "paper_2311_02854_b200", "csrc", "plan.cu")).read()
+    assert "getenv" not in src
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr, structure_only=True)
+    a = plan.stats()
+    fine = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, split_waves=4000.0, min_split_stages=1)
+    narrow = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, max_merged_cols=64)
+    assert fine.stats()["s2_tiles"] > a["s2_tiles"] and fine.stats()["s2_flops"] == a["s2_flops"]
+    assert narrow.stats()["s1_jobs"] > a["s1_jobs"] and narrow.stats()["s1_flops"] == a["s1_flops"]
+    assert a["xws_elems"] >= 2
+    with pytest.raises(TypeError):
+        g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, no_such_option=1)
+    for p_ in (fine, narrow, plan):
+        p_.destroy()
+    ops.free()
