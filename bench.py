@@ -50,6 +50,9 @@ def parse():
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="dmrg_plan_options field (copy_mode, split_waves, min_split_stages, max_merged_cols, "
                          "cost_order_only, split_small, release_r_store); repeatable")
+    ap.add_argument("--sigma-only", type=int, default=0, metavar="N",
+                    help="profiling mode: no Davidson, no oracle; N plain dmrg_sigma calls (after one warm-up call) and a short "
+                         "JSON line with the per-stage device times -- the command the ncu captures under profiles/ wrap")
     ap.add_argument("--operators", default="default", choices=["default", "direct", "renorm"],
                     help="cfg3-5 operator values: direct fill (seeded random blocks) or GPU renormalization (NEXT-1)")
     return ap.parse_args()
@@ -242,6 +245,24 @@ def main():
     x = torch.from_numpy(psi_h).cuda()
     sig = torch.empty_like(x)
 
+    if args.sigma_only > 0:
+        plan.sigma(x, sig, stream)
+        torch.cuda.synchronize()
+        plan.set_timing(True)
+        rows = []
+        for _ in range(args.sigma_only):
+            plan.sigma(x, sig, stream)
+            rows.append(plan.stage_ms())
+        med = [float(np.median([r[i] for r in rows])) for i in range(3)]
+        fl = st["s1_flops"] + st["s2_flops"]
+        print(json.dumps({"mode": "sigma-only", "config": workload_name(args.config, pr), "calls": args.sigma_only, "plan_options": popts,
+                          "stage1_ms": med[0], "stage2_ms": med[1], "hpsi_ms": med[2], "executed_tflops": fl / med[2] * 1e-9,
+                          "s1_tflops": st["s1_flops"] / med[0] * 1e-9, "s2_tflops": st["s2_flops"] / med[1] * 1e-9,
+                          "launches_per_hpsi": int(st["launches"]), "chunks": int(st["chunks"]),
+                          "stats": {k: st[k] for k in ("s1_flops", "s2_flops", "padded_flops", "stage_flops", "warp_flops", "canon_flops", "s1_tiles", "s2_tiles")}}))
+        plan.destroy()
+        ops.free()
+        return
     # FP64 pipe peak, measured live under the same conditions (roofline denominator)
     peak_dmma = g.fp64_peak_tflops(1, 300.0, stream)
     peak_dfma = g.fp64_peak_tflops(0, 300.0, stream)

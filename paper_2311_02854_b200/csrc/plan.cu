@@ -14,6 +14,7 @@
 //   * no grouping by equal shape: a single kernel walks a cost-sorted tile list with per-tile shapes.
 // Terms are processed in chunks sized so the X intermediates fit the workspace.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdlib>
 #include <new>
@@ -112,9 +113,18 @@ struct MapDesc { uint32_t space; int32_t kind; int64_t off; int32_t inner, outer
 
 struct MapTable {
     std::vector<MapDesc> descs;
-    std::unordered_map<uint64_t, int32_t> index;
+    struct KeyHash {
+        size_t operator()(const std::array<int64_t, 3>& k) const {
+            uint64_t h = 0x9E3779B97F4A7C15ull;
+            for (int64_t v : k) h = (h ^ (uint64_t)v) * 0xBF58476D1CE4E5B9ull + (h >> 29);
+            return (size_t)h;
+        }
+    };
+    std::unordered_map<std::array<int64_t, 3>, int32_t, KeyHash> index;
+    // the X workspace is reused by every chunk, so the same offset can carry matrices of different shapes: the key
+    // is the whole descriptor, not the address alone
     int32_t get(uint32_t space, int64_t off, int kind, int inner, int64_t outer, int ld) {
-        const uint64_t key = ((uint64_t)off << 3) | (space << 1) | (uint32_t)kind;
+        const std::array<int64_t, 3> key = {(off << 3) | (int64_t)(space << 1) | kind, ((int64_t)inner << 32) | (uint32_t)ld, outer};
         auto it = index.find(key);
         if (it != index.end()) return it->second;
         const int32_t id = (int32_t)descs.size();
