@@ -179,6 +179,7 @@ int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host
  * 13 executed flops with every segment's K padded to whole GEMM_BK(= 32)-wide pipeline stages
  * 14 the same with M and N padded to whole tiles as well; 15 ... padded to each tile's most loaded warp
  * 16 doubles allocated for the X workspace (X intermediates + split-K partial tiles of the largest chunk)
+ * 17 tensor maps of the TMA path (one per operand matrix and orientation, 128 bytes each)
  *                                           */
 double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
 

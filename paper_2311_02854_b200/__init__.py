@@ -31,7 +31,7 @@ COPY_LDGSTS, COPY_TMA = 1, 2
 
 STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
              "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops",
-             "xws_elems")
+             "xws_elems", "tensor_maps")
 
 EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_create_opts", "dmrg_plan_destroy",
            "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",

@@ -48,9 +48,12 @@ enum : uint32_t {
 };
 
 // One K-segment of a grouped GEMM job:  C += alpha * A(M x K) * B(K x N)
-// Operands are addressed twice: as (space, offset, ld) for the cp.async path and the identity-A prologue, and as
-// (tensor map, origin of the operand inside the mapped matrix) for the TMA path.  i0 / o0 are the origin along the
-// map's inner (contiguous) / outer dimension; the kernel adds the tile and K offsets.
+// Operands are addressed twice: as (space, offset, ld) for the cp.async path and the identity-A prologue, and as a
+// tensor map for the TMA path.  A tensor map covers exactly the operand (an operator block, an X slice, a psi
+// block, a packed R stack), so everything outside it is zero-filled by the TMA unit; the one exception is the
+// stage-1 A operand, a run of psi rows inside its panel's map, whose first row is a_o0.  The TMA box of a map is
+// sized to the operand (planner: box_shape): a_pitch / b_pitch = its inner dimension in doubles = the row pitch of
+// the shared-memory tile (always = 4 mod 8: conflict-free fragment loads), a_bytes / b_bytes = its size.
 struct Seg {
     int64_t  a_off;
     int64_t  b_off;
@@ -59,7 +62,9 @@ struct Seg {
     uint32_t flags;
     double   alpha;
     int32_t  a_map, b_map;
-    int32_t  a_i0, a_o0, b_i0, b_o0;
+    int32_t  a_o0;
+    uint16_t a_pitch, b_pitch;
+    uint32_t a_bytes, b_bytes;
 };
 static_assert(sizeof(Seg) == 64, "Seg layout");
 

@@ -16,12 +16,13 @@
 // Staging global -> shared (plan option copy_mode):
 //   * TMA (default): every operand matrix has a 2-D tensor map (cuTensorMapEncodeTiled, FP64 elements) built by the
 //     planner; one elected producer lane issues ONE cp.async.bulk.tensor.2d (SASS UTMALDG) per operand and stage,
-//     completion counted in bytes on the stage's "full" mbarrier (expect_tx).  The box is 36 x BM (k-contiguous
-//     operand) or (BM+4) x 32 (m/n-contiguous): the inner box dimension carries the 4 padding columns that make
-//     the fragment loads bank-conflict free, so TMA itself writes the padded shared-memory layout.  Elements
-//     outside the operand matrix are zero-filled by the TMA unit (ragged M, N, K tails cost nothing); rows or
-//     columns that belong to a neighbouring sub-matrix (X slices, psi runs) only feed accumulator rows / columns
-//     that are never stored, and the K tail of such slices is masked in registers (compute_stage).
+//     completion counted in bytes on the stage's "full" mbarrier (expect_tx).  The box is at most 36 x BM (k-contiguous
+//     operand) or (BM+4) x 32 (m/n-contiguous) and is shrunk to the operand (a 5 x 300 block is staged as 12 x 64
+//     boxes, an 8-column X slice as 12 x 32): the inner box dimension is the extent rounded up to 8 plus 4 padding
+//     columns, i.e. = 4 mod 8 doubles, which makes the fragment loads bank-conflict free -- TMA itself writes the
+//     padded shared-memory layout, with the pitch travelling in the stage metadata.  Elements outside the operand
+//     matrix are zero-filled by the TMA unit (ragged M, N, K tails cost no global traffic); the K tail is
+//     additionally masked in registers (compute_stage), which the cp.async path and psi runs rely on.
 //   * 16-byte cp.async (LDGSTS) with zero-fill (src-size 0) by all 32 producer lanes: the round-1 path, kept as a
 //     selectable alternative (it needs no tensor maps).
 // Every operand the planner emits is 16-byte aligned with an even leading dimension (operator blocks and the
@@ -52,7 +53,7 @@ __device__ __forceinline__ double lds64(uint32_t addr) {
     return v;
 }
 
-struct StageMeta { double alpha; uint32_t flags; int32_t kvalid; };   // kvalid: k-columns of this stage inside the segment
+struct StageMeta { double alpha; uint32_t flags; int32_t kvalid; uint32_t a_pitch, b_pitch; };   // kvalid: k-columns of this stage inside the segment; pitches in doubles
 
 // ---- mbarrier helpers (shared::cta) ----------------------------------------------------------------
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -298,9 +299,9 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
             const StageMeta mt = cx.meta[slot];
             const bool a_kc = !(mt.flags & SEG_A_MCONTIG);
             const bool b_kc = (mt.flags & SEG_B_KCONTIG) != 0;
-            // element (m,k) of A: a_kc ? m*KPAD + k : k*(BM+4) + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
-            const int a_sm = a_kc ? KPAD : 1, a_sk = a_kc ? 1 : BM + 4;
-            const int b_sn = b_kc ? KPAD : 1, b_sk = b_kc ? 1 : BN + 4;
+            // element (m,k) of A: a_kc ? m*pitch + k : k*pitch + m ; fragment: m = wm0+8i+lr, k = 4kk+lc
+            const int a_sm = a_kc ? (int)mt.a_pitch : 1, a_sk = a_kc ? 1 : (int)mt.a_pitch;
+            const int b_sn = b_kc ? (int)mt.b_pitch : 1, b_sk = b_kc ? 1 : (int)mt.b_pitch;
             const uint32_t pa = sa + 8u * (uint32_t)((wm0 + lr) * a_sm + lc * a_sk);
             const uint32_t pb = sb + 8u * (uint32_t)((wn0 + lr) * b_sn + lc * b_sk);
             const int mode = (mt.flags & SEG_ALPHA_ONE) ? 0 : ((mt.flags & SEG_ALPHA_NEG) ? 1 : 2);   // integer test: no FP64-pipe DSETP
@@ -388,8 +389,6 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
         if (copy_mode == COPY_TMA) {
             // ---- TMA: one elected lane, two tensor copies per stage ------------------------------------
             if (lane != 0) return;
-            constexpr uint32_t A_KC_BYTES = KPAD * BM * 8, A_MC_BYTES = (BM + 4) * BK * 8;
-            constexpr uint32_t B_KC_BYTES = KPAD * BN * 8, B_MC_BYTES = (BN + 4) * BK * 8;
             for (int it = 0; it < nstages; it++) {
                 const int slot = it % NST;
                 if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
@@ -401,9 +400,11 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
                 meta[slot].alpha = ls.alpha;
                 meta[slot].flags = ls.flags;
                 meta[slot].kvalid = min(ls.K - lk0, BK);
-                mbar_arrive_expect_tx(bar, (a_kc ? A_KC_BYTES : A_MC_BYTES) + (b_kc ? B_KC_BYTES : B_MC_BYTES));   // release: publishes meta[slot]
-                tma_load_2d(sa, tmaps + ls.a_map, a_kc ? ls.a_i0 + lk0 : ls.a_i0 + m0, a_kc ? ls.a_o0 + m0 : ls.a_o0 + lk0, bar);
-                tma_load_2d(sb, tmaps + ls.b_map, b_kc ? ls.b_i0 + lk0 : ls.b_i0 + n0, b_kc ? ls.b_o0 + n0 : ls.b_o0 + lk0, bar);
+                meta[slot].a_pitch = ls.a_pitch;
+                meta[slot].b_pitch = ls.b_pitch;
+                mbar_arrive_expect_tx(bar, ls.a_bytes + ls.b_bytes);   // release: publishes meta[slot]
+                tma_load_2d(sa, tmaps + ls.a_map, a_kc ? lk0 : m0, a_kc ? ls.a_o0 + m0 : lk0, bar);
+                tma_load_2d(sb, tmaps + ls.b_map, b_kc ? lk0 : n0, b_kc ? n0 : lk0, bar);
                 lk0 += BK;
                 if (lk0 >= ls.K) {
                     lk0 = 0;
@@ -439,6 +440,8 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
                 meta[slot].alpha = ls.alpha;
                 meta[slot].flags = ls.flags;
                 meta[slot].kvalid = min(k_lim, BK);
+                meta[slot].a_pitch = a_kc ? KPAD : BM + 4;
+                meta[slot].b_pitch = b_kc ? KPAD : BN + 4;
                 mbar_arrive(bar);   // release: publishes meta[slot]
             }
             lk0 += BK;

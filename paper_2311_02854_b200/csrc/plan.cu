@@ -18,6 +18,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <new>
+#include <thread>
 #include <unordered_map>
 
 #include <cuda.h>   // CUtensorMap types only; the encoder is reached through cudaGetDriverEntryPoint (no libcuda link)
@@ -37,7 +38,7 @@ struct Task {
     double alpha;
 };
 
-struct XLoc { int64_t off; int32_t ld; int64_t job_off; int32_t job_rows, r0, c0; };   // X of one task: a slice of a stage-1 job's output matrix
+struct XLoc { int64_t off; int32_t ld; };   // X of one task: a slice (origin, row pitch) of a stage-1 job's output matrix
 
 static inline int64_t xkey(int64_t r_off, int r_trans, int in_blk, int64_t nblk) {
     return (r_off * 2 + r_trans) * nblk + in_blk;
@@ -109,26 +110,38 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
 // bank-conflict padding of the shared-memory tile, written by the TMA unit itself.  Elements outside the matrix
 // (inner, outer) are zero-filled by the hardware.
 enum MapSpace : uint32_t { MS_OPS = 0, MS_X = 1, MS_PSI = 2, MS_PACK = 3 };
-struct MapDesc { uint32_t space; int32_t kind; int64_t off; int32_t inner, outer, ld; };
+struct MapDesc { uint32_t space; int32_t kind; int64_t off; int32_t inner, outer, ld, box_inner, box_outer; };
+
+// Box of an operand with `k` k-columns per segment and `mn` rows (kind 0) / columns (kind 1) in all:
+//   kind 0 (k-contiguous):   inner = min(GEMM_BK, round_up8(k)) + 4 doubles, outer = min(tile, round_up8(mn)) rows
+//   kind 1 (m/n-contiguous): inner = min(tile, round_up8(mn)) + 4 doubles,   outer = min(GEMM_BK, round_up4(k)) k-rows
+// inner = 4 mod 8 in every case (bank-conflict-free fragment loads); short segments and narrow blocks get small boxes.
+struct BoxShape { int inner, outer; };
+static inline BoxShape box_shape(int kind, int k, int64_t mn, int tile) {
+    const int k8 = std::min(GEMM_BK, (k + 7) & ~7), k4 = std::min(GEMM_BK, (k + 3) & ~3);
+    const int mn8 = (int)std::min<int64_t>(tile, (mn + 7) & ~int64_t(7));
+    return kind == 0 ? BoxShape{k8 + 4, mn8} : BoxShape{mn8 + 4, k4};
+}
 
 struct MapTable {
     std::vector<MapDesc> descs;
     struct KeyHash {
-        size_t operator()(const std::array<int64_t, 3>& k) const {
+        size_t operator()(const std::array<int64_t, 4>& k) const {
             uint64_t h = 0x9E3779B97F4A7C15ull;
             for (int64_t v : k) h = (h ^ (uint64_t)v) * 0xBF58476D1CE4E5B9ull + (h >> 29);
             return (size_t)h;
         }
     };
-    std::unordered_map<std::array<int64_t, 3>, int32_t, KeyHash> index;
+    std::unordered_map<std::array<int64_t, 4>, int32_t, KeyHash> index;
     // the X workspace is reused by every chunk, so the same offset can carry matrices of different shapes: the key
     // is the whole descriptor, not the address alone
-    int32_t get(uint32_t space, int64_t off, int kind, int inner, int64_t outer, int ld) {
-        const std::array<int64_t, 3> key = {(off << 3) | (int64_t)(space << 1) | kind, ((int64_t)inner << 32) | (uint32_t)ld, outer};
+    int32_t get(uint32_t space, int64_t off, int kind, int inner, int64_t outer, int ld, BoxShape box) {
+        const std::array<int64_t, 4> key = {(off << 3) | (int64_t)(space << 1) | kind, ((int64_t)inner << 32) | (uint32_t)ld, outer,
+                                            ((int64_t)box.inner << 16) | box.outer};
         auto it = index.find(key);
         if (it != index.end()) return it->second;
         const int32_t id = (int32_t)descs.size();
-        descs.push_back({space, kind, off, inner, (int32_t)outer, ld});
+        descs.push_back({space, kind, off, inner, (int32_t)outer, ld, box.inner, box.outer});
         index.emplace(key, id);
         return id;
     }
@@ -145,22 +158,38 @@ static int encode_tensor_maps(const std::vector<MapDesc>& descs, double* const b
     if (!fp || qres != cudaDriverEntryPointSuccess) { set_error("dmrg_plan_create: cuTensorMapEncodeTiled is not available in this driver"); return DMRG_ECUDA; }
     EncodeFn encode = (EncodeFn)fp;
     out.resize(descs.size());
-    const int bm = kVariants[0].bm;
-    for (size_t i = 0; i < descs.size(); i++) {
-        const MapDesc& d = descs[i];
-        const cuuint64_t gdim[2] = {(cuuint64_t)d.inner, (cuuint64_t)d.outer};
-        const cuuint64_t gstride[1] = {(cuuint64_t)d.ld * 8};
-        const cuuint32_t box[2] = {(cuuint32_t)(d.kind == 0 ? GEMM_BK + 4 : bm + 4), (cuuint32_t)(d.kind == 0 ? bm : GEMM_BK)};
-        const cuuint32_t estride[2] = {1, 1};
-        const CUresult r = encode((CUtensorMap*)&out[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)(base[d.space] + d.off), gdim, gstride, box,
-                                  estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                                  CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) {
-            set_error("dmrg_plan_create: cuTensorMapEncodeTiled failed (%d) for map %zu: space %u off %lld inner %d outer %d ld %d kind %d", (int)r, i,
-                      d.space, (long long)d.off, d.inner, d.outer, d.ld, d.kind);
+    // cuTensorMapEncodeTiled is a pure host function: the table (one map per operand matrix, ~1e6 at cfg 5) is
+    // encoded by all host threads
+    const unsigned nthr = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
+    std::vector<long long> bad(nthr, -1);
+    std::vector<int> bad_rc(nthr, 0);
+    int dev = 0;
+    DMRG_CUDA(cudaGetDevice(&dev));
+    auto work = [&](unsigned t) {
+        if (t > 0 && cudaSetDevice(dev) != cudaSuccess) { bad[t] = (long long)t; bad_rc[t] = -1; return; }   // the encoder wants a current context
+        for (size_t i = t; i < descs.size(); i += nthr) {
+            const MapDesc& d = descs[i];
+            const cuuint64_t gdim[2] = {(cuuint64_t)d.inner, (cuuint64_t)d.outer};
+            const cuuint64_t gstride[1] = {(cuuint64_t)d.ld * 8};
+            const cuuint32_t box[2] = {(cuuint32_t)d.box_inner, (cuuint32_t)d.box_outer};
+            const cuuint32_t estride[2] = {1, 1};
+            const CUresult r = encode((CUtensorMap*)&out[i], CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)(base[d.space] + d.off), gdim, gstride, box,
+                                      estride, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            if (r != CUDA_SUCCESS && bad[t] < 0) { bad[t] = (long long)i; bad_rc[t] = (int)r; }
+        }
+    };
+    std::vector<std::thread> pool;
+    for (unsigned t = 1; t < nthr; t++) pool.emplace_back(work, t);
+    work(0);
+    for (auto& th : pool) th.join();
+    for (unsigned t = 0; t < nthr; t++)
+        if (bad[t] >= 0) {
+            const MapDesc& d = descs[bad[t]];
+            set_error("dmrg_plan_create: cuTensorMapEncodeTiled failed (%d) for map %lld: space %u off %lld inner %d outer %d ld %d box %d x %d", bad_rc[t],
+                      bad[t], d.space, (long long)d.off, d.inner, d.outer, d.ld, d.box_inner, d.box_outer);
             return DMRG_ECUDA;
         }
-    }
     return DMRG_OK;
 }
 
@@ -375,6 +404,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         panel_rows[ir] += P->blocks[b].dl;
     }
     MapTable maps;
+    const int TILE = kVariants[0].bm;   // square tiles: the same box rules serve A and B operands
 
     auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
         PlanGroup grp{stage, (int)P->launches.size(), 0};
@@ -516,7 +546,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     const Run& Rc = runs[rblks[c].r0 + t];
                     int64_t rr = 0;
                     for (size_t q = Rc.i; q < Rc.j; q++) {
-                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx, xtop, (int32_t)rows, (int32_t)rr, (int32_t)col0s[c - c0]};
+                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx};
                         rr += P->blocks[req[q].in_blk].dl;
                     }
                     s1_flops += 2.0 * rows * dRi * req[Rc.i].dRo;
@@ -530,10 +560,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_KCONTIG;
                 {
                     const int64_t pf = panel_first[Bt.ir];
-                    s.a_map = maps.get(MS_PSI, ppad[pf], 0, dRi, panel_rows[Bt.ir], ldp);
-                    s.a_i0 = 0; s.a_o0 = (int32_t)((ppad[req[R0.i].in_blk] - ppad[pf]) / ldp);
-                    s.b_map = maps.get(MS_PACK, pack_top, 0, dRi, ncols, ldp);
-                    s.b_i0 = 0; s.b_o0 = 0;
+                    const BoxShape ba = box_shape(0, dRi, panel_rows[Bt.ir], TILE), bb = box_shape(0, dRi, ncols, TILE);
+                    s.a_map = maps.get(MS_PSI, ppad[pf], 0, dRi, panel_rows[Bt.ir], ldp, ba);
+                    s.a_o0 = (int32_t)((ppad[req[R0.i].in_blk] - ppad[pf]) / ldp);
+                    s.b_map = maps.get(MS_PACK, pack_top, 0, dRi, ncols, ldp, bb);
+                    s.a_pitch = (uint16_t)ba.inner; s.b_pitch = (uint16_t)bb.inner;
+                    s.a_bytes = 8u * ba.inner * ba.outer; s.b_bytes = 8u * bb.inner * bb.outer;
                 }
                 pack_segs.push_back(segs.size());
                 Job jb;
@@ -612,24 +644,30 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                 s.alpha = k.alpha;
                 s.K = k.dLi;
                 s.flags = 0;
-                s.a_map = s.b_map = 0; s.a_i0 = s.a_o0 = s.b_i0 = s.b_o0 = 0;
+                s.a_map = s.b_map = 0; s.a_o0 = 0; s.a_pitch = s.b_pitch = 0; s.a_bytes = s.b_bytes = 0;
+                auto set_a = [&](int32_t id, BoxShape b) { s.a_map = id; s.a_pitch = (uint16_t)b.inner; s.a_bytes = 8u * b.inner * b.outer; };
+                auto set_b = [&](int32_t id, BoxShape b) { s.b_map = id; s.b_pitch = (uint16_t)b.inner; s.b_bytes = 8u * b.inner * b.outer; };
                 if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
                 else {
                     s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
                     s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | (k.l_trans ? SEG_A_MCONTIG : 0);
-                    s.a_map = k.l_trans ? maps.get(MS_OPS, k.l_off, 1, k.dLo, k.dLi, s.lda) : maps.get(MS_OPS, k.l_off, 0, k.dLi, k.dLo, s.lda);
+                    const BoxShape ba = box_shape(k.l_trans ? 1 : 0, k.dLi, k.dLo, TILE);
+                    set_a(k.l_trans ? maps.get(MS_OPS, k.l_off, 1, k.dLo, k.dLi, s.lda, ba) : maps.get(MS_OPS, k.l_off, 0, k.dLi, k.dLo, s.lda, ba), ba);
                 }
                 if (k.r_off < 0) {
                     const dmrg_psi_block& IB = P->blocks[k.in_blk];
                     s.b_off = ppad[k.in_blk]; s.ldb = (int)round_up2(IB.dr);
                     s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT);
                     if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
-                    else s.b_map = maps.get(MS_PSI, ppad[k.in_blk], 1, IB.dr, IB.dl, s.ldb);
+                    else { const BoxShape bb = box_shape(1, k.dLi, IB.dr, TILE); set_b(maps.get(MS_PSI, ppad[k.in_blk], 1, IB.dr, IB.dl, s.ldb, bb), bb); }
                 } else {
                     const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
                     s.b_off = xl.off; s.ldb = xl.ld;
                     s.flags |= (SP_X << SEG_B_SPACE_SHIFT);
-                    if (!ident) { s.b_map = maps.get(MS_X, xl.job_off, 1, xl.ld, xl.job_rows, xl.ld); s.b_i0 = xl.c0; s.b_o0 = xl.r0; }
+                    if (!ident) {   // the X slice of this task as a matrix of its own: dLi rows x dRo columns, row pitch = the stage-1 job's
+                        const BoxShape bb = box_shape(1, k.dLi, k.dRo, TILE);
+                        set_b(maps.get(MS_X, xl.off, 1, k.dRo, k.dLi, xl.ld, bb), bb);
+                    }
                     alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
                 }
                 if (!ident) {
@@ -737,6 +775,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     // ---- upload ---------------------------------------------------------------------------------------
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
     P->stats[ST_XWS_ELEMS] = (double)P->xws_elems;
+    P->stats[ST_TENSOR_MAPS] = (double)maps.descs.size();
     P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
                                          hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +
                                          8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems);
