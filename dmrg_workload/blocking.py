@@ -265,6 +265,16 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
         new_secs.append(q)
         new_dims.append(k)
     nb = RBlock(labs_l + labs_r, new_secs, new_dims)
+    # the site tensor A of Eq. (8) as the renormalization step consumes it: one sub-block per
+    # (old-block sector, site state) -> new sector, rows of the kept isometry W (identity where nothing is rotated)
+    nb.site_tensor = []
+    for (il, ir), (a, off) in sorted(E.offset.items()):
+        if a not in remap:
+            continue
+        d = left.dims[il] * right.dims[ir]
+        Wa = np.eye(E.dims[a]) if W[a] is None else W[a]
+        i_old, n_site = (il, ir) if site_is_right else (ir, il)
+        nb.site_tensor.append((i_old, n_site, remap[a], np.ascontiguousarray(Wa[off:off + d, :])))
     for key, blocks in ops.items():
         out = {}
         for (a, b), m in blocks.items():
