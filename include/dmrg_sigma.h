@@ -220,6 +220,67 @@ int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_spac
                   void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * dmrg_renormalize: the renormalization step that follows the Davidson step at every bond (Eq. 8),
+ *     [O_new]_{r'r} = sum_{l'c'} sum_{lc} zeta A^{c'}_{l'r'} [O^blk]_{l'l} [O^site]_{c'c} A^{c}_{lr},
+ * for every operator the enlarged block carries, evaluated block by block as Eqs. (15)-(18)
+ * through the same grouped FP64 GEMM kernel as dmrg_sigma: Y = sum_terms (coef zeta o[c',c]) O^blk[L',L] A[(L c), R]
+ * (Eqs. 15-16, one multi-segment GEMM per bra sub-block), then O_new[R',R] = A[., R']^T Y[., R] (Eqs. 17-18, the sum
+ * over (L' C' L C) is the K-loop).  Deterministic, no atomics.
+ *   in       the store of the block being enlarged (operators of side `side`, incl. the LINCOMB "intermediates"
+ *            the terms use); borrowed, unchanged
+ *   side     0: enlarged basis |l>|c> (a left block growing to the right), 1: |c>|r> (a right block growing left)
+ *   new_sec  [host] sector table of the renormalized block
+ *   wblocks  [host] the site tensor A (Eq. 3): block w is the row-major dim_old[old_sector] x
+ *            dim_new[new_sector] matrix A[(l in old_sector, c = site_state), r in new_sector] at wvalues + offset;
+ *            (N, 2Sz) of old_sector + site_state must equal those of new_sector; at most one block per triple
+ *   wvalues  [host]
+ *   new_ops  [host] descriptors of the operators to build (side is overwritten by `side`; kind, p, q are labels;
+ *            dn, d2sz = the charge; first_block / nblocks ignored)
+ *   term_ptr, terms [host] CSR: new operator k = sum_{t in [term_ptr[k], term_ptr[k+1])} coef_t * O^blk_t (x) o_t with
+ *            O^blk_t = operator `op` of `in` (-1 = identity), every block transposed if trans != 0, and o_t =
+ *            site_ops[site_op]; every term must carry the charge of its operator (else DMRG_ECHARGE).
+ *            zeta is NOT part of coef: zeta = (-1)^{parity(second factor's operator) * N(ket of the first factor)},
+ *            first/second = (block, site) for side 0, (site, block) for side 1 (reading 3, two factors)
+ *   site_ops [host] nsite row-major 4x4 matrices, site_parity their fermion parities
+ *   options  NULL = defaults: workspace_bytes (0 = 4 GiB) bounds the Y intermediates (new operators are processed in
+ *            chunks), copy_mode as in dmrg_plan_options
+ *   out      a new store holding the side-`side` operators new_ops[0..n) over new_sec (a block is present iff some
+ *            term reaches it); owns its HBM, free with dmrg_ops_free
+ *   stats    [host, may be NULL]
+ * Enqueues on cuda_stream and synchronises it before returning.
+ */
+typedef struct { int32_t old_sector, site_state, new_sector, reserved; int64_t offset; } dmrg_wblock;
+typedef struct { double coef; int32_t op, trans, site_op, reserved; } dmrg_rterm;
+typedef struct { int64_t workspace_bytes; int32_t copy_mode; int32_t reserved[5]; } dmrg_renorm_options;
+typedef struct { double flops, device_ms; int64_t launches, jobs, tiles, out_values, workspace_values, tensor_maps; } dmrg_renorm_stats;
+int dmrg_renormalize(const dmrg_ops* in, int32_t side, const dmrg_sector* new_sec, int32_t n_new,
+                     const dmrg_wblock* wblocks, int64_t n_wblocks, const double* wvalues, int64_t n_wvalues,
+                     const dmrg_op_desc* new_ops, int32_t n_new_ops, const int64_t* term_ptr, const dmrg_rterm* terms,
+                     const double* site_ops, const int32_t* site_parity, int32_t nsite,
+                     const dmrg_renorm_options* options, void* cuda_stream, dmrg_ops** out, dmrg_renorm_stats* stats);
+
+/* Store utilities a sweep needs around the renormalization step.
+ * dmrg_ops_export: the store in the format dmrg_ops_load takes (unpadded row-major blocks): ops_out[num_ops] with
+ *   first_block / nblocks filled, blocks_out[num_blocks], values_out[num_values], all [host]; LINCOMB operators are
+ *   exported with the blocks they were formed into.  Synchronous.
+ * dmrg_ops_sectors: copies up to `capacity` sectors of `side` to out (may be NULL); returns the sector count.
+ * dmrg_ops_join: one two-sided store from a store with only side-0 operators and one with only side-1 operators
+ *   (e.g. two dmrg_renormalize outputs).  No copy: *out takes over the device memory of both, which are consumed
+ *   (freed as objects; do not use or free them afterwards).  Operator ids: left's, then right's shifted by
+ *   dmrg_ops_num_ops(left).
+ * dmrg_ops_add_lincombs: appends linear-combination operators O = sum_i coef_i ops[lin_op[i]] to a
+ *   device-resident store (summands: existing operators of the same side and charge; CSR as in dmrg_ops_load,
+ *   lin_ops[q].p = row of lin_ptr); the new operators get ids num_ops, num_ops + 1, ...  Synchronous. */
+int64_t dmrg_ops_num_ops(const dmrg_ops* ops);
+int64_t dmrg_ops_num_blocks(const dmrg_ops* ops);
+int64_t dmrg_ops_num_values(const dmrg_ops* ops);
+int     dmrg_ops_export(const dmrg_ops* ops, dmrg_op_desc* ops_out, dmrg_block_desc* blocks_out, double* values_out);
+int     dmrg_ops_sectors(const dmrg_ops* ops, int32_t side, dmrg_sector* out, int32_t capacity);
+int     dmrg_ops_join(dmrg_ops* left, dmrg_ops* right, dmrg_ops** out);
+int     dmrg_ops_add_lincombs(dmrg_ops* ops, const dmrg_op_desc* lin_ops, int32_t n_lin_ops,
+                              const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin);
+
+/* ---------------------------------------------------------------------------------------------
  * Per-stage device timing of the most recent dmrg_sigma with timing enabled (adds CUDA events
  * around each launch; off by default).  dmrg_plan_stage_ms synchronises and returns milliseconds:
  * which = 0 stage 1 (Eq. 11), 1 stage 2 + reduction (Eqs. 12-13), 2 whole call. */

@@ -28,6 +28,12 @@ PLANOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("min_s
                        ("reserved", "<i4", (8,))], align=True)
 assert PLANOPT_DT.itemsize == 72
 COPY_LDGSTS, COPY_TMA = 1, 2
+WBLOCK_DT = np.dtype([("old_sector", "<i4"), ("site_state", "<i4"), ("new_sector", "<i4"), ("reserved", "<i4"), ("offset", "<i8")], align=True)
+RTERM_DT = np.dtype([("coef", "<f8"), ("op", "<i4"), ("trans", "<i4"), ("site_op", "<i4"), ("reserved", "<i4")], align=True)
+RENORMOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("reserved", "<i4", (5,))], align=True)
+RENORMSTATS_DT = np.dtype([("flops", "<f8"), ("device_ms", "<f8"), ("launches", "<i8"), ("jobs", "<i8"), ("tiles", "<i8"),
+                           ("out_values", "<i8"), ("workspace_values", "<i8"), ("tensor_maps", "<i8")], align=True)
+assert WBLOCK_DT.itemsize == 24 and RTERM_DT.itemsize == 24 and RENORMOPT_DT.itemsize == 32 and RENORMSTATS_DT.itemsize == 64
 
 STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
              "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops",
@@ -36,7 +42,9 @@ STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_j
 EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_create_opts", "dmrg_plan_destroy",
            "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",
            "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
-           "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version")
+           "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
+           "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
+           "dmrg_ops_join", "dmrg_ops_add_lincombs")
 
 _lib = None
 
@@ -90,6 +98,19 @@ def lib():
         L.dmrg_plan_stage_ms.restype = f64
         L.dmrg_fp64_peak_tflops.argtypes = [i32, f64, vp]
         L.dmrg_fp64_peak_tflops.restype = f64
+        L.dmrg_renormalize.argtypes = [vp, i32, vp, i32, vp, i64, vp, i64, vp, i32, vp, vp, vp, vp, i32, vp, vp, C.POINTER(vp), vp]
+        L.dmrg_renormalize.restype = C.c_int
+        for name in ("dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values"):
+            getattr(L, name).argtypes = [vp]
+            getattr(L, name).restype = i64
+        L.dmrg_ops_export.argtypes = [vp, vp, vp, vp]
+        L.dmrg_ops_export.restype = C.c_int
+        L.dmrg_ops_sectors.argtypes = [vp, i32, vp, i32]
+        L.dmrg_ops_sectors.restype = C.c_int
+        L.dmrg_ops_join.argtypes = [vp, vp, C.POINTER(vp)]
+        L.dmrg_ops_join.restype = C.c_int
+        L.dmrg_ops_add_lincombs.argtypes = [vp, vp, i32, vp, vp, vp, i32]
+        L.dmrg_ops_add_lincombs.restype = C.c_int
         L.dmrg_last_error.restype = C.c_char_p
         L.dmrg_version.restype = C.c_char_p
         _lib = L
@@ -100,6 +121,12 @@ def _check(rc, allow=()):
     if rc != 0 and rc not in allow:
         raise DmrgError(rc, lib().dmrg_last_error().decode())
     return rc
+
+
+def _check_count(n):
+    if n < 0:
+        raise DmrgError(n, lib().dmrg_last_error().decode())
+    return int(n)
 
 
 def _ptr(a):
@@ -156,9 +183,55 @@ class OpsStore:
                                    _ptr(values), nvalues, on_dev, _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1, C.byref(h)))
         self._h = h
 
+    @classmethod
+    def _from_handle(cls, h):
+        self = cls.__new__(cls)
+        self._h = h
+        return self
+
     @property
     def device_bytes(self):
         return int(lib().dmrg_ops_device_bytes(self._h))
+
+    @property
+    def num_ops(self):
+        return int(lib().dmrg_ops_num_ops(self._h))
+
+    def sectors(self, side):
+        """int32 [n,3] (N, 2Sz, dim) of side 0 (L) / 1 (R)."""
+        n = _check_count(lib().dmrg_ops_sectors(self._h, int(side), None, 0))
+        out = np.zeros(n, dtype=SECTOR_DT)
+        _check_count(lib().dmrg_ops_sectors(self._h, int(side), _ptr(out), n))
+        return np.stack([out[k] for k in ("n", "two_sz", "dim")], axis=1).astype(np.int32).reshape(-1, 3)
+
+    def export(self):
+        """dmrg_ops_export: (ops int64 [nops,8], blocks int64 [nblk,3], values float64) in the dmrg_ops_load format."""
+        L = lib()
+        no, nb, nv = (int(f(self._h)) for f in (L.dmrg_ops_num_ops, L.dmrg_ops_num_blocks, L.dmrg_ops_num_values))
+        od, bd, vals = np.zeros(no, dtype=OP_DT), np.zeros(max(nb, 1), dtype=BLOCK_DT), np.zeros(max(nv, 1))
+        _check(L.dmrg_ops_export(self._h, _ptr(od), _ptr(bd), _ptr(vals)))
+        ops = np.stack([od[k].astype(np.int64) for k in ("side", "kind", "p", "q", "dn", "d2sz", "first_block", "nblocks")], axis=1)
+        blocks = np.stack([bd[k].astype(np.int64) for k in ("row_sector", "col_sector", "offset")], axis=1)[:nb]
+        return ops.reshape(-1, 8), blocks.reshape(-1, 3), vals[:nv]
+
+    def add_lincombs(self, lin_ops, lin_ptr, lin_op, lin_coef):
+        """dmrg_ops_add_lincombs; lin_ops int [n,8] rows as in `ops` (p = row of lin_ptr).  Returns the id of the first new operator."""
+        first = self.num_ops
+        od = _structured(np.asarray(lin_ops).reshape(-1, 8), OP_DT, (("side", 0), ("kind", 1), ("p", 2), ("q", 3), ("dn", 4), ("d2sz", 5),
+                                                                     ("first_block", 6), ("nblocks", 7)))
+        lp = np.ascontiguousarray(lin_ptr, dtype=np.int64)
+        lo = np.ascontiguousarray(lin_op, dtype=np.int32)
+        lc = np.ascontiguousarray(lin_coef, dtype=np.float64)
+        _check(lib().dmrg_ops_add_lincombs(self._h, _ptr(od), len(od), _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1))
+        return first
+
+    @staticmethod
+    def join(left, right):
+        """dmrg_ops_join: consumes both stores (their handles are cleared)."""
+        h = C.c_void_p()
+        _check(lib().dmrg_ops_join(left._h, right._h, C.byref(h)))
+        left._h = right._h = None
+        return OpsStore._from_handle(h)
 
     def free(self):
         if self._h is not None:
@@ -255,6 +328,32 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+def renormalize(store, side, sec_new, wblocks, wvalues, new_ops, term_ptr, term_coef, term_idx, site_ops, site_parity,
+                workspace_bytes=0, copy_mode=0, stream=None):
+    """dmrg_renormalize (Eq. 8 / Eqs. 15-18).  Array formats of dmrg_workload/renorm_terms.py: wblocks int [nw,4]
+    (old sector, site state, new sector, offset), term_idx int [nt,3] (op or -1, trans, site op).
+    Returns (OpsStore of the renormalized block, stats dict)."""
+    sn = _structured(np.asarray(sec_new).reshape(-1, 3), SECTOR_DT, (("n", 0), ("two_sz", 1), ("dim", 2)))
+    wb = _structured(np.asarray(wblocks).reshape(-1, 4), WBLOCK_DT, (("old_sector", 0), ("site_state", 1), ("new_sector", 2), ("offset", 3)))
+    wv = np.ascontiguousarray(wvalues, dtype=np.float64)
+    od = _structured(np.asarray(new_ops).reshape(-1, 8), OP_DT, (("side", 0), ("kind", 1), ("p", 2), ("q", 3), ("dn", 4), ("d2sz", 5),
+                                                                 ("first_block", 6), ("nblocks", 7)))
+    tp = np.ascontiguousarray(term_ptr, dtype=np.int64)
+    ti = np.asarray(term_idx).reshape(-1, 3)
+    td = np.zeros(len(ti), dtype=RTERM_DT)
+    td["coef"] = np.asarray(term_coef, dtype=np.float64)
+    td["op"], td["trans"], td["site_op"] = ti[:, 0], ti[:, 1], ti[:, 2]
+    so = np.ascontiguousarray(site_ops, dtype=np.float64).reshape(-1, 16)
+    sp = np.ascontiguousarray(site_parity, dtype=np.int32)
+    opt = np.zeros(1, dtype=RENORMOPT_DT)
+    opt["workspace_bytes"], opt["copy_mode"] = int(workspace_bytes), int(copy_mode)
+    st = np.zeros(1, dtype=RENORMSTATS_DT)
+    h = C.c_void_p()
+    _check(lib().dmrg_renormalize(store._h, int(side), _ptr(sn), len(sn), _ptr(wb), len(wb), _ptr(wv), len(wv), _ptr(od), len(od),
+                                  _ptr(tp), _ptr(td), _ptr(so), _ptr(sp), len(so), _ptr(opt), _stream_ptr(stream), C.byref(h), _ptr(st)))
+    return OpsStore._from_handle(h), {k: (float(st[k][0]) if st.dtype[k].kind == "f" else int(st[k][0])) for k in st.dtype.names}
 
 
 def fp64_peak_tflops(which, ms=200.0, stream=None):

@@ -122,7 +122,8 @@ struct dmrg_ops {
     // charge implies (or -1); all blocks are row-major with leading dimension round_up2(dim[col]).
     std::vector<std::vector<int64_t>> row_off;
     std::vector<std::vector<int32_t>> colsec;
-    double* d_values = nullptr;
+    double* d_values = nullptr;    // base of the store's address space: every block offset is relative to it
+    std::vector<double*> owned;    // device allocations the store owns (d_values first; joined / appended arrays after it)
     bool structure_only = false;   // loaded with values == NULL: planning / statistics only, no device memory
     int64_t nvalues_dev = 0;     // doubles allocated (stored + lincomb, padded)
     int64_t device_bytes = 0;

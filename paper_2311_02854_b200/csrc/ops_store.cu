@@ -66,7 +66,7 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
                          const double* values, int64_t nvalues, int32_t values_on_device,
                          const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin,
                          dmrg_ops* S) {
-    DMRG_REQUIRE(secL && secR && nsecL > 0 && nsecR > 0, "dmrg_ops_load: empty sector table");
+    DMRG_REQUIRE((secL || nsecL == 0) && (secR || nsecR == 0) && nsecL >= 0 && nsecR >= 0 && nsecL + nsecR > 0, "dmrg_ops_load: empty sector table");
     DMRG_REQUIRE(nops >= 0 && nblocks >= 0 && nvalues >= 0, "dmrg_ops_load: negative count");
     DMRG_REQUIRE(nops == 0 || ops, "dmrg_ops_load: ops is NULL");
     DMRG_REQUIRE(nblocks == 0 || blocks, "dmrg_ops_load: blocks is NULL");
@@ -76,8 +76,8 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
         int ndev = 0;
         DMRG_CUDA(cudaGetDeviceCount(&ndev));
     }
-    S->sec[0].assign(secL, secL + nsecL);
-    S->sec[1].assign(secR, secR + nsecR);
+    if (nsecL) S->sec[0].assign(secL, secL + nsecL);
+    if (nsecR) S->sec[1].assign(secR, secR + nsecR);
     for (int side = 0; side < 2; side++)
         for (auto& s : S->sec[side]) DMRG_REQUIRE(s.dim > 0, "dmrg_ops_load: sector with dim <= 0");
     S->ops.assign(ops, ops + nops);
@@ -151,6 +151,7 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
     S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
     if (S->structure_only) return DMRG_OK;
     DMRG_CUDA(cudaMalloc(&S->d_values, sizeof(double) * (size_t)std::max<int64_t>(top, 2)));
+    S->owned.push_back(S->d_values);
     S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
 
     // ---- repack stored blocks (row padding) -------------------------------------------------
@@ -254,7 +255,7 @@ int dmrg_ops_load(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* sec
 
 void dmrg_ops_free(dmrg_ops* ops) {
     if (!ops) return;
-    if (ops->d_values) cudaFree(ops->d_values);
+    for (double* p : ops->owned) cudaFree(p);
     delete ops;
 }
 
