@@ -49,10 +49,49 @@ def _store_key(op):
     return (k, op.p, op.q)
 
 
-def build_renorm_problem(blk, site_k, side, ints, outside_new, new_blk):
+class BlockShape:
+    """What a step needs to know about a block when its operator VALUES live elsewhere (on the device): labels,
+    sector table, and which operators it carries (RBlock keys)."""
+
+    def __init__(self, labels, sectors, dims, op_keys):
+        self.labels, self.sectors, self.dims, self.op_keys = list(labels), list(sectors), list(dims), list(op_keys)
+        self.site_tensor = None
+
+
+def carried_keys(labels, outside):
+    """RBlock keys of the operators a block over `labels` carries: a+_p, A_pq (p<q), B_pt (p<=t), S_p (p outside), H."""
+    X = sorted(labels)
+    keys = [("C", p) for p in X]
+    keys += [("A", p, q) for i, p in enumerate(X) for q in X[i + 1:]]
+    keys += [("B", p, t) for i, p in enumerate(X) for t in X[i:]]
+    keys += [("S", p) for p in outside]
+    keys.append(("H",))
+    return keys
+
+
+def compl_P_items(X, p, q, ints, side):
+    """P_pq = sum_{s<r in X} V[p,q,s,r] a_r a_s = sum V (A_sr)^T  (Eq. 22): [(BlockOp, coef, trans)]."""
+    X = sorted(X)
+    return [(BlockOp(side, "A", s, r), ints.V(p, q, s, r), 1) for i, s in enumerate(X) for r in X[i + 1:] if ints.V(p, q, s, r) != 0.0]
+
+
+def compl_Q_items(X, p, t, ints, side):
+    """Q_pt = sum_{q,r in X} V[p,q,t,r] a+_q a_r (Eq. 23), B_qr stored for q <= r: [(BlockOp, coef, trans)]."""
+    out = []
+    for q in sorted(X):
+        for r in sorted(X):
+            v = ints.V(p, q, t, r)
+            if v != 0.0:
+                out.append((BlockOp(side, "B", q, r), v, 0) if q <= r else (BlockOp(side, "B", r, q), v, 1))
+    return out
+
+
+def build_renorm_problem(blk, site_k, side, ints, outside_new, new_blk, structure_only=False):
     """blk: RBlock being enlarged by spatial orbital site_k; side 0: blk x site, 1: site x blk;
     outside_new: labels p for which the new block carries S_p; new_blk: the RBlock blocking.merge produced
-    (its sector table and site tensor are the projection this step applies)."""
+    (its sector table and site tensor are the projection this step applies).
+    structure_only: blk / new_blk are BlockShapes; no operator values are read and rp.blocks / rp.values stay empty
+    (the values live in a device store whose operators are matched by (kind, p, q))."""
     so = SiteOps(site_k, ints)
     s0, s1 = so.labels
     sname = "L" if side == 0 else "R"
@@ -61,7 +100,7 @@ def build_renorm_problem(blk, site_k, side, ints, outside_new, new_blk):
     rp.side = side
     # ---- old store: every carried operator of blk, then the linear combinations the terms need -------------
     stored = []
-    for key in blk.ops:
+    for key in (blk.op_keys if structure_only else blk.ops):
         kind = key[0]
         p = key[1] if len(key) > 1 else -1
         q = key[2] if len(key) > 2 else -1
@@ -73,7 +112,7 @@ def build_renorm_problem(blk, site_k, side, ints, outside_new, new_blk):
     for op in stored:
         dq = op_charge(op)
         first = len(blk_rows)
-        for (r, c), m in sorted(blk.ops[_store_key(op)].items()):
+        for (r, c), m in ([] if structure_only else sorted(blk.ops[_store_key(op)].items())):
             assert (blk.sectors[c][0] + dq[0], blk.sectors[c][1] + dq[1]) == blk.sectors[r]
             blk_rows.append((r, c, off))
             vals.append(np.ascontiguousarray(m, dtype=np.float64).ravel())

@@ -268,9 +268,15 @@ int dmrg_renormalize(const dmrg_ops* in, int32_t side, const dmrg_sector* new_se
  *   (e.g. two dmrg_renormalize outputs).  No copy: *out takes over the device memory of both, which are consumed
  *   (freed as objects; do not use or free them afterwards).  Operator ids: left's, then right's shifted by
  *   dmrg_ops_num_ops(left).
- * dmrg_ops_add_lincombs: appends linear-combination operators O = sum_i coef_i ops[lin_op[i]] to a
- *   device-resident store (summands: existing operators of the same side and charge; CSR as in dmrg_ops_load,
- *   lin_ops[q].p = row of lin_ptr); the new operators get ids num_ops, num_ops + 1, ...  Synchronous. */
+ * dmrg_ops_add_lincombs: appends linear-combination operators O = sum_i coef_i op_i to a
+ *   device-resident store; op_i = ops[lin_op[i]], or its transpose if lin_trans (may be NULL) has lin_trans[i] != 0
+ *   (summands: existing operators of the same side whose charge, negated for a transposed summand, is the new
+ *   operator's; CSR as in dmrg_ops_load, lin_ops[q].p = row of lin_ptr).  This is how the complementary operators
+ *   are formed from the normal ones, P_pq = sum V (A_sr)^T, Q_pt = sum V B_qr + sum V (B_rq)^T (Eqs. 22-23,
+ *   PAPER.md:135-137).  The new operators get ids num_ops, num_ops + 1, ...  Synchronous.
+ * dmrg_ops_derive: the same linear combinations formed into a NEW store over the same sector tables (operator ids
+ *   0 .. n_lin_ops-1, kinds as given); `src` is unchanged and can be freed afterwards -- e.g. keep {a+, S, H, P, Q}
+ *   of a right block and drop its O(K^2) A and B operators. */
 int64_t dmrg_ops_num_ops(const dmrg_ops* ops);
 int64_t dmrg_ops_num_blocks(const dmrg_ops* ops);
 int64_t dmrg_ops_num_values(const dmrg_ops* ops);
@@ -278,7 +284,11 @@ int     dmrg_ops_export(const dmrg_ops* ops, dmrg_op_desc* ops_out, dmrg_block_d
 int     dmrg_ops_sectors(const dmrg_ops* ops, int32_t side, dmrg_sector* out, int32_t capacity);
 int     dmrg_ops_join(dmrg_ops* left, dmrg_ops* right, dmrg_ops** out);
 int     dmrg_ops_add_lincombs(dmrg_ops* ops, const dmrg_op_desc* lin_ops, int32_t n_lin_ops,
-                              const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin);
+                              const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef,
+                              const int32_t* lin_trans, int32_t nlin);
+int     dmrg_ops_derive(const dmrg_ops* src, const dmrg_op_desc* lin_ops, int32_t n_lin_ops,
+                        const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef,
+                        const int32_t* lin_trans, int32_t nlin, dmrg_ops** out);
 
 /* ---------------------------------------------------------------------------------------------
  * Per-stage device timing of the most recent dmrg_sigma with timing enabled (adds CUDA events

@@ -44,7 +44,7 @@ EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan
            "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
            "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
-           "dmrg_ops_join", "dmrg_ops_add_lincombs")
+           "dmrg_ops_join", "dmrg_ops_add_lincombs", "dmrg_ops_derive")
 
 _lib = None
 
@@ -109,8 +109,10 @@ def lib():
         L.dmrg_ops_sectors.restype = C.c_int
         L.dmrg_ops_join.argtypes = [vp, vp, C.POINTER(vp)]
         L.dmrg_ops_join.restype = C.c_int
-        L.dmrg_ops_add_lincombs.argtypes = [vp, vp, i32, vp, vp, vp, i32]
+        L.dmrg_ops_add_lincombs.argtypes = [vp, vp, i32, vp, vp, vp, vp, i32]
         L.dmrg_ops_add_lincombs.restype = C.c_int
+        L.dmrg_ops_derive.argtypes = [vp, vp, i32, vp, vp, vp, vp, i32, C.POINTER(vp)]
+        L.dmrg_ops_derive.restype = C.c_int
         L.dmrg_last_error.restype = C.c_char_p
         L.dmrg_version.restype = C.c_char_p
         _lib = L
@@ -214,16 +216,30 @@ class OpsStore:
         blocks = np.stack([bd[k].astype(np.int64) for k in ("row_sector", "col_sector", "offset")], axis=1)[:nb]
         return ops.reshape(-1, 8), blocks.reshape(-1, 3), vals[:nv]
 
-    def add_lincombs(self, lin_ops, lin_ptr, lin_op, lin_coef):
-        """dmrg_ops_add_lincombs; lin_ops int [n,8] rows as in `ops` (p = row of lin_ptr).  Returns the id of the first new operator."""
-        first = self.num_ops
+    @staticmethod
+    def _lin_args(lin_ops, lin_ptr, lin_op, lin_coef, lin_trans):
         od = _structured(np.asarray(lin_ops).reshape(-1, 8), OP_DT, (("side", 0), ("kind", 1), ("p", 2), ("q", 3), ("dn", 4), ("d2sz", 5),
                                                                      ("first_block", 6), ("nblocks", 7)))
         lp = np.ascontiguousarray(lin_ptr, dtype=np.int64)
         lo = np.ascontiguousarray(lin_op, dtype=np.int32)
         lc = np.ascontiguousarray(lin_coef, dtype=np.float64)
-        _check(lib().dmrg_ops_add_lincombs(self._h, _ptr(od), len(od), _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1))
+        lt = None if lin_trans is None else np.ascontiguousarray(lin_trans, dtype=np.int32)
+        assert len(lo) == len(lc) == int(lp[-1]) and (lt is None or len(lt) == len(lo))
+        return od, lp, lo, lc, lt
+
+    def add_lincombs(self, lin_ops, lin_ptr, lin_op, lin_coef, lin_trans=None):
+        """dmrg_ops_add_lincombs; lin_ops int [n,8] rows as in `ops` (p = row of lin_ptr).  Returns the id of the first new operator."""
+        first = self.num_ops
+        od, lp, lo, lc, lt = self._lin_args(lin_ops, lin_ptr, lin_op, lin_coef, lin_trans)
+        _check(lib().dmrg_ops_add_lincombs(self._h, _ptr(od), len(od), _ptr(lp), _ptr(lo), _ptr(lc), _ptr(lt), len(lp) - 1))
         return first
+
+    def derive(self, lin_ops, lin_ptr, lin_op, lin_coef, lin_trans=None):
+        """dmrg_ops_derive: a new store whose operators are the given linear combinations of this store's operators."""
+        od, lp, lo, lc, lt = self._lin_args(lin_ops, lin_ptr, lin_op, lin_coef, lin_trans)
+        h = C.c_void_p()
+        _check(lib().dmrg_ops_derive(self._h, _ptr(od), len(od), _ptr(lp), _ptr(lo), _ptr(lc), _ptr(lt), len(lp) - 1, C.byref(h)))
+        return OpsStore._from_handle(h)
 
     @staticmethod
     def join(left, right):

@@ -29,17 +29,22 @@ __global__ void __launch_bounds__(256) unpack_kernel(const UnpackDesc* __restric
     }
 }
 
-struct LinDesc2 { int64_t dst; int64_t n; int32_t sum_begin, sum_end; };
-struct LinSummand2 { int64_t src; double coef; };
-// the same arithmetic as ops_store.cu's lincomb_kernel (summand order = caller's order), for lincombs appended later
+struct LinDesc2 { int64_t dst; int32_t rows, cols, ld, pad_; int32_t sum_begin, sum_end; };   // dst block: rows x cols, row pitch ld
+struct LinSummand2 { int64_t src; double coef; int32_t present, trans, ld_src, pad_; };   // trans: the summand's block is used transposed
+// dst[i][j] = sum_s coef_s * (trans_s ? src_s[j][i] : src_s[i][j])  in summand order (deterministic); row pads are written as zeros.
+// The same arithmetic as ops_store.cu's lincomb_kernel, plus transposed summands (P_pq = sum V (A_sr)^T, Q_pt = sum V B_qr + sum V (B_rq)^T:
+// the complementary operators from the normal ones, SURVEY.md section 8.0 identity I5).      grid (chunks, blocks)
 __global__ void __launch_bounds__(256) lincomb2_kernel(const LinDesc2* __restrict__ desc, const LinSummand2* __restrict__ sums, double* __restrict__ vals) {
     const LinDesc2 d = desc[blockIdx.y];
-    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < d.n; e += (int64_t)gridDim.x * blockDim.x) {
+    const int64_t n = (int64_t)d.rows * d.ld;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / d.ld), j = (int)(e - (int64_t)i * d.ld);
         double acc = 0.0;
-        for (int i = d.sum_begin; i < d.sum_end; i++) {
-            const LinSummand2 s = sums[i];
-            if (s.src >= 0) acc = fma(s.coef, vals[s.src + e], acc);
-        }
+        if (j < d.cols)
+            for (int q = d.sum_begin; q < d.sum_end; q++) {
+                const LinSummand2 s = sums[q];
+                if (s.present) acc = fma(s.coef, s.trans ? vals[s.src + (int64_t)j * s.ld_src + i] : vals[s.src + (int64_t)i * s.ld_src + j], acc);
+            }
         vals[d.dst + e] = acc;
     }
 }
@@ -469,54 +474,58 @@ int dmrg_ops_join(dmrg_ops* left, dmrg_ops* right, dmrg_ops** out) {
     return DMRG_OK;
 }
 
-int dmrg_ops_add_lincombs(dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
-                          const double* lin_coef, int32_t nlin) {
-    if (!S || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_add_lincombs: NULL or empty argument"); return DMRG_EINVAL; }
-    if (S->structure_only || S->owned.empty()) { set_error("dmrg_ops_add_lincombs: the store holds no device values"); return DMRG_EINVAL; }
+// Shared core of dmrg_ops_add_lincombs / dmrg_ops_derive: forms the blocks of `n_lin_ops` linear combinations of operators of `S`
+// in a fresh device allocation (*d_new_out) and returns their tables with offsets relative to that allocation.
+static int form_lincombs(const dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
+                         const double* lin_coef, const int32_t* lin_trans, int32_t nlin, const char* who, double** d_new_out, int64_t* top_out,
+                         std::vector<std::vector<int64_t>>& new_off, std::vector<std::vector<int32_t>>& new_colsec) {
     const int nops0 = (int)S->ops.size();
     std::vector<LinDesc2> lind;
     std::vector<LinSummand2> lins;
-    struct LinSrc { int32_t op, row; };   // summand offsets are resolved after the (possible) rebase
-    std::vector<LinSrc> lsrc;
-    std::vector<std::vector<int64_t>> new_off;
-    std::vector<std::vector<int32_t>> new_colsec;
     int64_t top = 0;
     for (int q = 0; q < n_lin_ops; q++) {
         const dmrg_op_desc& d = lin_ops[q];
-        DMRG_REQUIRE((d.side == 0 || d.side == 1) && d.p >= 0 && d.p < nlin, "dmrg_ops_add_lincombs: op %d: bad side or lin_ptr row", q);
+        DMRG_REQUIRE((d.side == 0 || d.side == 1) && d.p >= 0 && d.p < nlin, "%s: op %d: bad side or lin_ptr row", who, q);
         const auto& sec = S->sec[d.side];
         const int ns = (int)sec.size();
         const int64_t i0 = lin_ptr[d.p], i1 = lin_ptr[d.p + 1];
-        DMRG_REQUIRE(i0 <= i1, "dmrg_ops_add_lincombs: lin_ptr not monotone");
+        DMRG_REQUIRE(i0 <= i1, "%s: lin_ptr not monotone", who);
         for (int64_t i = i0; i < i1; i++) {
             const int s = lin_op[i];
-            DMRG_REQUIRE(s >= 0 && s < nops0 && S->ops[s].side == d.side && S->ops[s].dn == d.dn && S->ops[s].d2sz == d.d2sz,
-                         "dmrg_ops_add_lincombs: op %d: summand %d is not an operator of the same side and charge", q, s);
+            const int sg = (lin_trans && lin_trans[i]) ? -1 : 1;
+            DMRG_REQUIRE(s >= 0 && s < nops0 && S->ops[s].side == d.side && sg * S->ops[s].dn == d.dn && sg * S->ops[s].d2sz == d.d2sz,
+                         "%s: op %d: summand %d is not an operator of the same side and (signed) charge", who, q, s);
         }
         std::vector<int64_t> ro(ns, -1);
         std::vector<int32_t> cs(ns, -1);
         for (int r = 0; r < ns; r++) {
-            cs[r] = find_sec(sec, sec[r].n - d.dn, sec[r].two_sz - d.d2sz);
-            if (cs[r] < 0) continue;
+            const int c = cs[r] = find_sec(sec, sec[r].n - d.dn, sec[r].two_sz - d.d2sz);
+            if (c < 0) continue;
+            // summand block feeding dst block (r, c): normal: the summand's block in row sector r; transposed: its block in row sector c
+            // (whose column sector is then r)
+            auto src_of = [&](int64_t i) -> int64_t { return (lin_trans && lin_trans[i]) ? S->row_off[lin_op[i]][c] : S->row_off[lin_op[i]][r]; };
             bool any = false;
-            for (int64_t i = i0; i < i1; i++) any = any || S->row_off[lin_op[i]][r] >= 0;
+            for (int64_t i = i0; i < i1; i++) any = any || src_of(i) >= 0;
             if (!any) continue;
-            const int64_t n = (int64_t)sec[r].dim * round_up2(sec[cs[r]].dim);
-            LinDesc2 ld{top, n, (int32_t)lins.size(), 0};
-            for (int64_t i = i0; i < i1; i++) { lins.push_back({-1, lin_coef[i]}); lsrc.push_back({lin_op[i], r}); }
-            ld.sum_end = (int32_t)lins.size();
-            lind.push_back(ld);
+            const int ld = (int)round_up2(sec[c].dim);
+            LinDesc2 ld2{top, sec[r].dim, sec[c].dim, ld, 0, (int32_t)lins.size(), 0};
+            for (int64_t i = i0; i < i1; i++) {
+                const int64_t so = src_of(i);
+                const int tr = (lin_trans && lin_trans[i]) ? 1 : 0;
+                lins.push_back({so >= 0 ? so : 0, lin_coef[i], so >= 0 ? 1 : 0, tr, (int32_t)round_up2(tr ? sec[r].dim : sec[c].dim), 0});
+            }
+            ld2.sum_end = (int32_t)lins.size();
+            lind.push_back(ld2);
             ro[r] = top;
-            top += n;
+            top += (int64_t)sec[r].dim * ld;
         }
-        new_off.push_back(std::move(ro)); new_colsec.push_back(std::move(cs));
+        new_off.push_back(std::move(ro));
+        new_colsec.push_back(std::move(cs));
     }
     double* d_new = nullptr;
     DMRG_CUDA(cudaMalloc(&d_new, sizeof(double) * (size_t)std::max<int64_t>(top, 2)));
-    if (d_new < S->d_values) rebase(S, d_new);   // keep every offset of the store >= 0 (< 0 means "absent" / "identity")
-    const int64_t delta = (int64_t)(d_new - S->d_values);
+    const int64_t delta = (int64_t)(d_new - S->d_values);   // the kernel addresses everything relative to S->d_values (signed offsets)
     for (auto& l : lind) l.dst += delta;
-    for (size_t i = 0; i < lins.size(); i++) lins[i].src = S->row_off[lsrc[i].op][lsrc[i].row];   // -1 where the summand has no block
     int rc = DMRG_OK;
     if (!lind.empty()) {
         LinDesc2* d_lind = nullptr;
@@ -533,20 +542,70 @@ int dmrg_ops_add_lincombs(dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_li
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
         cudaFree(d_lind);
         cudaFree(d_lins);
-        if (e != cudaSuccess) { set_error("dmrg_ops_add_lincombs: %s", cudaGetErrorString(e)); rc = DMRG_ECUDA; }
+        if (e != cudaSuccess) { set_error("%s: %s", who, cudaGetErrorString(e)); rc = DMRG_ECUDA; }
     }
     if (rc != DMRG_OK) { cudaFree(d_new); return rc; }
+    *d_new_out = d_new;
+    *top_out = top;
+    return DMRG_OK;
+}
+
+int dmrg_ops_add_lincombs(dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
+                          const double* lin_coef, const int32_t* lin_trans, int32_t nlin) {
+    if (!S || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_add_lincombs: NULL or empty argument"); return DMRG_EINVAL; }
+    if (S->structure_only || S->owned.empty()) { set_error("dmrg_ops_add_lincombs: the store holds no device values"); return DMRG_EINVAL; }
+    std::vector<std::vector<int64_t>> new_off;
+    std::vector<std::vector<int32_t>> new_colsec;
+    double* d_new = nullptr;
+    int64_t top = 0;
+    int rc;
+    try {
+        rc = form_lincombs(S, lin_ops, n_lin_ops, lin_ptr, lin_op, lin_coef, lin_trans, nlin, "dmrg_ops_add_lincombs", &d_new, &top, new_off, new_colsec);
+    } catch (const std::bad_alloc&) { set_error("dmrg_ops_add_lincombs: out of host memory"); rc = DMRG_ENOMEM; }
+    if (rc != DMRG_OK) return rc;
+    if (d_new < S->d_values) rebase(S, d_new);   // keep every offset of the store >= 0 (< 0 means "absent" / "identity")
+    const int64_t delta = (int64_t)(d_new - S->d_values);
     S->owned.push_back(d_new);
     for (int q = 0; q < n_lin_ops; q++) {
         dmrg_op_desc d = lin_ops[q];
         d.kind = DMRG_OP_LINCOMB; d.first_block = 0; d.nblocks = 0;
         S->ops.push_back(d);
-        for (size_t r = 0; r < new_off[q].size(); r++) if (new_off[q][r] >= 0) new_off[q][r] += delta;
+        for (auto& o : new_off[q]) if (o >= 0) o += delta;
         S->row_off.push_back(std::move(new_off[q]));
         S->colsec.push_back(std::move(new_colsec[q]));
     }
     S->nvalues_dev += top;
     S->device_bytes += sizeof(double) * (size_t)std::max<int64_t>(top, 2);
+    return DMRG_OK;
+}
+
+int dmrg_ops_derive(const dmrg_ops* src, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
+                    const double* lin_coef, const int32_t* lin_trans, int32_t nlin, dmrg_ops** out) {
+    if (!out) { set_error("dmrg_ops_derive: out is NULL"); return DMRG_EINVAL; }
+    *out = nullptr;
+    if (!src || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_derive: NULL or empty argument"); return DMRG_EINVAL; }
+    if (src->structure_only || src->owned.empty()) { set_error("dmrg_ops_derive: the source store holds no device values"); return DMRG_EINVAL; }
+    dmrg_ops* D = new (std::nothrow) dmrg_ops();
+    if (!D) { set_error("dmrg_ops_derive: out of host memory"); return DMRG_ENOMEM; }
+    double* d_new = nullptr;
+    int64_t top = 0;
+    int rc;
+    try {
+        rc = form_lincombs(src, lin_ops, n_lin_ops, lin_ptr, lin_op, lin_coef, lin_trans, nlin, "dmrg_ops_derive", &d_new, &top, D->row_off, D->colsec);
+    } catch (const std::bad_alloc&) { set_error("dmrg_ops_derive: out of host memory"); rc = DMRG_ENOMEM; }
+    if (rc != DMRG_OK) { delete D; return rc; }
+    D->sec[0] = src->sec[0];
+    D->sec[1] = src->sec[1];
+    for (int q = 0; q < n_lin_ops; q++) {
+        dmrg_op_desc d = lin_ops[q];
+        d.first_block = 0; d.nblocks = 0;
+        D->ops.push_back(d);   // kind, p, q as the caller labels them: in the new store these are stored operators
+    }
+    D->d_values = d_new;
+    D->owned.push_back(d_new);
+    D->nvalues_dev = top;
+    D->device_bytes = sizeof(double) * (size_t)std::max<int64_t>(top, 2);
+    *out = D;
     return DMRG_OK;
 }
 

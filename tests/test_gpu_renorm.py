@@ -165,3 +165,58 @@ def test_cfg2_size_step():
     assert np.array_equal(outs[0][0].sectors(0), pr.secL) and np.array_equal(outs[1][0].sectors(1), pr.secR)
     for o, _ in outs.values():
         o.free()
+
+
+def _cpu_chain_problem(K, nL, N, D, seed, force_dmax=False):
+    """The CPU-blocked problem (dmrg_workload.blocking, as make_blocked_problem builds it) together with the site
+    tensor of every step, so that the device chain can be driven through exactly the same projections."""
+    from dmrg_workload import blocking
+    from dmrg_workload.store import assemble, block_values_from_rblocks, sectors_of
+    from dmrg_workload.terms import Partition, TermTable
+    ints = make_integrals(K, seed)
+    rng = np.random.Generator(np.random.Philox(seed + 7919))
+    tensors, blocks = {}, {}
+    for side, sites in ((0, list(range(0, nL))), (1, list(range(nL + 2, K)))):
+        order = sites if side == 0 else sites[::-1]
+        inside, blk = [], None
+        for k in order:
+            inside.append(k)
+            outside = [P for P in range(2 * K) if (P >> 1) not in inside]
+            site = blocking.site_block(k, ints, [P for P in range(2 * K) if (P >> 1) != k])
+            if blk is None:
+                blk = site
+                continue
+            args = (blk, site) if side == 0 else (site, blk)
+            blk = blocking.merge(*args, ints, outside, K, N, 0, D, rng, False, force_dmax, site_side="right" if side == 0 else "left")
+            tensors[(side, k)] = (blk.sectors, blk.dims, blk.site_tensor)
+        blocks[side] = blk
+    tt = TermTable(Partition(K, nL), ints)
+    pr = assemble(tt, sectors_of(blocks[0]), sectors_of(blocks[1]), block_values_from_rblocks(blocks[0], blocks[1], ints), N, 0)
+    return ints, pr, tensors
+
+
+@pytest.mark.parametrize("K,nL,N,D,seed", [(8, 3, 8, 14, 31), (10, 4, 10, 40, 32), (12, 5, 12, 90, 33)])
+def test_device_built_bond_gives_the_oracle_sigma(K, nL, N, D, seed):
+    """End to end: both blocks grown on the device by chained dmrg_renormalize calls (the operators never leave HBM),
+    complementary operators formed on the device, stores joined -- dmrg_sigma on that store equals the oracle's
+    sigma on the CPU-blocked problem built through the same site tensors."""
+    g = _gpu()
+    import oracle
+    from dmrg_workload.problem import random_psi
+    from paper_2311_02854_b200 import bondgen
+    ints, pr, tensors = _cpu_chain_problem(K, nL, N, D, seed)
+    bond = bondgen.build_bond(g, K, nL, N, 0, D, ints, seed, tensor_provider=lambda side, k: tensors[(side, k)],
+                              stream=torch.cuda.current_stream())
+    assert np.array_equal(bond.secL, pr.secL) and np.array_equal(bond.secR, pr.secR) and np.array_equal(bond.layout, pr.layout)
+    plan = g.Plan(bond.ops, bond.term_coef, bond.term_idx, bond.site_ops, bond.site_parity, N, 0)
+    assert np.array_equal(plan.psi_layout(), pr.layout)
+    for s in (5, 6):
+        psi = random_psi(pr.psi_size, s)
+        d = torch.from_numpy(psi).cuda()
+        o = torch.empty_like(d)
+        plan.sigma(d, o, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ref = oracle.opair_sigma(pr, psi)
+        assert np.abs(o.cpu().numpy() - ref).max() / np.linalg.norm(ref) <= 1e-10
+    plan.destroy()
+    bond.ops.free()
