@@ -53,8 +53,13 @@ def parse():
     ap.add_argument("--sigma-only", type=int, default=0, metavar="N",
                     help="profiling mode: no Davidson, no oracle; N plain dmrg_sigma calls (after one warm-up call) and a short "
                          "JSON line with the per-stage device times -- the command the ncu captures under profiles/ wrap")
-    ap.add_argument("--operators", default="default", choices=["default", "direct", "renorm"],
-                    help="cfg3-5 operator values: direct fill (seeded random blocks) or GPU renormalization (NEXT-1)")
+    ap.add_argument("--operators", default="default", choices=["default", "renorm"],
+                    help="default: the config's generator (CPU blocking for cfg1-2, direct fill for cfg3-5); renorm: both blocks "
+                         "grown ON THE DEVICE by chained dmrg_renormalize calls with seeded random site tensors (physical operators; "
+                         "the oracle legs are skipped: oracle inputs must not come from the CUDA path)")
+    ap.add_argument("--davidson-to", type=float, default=0.0, metavar="TOL",
+                    help="after the timed steps, run the Davidson from the reading-12 guess (unit vector at argmin Hd + 1e-3 noise) "
+                         "to this residual and report iterations and wall time (BASELINE.json configs[2])")
     return ap.parse_args()
 
 
@@ -227,12 +232,29 @@ def main():
     stream = torch.cuda.current_stream()
 
     t0 = time.perf_counter()
-    pr = make_config(args.config)
-    t_gen = time.perf_counter() - t0
-    free0, _ = torch.cuda.mem_get_info()
-    t0 = time.perf_counter()
-    ops = g.OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks, pr.values, pr.lin_ptr, pr.lin_op, pr.lin_coef)
-    t_load = time.perf_counter() - t0
+    renorm_info = None
+    if args.operators == "renorm":
+        from dmrg_workload.integrals import make_integrals
+        from dmrg_workload.problem import CONFIGS
+        from paper_2311_02854_b200 import bondgen
+        c = CONFIGS[args.config]
+        ints = make_integrals(c["K"], c["seed"], banded=c.get("banded", False))
+        pr = bondgen.build_bond(g, c["K"], c["nL"], c["N_tot"], 0, c["D"], ints, c["seed"], stream=stream,
+                                log=(lambda m: print(m, file=sys.stderr)) if rank == 0 else None)
+        pr.meta["banded"] = c.get("banded", False)
+        ops = pr.ops
+        t_gen, t_load = pr.seconds["total"], 0.0
+        rs = pr.renorm_stats
+        big = [r for r in rs if r["dim"] >= 0.9 * max(x["dim"] for x in rs)]
+        renorm_info = {"steps": len(rs), "flops": sum(r["flops"] for r in rs), "device_ms": sum(r["device_ms"] for r in rs),
+                       "tflops_full_size_steps": sum(r["flops"] for r in big) / max(1e-9, sum(r["device_ms"] for r in big)) * 1e-9,
+                       "seconds_total": pr.seconds["total"], "seconds_chains": pr.seconds["chains"]}
+    else:
+        pr = make_config(args.config)
+        t_gen = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        ops = g.OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks, pr.values, pr.lin_ptr, pr.lin_op, pr.lin_coef)
+        t_load = time.perf_counter() - t0
     free1, _ = torch.cuda.mem_get_info()
     ws = int(args.workspace_gib * 2 ** 30) if args.workspace_gib > 0 else int(min(24 * 2 ** 30, 0.25 * free1))
     t0 = time.perf_counter()
@@ -347,7 +369,20 @@ def main():
     # ---- CPU oracle beside it (rank 0, N = 1 only) ---------------------------------------------------
     cpu = None
     parity = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    dav_to = None
+    if args.davidson_to > 0:
+        hd = torch.empty_like(x)
+        plan.hdiag(hd, stream)
+        torch.cuda.synchronize()
+        guess = torch.from_numpy(1e-3 * random_psi(n, 7)).cuda()
+        guess[int(torch.argmin(hd))] += 1.0
+        t0 = time.perf_counter()
+        r2 = plan.davidson(guess, max_iter=300, max_space=30, tol=args.davidson_to, stream=stream)
+        torch.cuda.synchronize()
+        dav_to = {"tol": args.davidson_to, "iters": r2["iters"], "converged": r2["converged"], "seconds": time.perf_counter() - t0,
+                  "energy": r2["energy"], "resid": r2["resid"], "guess": "unit vector at argmin Hd + 1e-3 seeded noise (DESIGN.md reading 12)",
+                  "max_space": 30}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and args.operators != "renorm":
         cpu = oracle_term_sample(pr, psi_h, flops_canon, args.cpu_seconds)
         # parity on sampled sigma blocks (all terms), in the launch configuration that was timed; the oracle's
         # fixed cost (full term expansion, all intermediates) dominates this call, so it is not the cpu_baseline
@@ -379,6 +414,7 @@ def main():
                                  "davidson_vectors": (2 * max(W, K) + 3) * 8 * n / 1e9},
                 "setup_s": {"generate": t_gen, "ops_load": t_load, "plan": t_plan},
                 "davidson": {"iters": res["iters"], "theta_last": res["energy"], "resid_last": res["resid"]},
+                "davidson_to_tol": dav_to, "renormalization": renorm_info,
                 "context": "paper: ~13-15 TFLOP/s FP64-TC per A100 for the GEMM step at large D (PAPER.md:231); D=14000 on 48 A100-80GB (PAPER.md:17)"}
         print(json.dumps(line))
     plan.destroy()

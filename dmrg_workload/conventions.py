@@ -52,6 +52,28 @@ class SpinOrbitalIntegrals:
             v -= self.eri[p, s, q, r]
         return float(v)
 
+    def V_pq(self, P, Q):
+        """V[P, Q, :, :] as a (2K x 2K) array over (R, S) -- the same numbers as V(), one slice at a time."""
+        K = self.K
+        p, q, oP, oQ = P >> 1, Q >> 1, P & 1, Q & 1
+        e = self.eri[p, :, q, :]                 # e[r, s] = (pr|qs)
+        out = np.zeros((2 * K, 2 * K))
+        out[oP::2, oQ::2] += e                   # <PQ|RS>: spin(R) = spin(P), spin(S) = spin(Q)
+        out[oQ::2, oP::2] -= e.T                 # <PQ|SR>: spin(S) = spin(P), spin(R) = spin(Q); (ps|qr) = e[s, r]
+        return out
+
+    def V_pt(self, P, T):
+        """V[P, :, T, :] as a (2K x 2K) array over (Q, R)."""
+        K = self.K
+        p, t, oP, oT = P >> 1, T >> 1, P & 1, T & 1
+        out = np.zeros((2 * K, 2 * K))
+        if oP == oT:                             # <PQ|TR> = (pt|qr) d(sP,sT) d(sQ,sR)
+            e = self.eri[p, t, :, :]
+            out[0::2, 0::2] += e
+            out[1::2, 1::2] += e
+        out[oT::2, oP::2] -= self.eri[p, :, :, t].T   # <PQ|RT> = (pr|qt) d(sP,sR) d(sQ,sT); [q, r] = eri[p, r, q, t]
+        return out
+
     def dense_h(self):
         n = 2 * self.K
         out = np.zeros((n, n))

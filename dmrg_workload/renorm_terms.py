@@ -72,15 +72,17 @@ def carried_keys(labels, outside):
 def compl_P_items(X, p, q, ints, side):
     """P_pq = sum_{s<r in X} V[p,q,s,r] a_r a_s = sum V (A_sr)^T  (Eq. 22): [(BlockOp, coef, trans)]."""
     X = sorted(X)
-    return [(BlockOp(side, "A", s, r), ints.V(p, q, s, r), 1) for i, s in enumerate(X) for r in X[i + 1:] if ints.V(p, q, s, r) != 0.0]
+    v = ints.V_pq(p, q)
+    return [(BlockOp(side, "A", s, r), float(v[s, r]), 1) for i, s in enumerate(X) for r in X[i + 1:] if v[s, r] != 0.0]
 
 
 def compl_Q_items(X, p, t, ints, side):
     """Q_pt = sum_{q,r in X} V[p,q,t,r] a+_q a_r (Eq. 23), B_qr stored for q <= r: [(BlockOp, coef, trans)]."""
     out = []
+    vm = ints.V_pt(p, t)
     for q in sorted(X):
         for r in sorted(X):
-            v = ints.V(p, q, t, r)
+            v = float(vm[q, r])
             if v != 0.0:
                 out.append((BlockOp(side, "B", q, r), v, 0) if q <= r else (BlockOp(side, "B", r, q), v, 1))
     return out
@@ -136,12 +138,14 @@ def build_renorm_problem(blk, site_k, side, ints, outside_new, new_blk, structur
         return lin_index[items]
 
     def LP(p, q):   # sum_{s<r in blk} V[p,q,s,r] A_sr   (P_pq = LP^T)
-        items = [(BlockOp(sname, "A", s, r), ints.V(p, q, s, r)) for i, s in enumerate(X) for r in X[i + 1:]]
+        v = ints.V_pq(p, q)
+        items = [(BlockOp(sname, "A", s, r), float(v[s, r])) for i, s in enumerate(X) for r in X[i + 1:]]
         return lincomb(items, (2, -(-spin_of(p) - spin_of(q))))
 
     def LQ(p, t):   # (LQ1, LQ2): Q_pt = LQ1 + LQ2^T
-        i1 = [(BlockOp(sname, "B", q, r), ints.V(p, q, t, r)) for q in X for r in X if q <= r]
-        i2 = [(BlockOp(sname, "B", r, q), ints.V(p, q, t, r)) for q in X for r in X if q > r]
+        v = ints.V_pt(p, t)
+        i1 = [(BlockOp(sname, "B", q, r), float(v[q, r])) for q in X for r in X if q <= r]
+        i2 = [(BlockOp(sname, "B", r, q), float(v[q, r])) for q in X for r in X if q > r]
         dq = (0, spin_of(t) - spin_of(p))
         return lincomb(i1, dq), lincomb(i2, (0, -dq[1]))
 
