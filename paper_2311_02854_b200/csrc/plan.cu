@@ -15,6 +15,7 @@
 // Terms are processed in chunks sized so the X intermediates fit the workspace.
 #include <algorithm>
 #include <array>
+#include <atomic>
 #include <cmath>
 #include <cstdlib>
 #include <new>
@@ -64,7 +65,7 @@ static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N
 
 __global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops, double* __restrict__ pack);
 
-struct TileRec { Tile t; double cost; int64_t key = 0; };   // key: secondary launch order inside a cost bucket
+struct TileRec { Tile t; double cost; int64_t key = 0; int32_t bucket = 0; };   // key: secondary launch order inside a cost bucket
 
 constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are offsets into the packed R store
 
@@ -280,17 +281,6 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     P->stats[ST_CHUNKS] = (double)nchunks;
 
     // ---- build jobs / segments / tiles chunk by chunk ---------------------------------------------
-    std::vector<Job> jobs;
-    std::vector<Seg> segs;
-    std::vector<Tile> tiles;
-    std::vector<std::vector<HdItem>> hd(nblk);
-    std::vector<RedJob> reds;   // split-K reductions (stage 3)
-    std::vector<PackDesc> packs;   // packed R store (stage-1 B operands), filled on the device after upload
-    std::vector<size_t> pack_segs;  // segments whose b_off is relative to the packed store
-    int64_t pack_top = 0;
-    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
-    int64_t s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, ws_peak = 0;
-
     // The GEMM kernels read psi from a padded copy (rows padded to an even length, refreshed at the start of every
     // dmrg_sigma): every psi operand is then 16-byte aligned; consecutive blocks of a panel stay contiguous.
     std::vector<int64_t> ppad(nblk);
@@ -306,58 +296,69 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         if (panel_first[ir] < 0) panel_first[ir] = b;
         panel_rows[ir] += P->blocks[b].dl;
     }
-    MapTable maps;
     const int TILE = kVariants[0].bm;   // square tiles: the same box rules serve A and B operands
 
-    auto emit_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int stage) {
-        PlanGroup grp{stage, (int)P->launches.size(), 0};
-        for (int v = 0; v < NUM_VARIANTS; v++) {
-            auto& r = recs[v];
-            if (r.empty()) continue;
-            // longest first (LPT through the hardware block scheduler); inside a sqrt(2)-wide cost bucket, stage-2
-            // tiles follow `key` = (L sector of the sigma block, split-K part): sigma blocks of one L-sector row walk
-            // the same L operator blocks, so launching them together lets them share those blocks in L2
-            if (kTileOrder)
-                std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) {
-                    const int ba = (int)std::floor(2.0 * std::log2(a.cost)), bb = (int)std::floor(2.0 * std::log2(b.cost));
-                    if (ba != bb) return ba > bb;
-                    return a.key < b.key;
-                });
-            else
-                std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
-            // measurement knob: tiles of small-block jobs (min(M, N) < kSplitSmall) move, in order, to the end of the
-            // list and get a launch of their own, so that ncu reports the small-block batch (HBM-bound) apart from the
-            // large-block one (FP64-pipe bound).  Same kernel, same tiles, same results; default off.
-            size_t nbig = r.size();
-            if (kSplitSmall > 0)
-                nbig = std::stable_partition(r.begin(), r.end(), [&](const TileRec& a) {
-                           const Job& j = jobs[a.t.job];
-                           int d = std::min(j.M, j.N);
-                           if (j.seg_end - j.seg_begin == 1) d = std::min(d, segs[j.seg_begin].K);   // stage 1: K = d_R
-                           return d >= kSplitSmall;
-                       }) - r.begin();
-            // grid.x limit: split very long lists
-            size_t i = 0;
-            if (nbig > 0 && nbig < r.size()) {
-                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)nbig});
-                for (size_t j = 0; j < nbig; j++) tiles.push_back(r[j].t);
-                i = nbig;
-            }
-            while (i < r.size()) {
-                const size_t n = std::min<size_t>(r.size() - i, (size_t)1 << 30);
-                P->launches.push_back({v, stage, (int64_t)tiles.size(), (int64_t)n});
-                for (size_t j = i; j < i + n; j++) tiles.push_back(r[j].t);
-                i += n;
-            }
-            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)r.size();
+    // The chunks are planned independently of each other by all host threads, each into its own ChunkOut with
+    // chunk-local job / segment / tensor-map indices and pack offsets; they are then appended in chunk order (the
+    // result does not depend on the thread count).
+    struct TileList { std::vector<Tile> tiles; size_t nbig = 0; };   // sorted tiles of one stage; [0, nbig) = large-block jobs (split_small)
+    struct ChunkOut {
+        std::vector<Job> jobs;
+        std::vector<Seg> segs;
+        TileList t1, t2;
+        std::vector<RedJob> reds;
+        std::vector<PackDesc> packs;
+        std::vector<size_t> pack_segs;
+        std::vector<std::pair<int32_t, HdItem>> hd;
+        MapTable maps;
+        int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0;
+        double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
+        int rc = DMRG_OK;
+        std::string err;
+    };
+    // longest first (LPT through the hardware block scheduler); inside a sqrt(2)-wide cost bucket, stage-2
+    // tiles follow `key` = (L sector of the sigma block, split-K part): sigma blocks of one L-sector row walk
+    // the same L operator blocks, so launching them together lets them share those blocks in L2
+    auto sort_tiles = [&](std::vector<TileRec>& r, const std::vector<Job>& jobs, const std::vector<Seg>& segs, TileList& out) {
+        if (kTileOrder) {
+            for (auto& x : r) x.bucket = (int32_t)std::floor(2.0 * std::log2(x.cost));
+            std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) {
+                if (a.bucket != b.bucket) return a.bucket > b.bucket;
+                return a.key < b.key;
+            });
+        } else {
+            std::stable_sort(r.begin(), r.end(), [](const TileRec& a, const TileRec& b) { return a.cost > b.cost; });
         }
-        grp.nlaunch = (int)P->launches.size() - grp.first_launch;
-        if (grp.nlaunch > 0) P->groups.push_back(grp);
+        // measurement aid: tiles of small-block jobs (min(M, N, K) < split_small) move, in order, to the end of the
+        // list and get a launch of their own, so that ncu reports the small-block batch (HBM-side) apart from the
+        // large-block one (FP64-pipe bound).  Same kernel, same tiles, same results; default off.
+        size_t nbig = r.size();
+        if (kSplitSmall > 0)
+            nbig = std::stable_partition(r.begin(), r.end(), [&](const TileRec& a) {
+                       const Job& j = jobs[a.t.job];
+                       int d = std::min(j.M, j.N);
+                       if (j.seg_end - j.seg_begin == 1) d = std::min(d, segs[j.seg_begin].K);   // stage 1: K = d_R
+                       return d >= kSplitSmall;
+                   }) - r.begin();
+        out.nbig = nbig;
+        out.tiles.reserve(r.size());
+        for (auto& x : r) out.tiles.push_back(x.t);
     };
 
-    for (int64_t ch = 0; ch < nchunks; ch++) {
+    auto build_chunk = [&](int64_t ch, ChunkOut& O) -> int {
+        auto& jobs = O.jobs;
+        auto& segs = O.segs;
+        auto& reds = O.reds;
+        auto& packs = O.packs;
+        auto& pack_segs = O.pack_segs;
+        auto& maps = O.maps;
+        int64_t& pack_top = O.pack_top;
+        int64_t& ws_peak = O.ws_peak;
+        int64_t& s1_jobs = O.s1_jobs;
+        double &alg_flops = O.alg_flops, &s1_flops = O.s1_flops, &s2_flops = O.s2_flops, &padded_flops = O.padded_flops, &alg_bytes = O.alg_bytes,
+               &stage_flops = O.stage_flops, &tile_flops = O.tile_flops, &warp_flops = O.warp_flops;
         const int64_t t0 = term_task_begin[chunk_begin[ch]], t1 = term_task_begin[chunk_begin[ch + 1]];
-        if (t0 == t1) continue;
+        if (t0 == t1) return DMRG_OK;
         // -- stage 1: unique (R block, trans, psi block) products, merged into runs of consecutive psi blocks
         struct XReq { int64_t r_off; int32_t r_trans, in_blk, dRo; };
         std::vector<XReq> req;
@@ -497,7 +498,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             c0 = c1;
         }
         ws_peak = std::max(ws_peak, xtop);
-        emit_tiles(recs1, 1);
+        sort_tiles(recs1[0], jobs, segs, O.t1);
 
         // -- stage 2: per sigma block, the ordered list of contributions -----------------------------
         std::vector<int64_t> idx(t1 - t0);
@@ -531,7 +532,6 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         // write (8 bytes per 2*K flops) cost nothing.
         const double smax = std::max<double>(kMinSplitStages, tile_stages / (kCtaSlots * kSplitWaves));
         std::vector<TileRec> recs2[NUM_VARIANTS];
-        const size_t red_begin = reds.size();
         int64_t ptop = xtop;   // split-K partial tiles live behind the X intermediates
         std::vector<Seg> ident_segs, gemm_segs;
         for (const Group& g : groups) {
@@ -580,7 +580,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
                 }
                 (ident ? ident_segs : gemm_segs).push_back(s);
-                if (k.in_blk == k.out_blk) hd[ob].push_back({k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha});
+                if (k.in_blk == k.out_blk) O.hd.push_back({(int32_t)ob, HdItem{k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha}});
             }
             cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
             cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
@@ -644,9 +644,95 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             DMRG_REQUIRE(segs.size() < ((size_t)1 << 31) && jobs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
         }
         ws_peak = std::max(ws_peak, ptop);
-        emit_tiles(recs2, 2);
-        if (reds.size() > red_begin) P->groups.push_back({3, (int)red_begin, (int)(reds.size() - red_begin)});
+        sort_tiles(recs2[0], jobs, segs, O.t2);
+        return DMRG_OK;
+    };
+
+    std::vector<ChunkOut> outs((size_t)nchunks);
+    {
+        const unsigned nthr = (unsigned)std::max<int64_t>(1, std::min<int64_t>({(int64_t)std::thread::hardware_concurrency(), nchunks, 32}));
+        std::atomic<int64_t> next{0};
+        auto worker = [&]() {
+            for (int64_t ch = next.fetch_add(1); ch < nchunks; ch = next.fetch_add(1)) {
+                try {
+                    outs[ch].rc = build_chunk(ch, outs[ch]);
+                    if (outs[ch].rc != DMRG_OK) outs[ch].err = dmrg_last_error();   // set_error is thread-local
+                } catch (const std::bad_alloc&) {
+                    outs[ch].rc = DMRG_ENOMEM;
+                    outs[ch].err = "dmrg_plan_create: out of host memory";
+                } catch (const std::exception& e) {
+                    outs[ch].rc = DMRG_EINVAL;
+                    outs[ch].err = std::string("dmrg_plan_create: ") + e.what();
+                }
+            }
+        };
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < nthr; t++) pool.emplace_back(worker);
+        worker();
+        for (auto& th : pool) th.join();
     }
+    // ---- append the chunks in order ----------------------------------------------------------------------------
+    std::vector<Job> jobs;
+    std::vector<Seg> segs;
+    std::vector<Tile> tiles;
+    std::vector<std::vector<HdItem>> hd(nblk);
+    std::vector<RedJob> reds;   // split-K reductions (stage 3)
+    std::vector<PackDesc> packs;   // packed R store (stage-1 B operands), filled on the device after upload
+    std::vector<size_t> pack_segs;  // segments whose b_off is relative to the packed store
+    MapTable maps;
+    int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0;
+    double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
+    for (int64_t ch = 0; ch < nchunks; ch++) {
+        ChunkOut& O = outs[ch];
+        if (O.rc != DMRG_OK) { set_error("%s", O.err.c_str()); return O.rc; }
+        const size_t job_base = jobs.size(), seg_base = segs.size();
+        DMRG_REQUIRE(job_base + O.jobs.size() < ((size_t)1 << 31) && seg_base + O.segs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
+        std::vector<int32_t> map_id(O.maps.descs.size());
+        for (size_t m = 0; m < O.maps.descs.size(); m++) {
+            MapDesc d = O.maps.descs[m];
+            if (d.space == MS_PACK) d.off += pack_top;
+            map_id[m] = maps.get(d.space, d.off, d.kind, d.inner, d.outer, d.ld, BoxShape{d.box_inner, d.box_outer});
+        }
+        for (Job jb : O.jobs) { jb.seg_begin += (int32_t)seg_base; jb.seg_end += (int32_t)seg_base; jobs.push_back(jb); }
+        for (Seg sg : O.segs) {
+            if (!(sg.flags & SEG_A_IDENT)) { sg.a_map = map_id[sg.a_map]; sg.b_map = map_id[sg.b_map]; }
+            segs.push_back(sg);
+        }
+        for (size_t q : O.pack_segs) { segs[seg_base + q].b_off += pack_top; pack_segs.push_back(seg_base + q); }
+        for (PackDesc pd : O.packs) { pd.dst += pack_top; packs.push_back(pd); }
+        for (auto& h : O.hd) hd[h.first].push_back(h.second);
+        int stage = 1;
+        for (TileList* tl : {&O.t1, &O.t2}) {
+            PlanGroup grp{stage, (int)P->launches.size(), 0};
+            size_t i = 0;
+            const size_t n = tl->tiles.size();
+            auto push_range = [&](size_t lo, size_t hi) {
+                while (lo < hi) {   // grid.x limit: split very long lists
+                    const size_t cnt = std::min<size_t>(hi - lo, (size_t)1 << 30);
+                    P->launches.push_back({0, stage, (int64_t)tiles.size(), (int64_t)cnt});
+                    for (size_t j = lo; j < lo + cnt; j++) { Tile t = tl->tiles[j]; t.job += (int32_t)job_base; tiles.push_back(t); }
+                    lo += cnt;
+                }
+            };
+            if (tl->nbig > 0 && tl->nbig < n) { push_range(0, tl->nbig); i = tl->nbig; }
+            push_range(i, n);
+            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)n;
+            grp.nlaunch = (int)P->launches.size() - grp.first_launch;
+            if (grp.nlaunch > 0) P->groups.push_back(grp);
+            stage++;
+        }
+        if (!O.reds.empty()) {
+            P->groups.push_back({3, (int)reds.size(), (int)O.reds.size()});
+            reds.insert(reds.end(), O.reds.begin(), O.reds.end());
+        }
+        pack_top += O.pack_top;
+        ws_peak = std::max(ws_peak, O.ws_peak);
+        s1_jobs += O.s1_jobs;
+        alg_flops += O.alg_flops; s1_flops += O.s1_flops; s2_flops += O.s2_flops; padded_flops += O.padded_flops; alg_bytes += O.alg_bytes;
+        stage_flops += O.stage_flops; tile_flops += O.tile_flops; warp_flops += O.warp_flops;
+        O = ChunkOut();   // release the chunk's host memory
+    }
+
     P->stats[ST_ALG_FLOPS] = alg_flops;
     P->stats[ST_S1_FLOPS] = s1_flops;
     P->stats[ST_S2_FLOPS] = s2_flops;
