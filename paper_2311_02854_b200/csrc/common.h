@@ -124,6 +124,9 @@ struct dmrg_ops {
     std::vector<std::vector<int32_t>> colsec;
     double* d_values = nullptr;    // base of the store's address space: every block offset is relative to it
     std::vector<double*> owned;    // device allocations the store owns (d_values first; joined / appended arrays after it)
+    double* side_alloc[2] = {nullptr, nullptr};   // dmrg_ops_load: the allocation holding the L-side / R-side blocks (also in `owned`)
+    size_t side_bytes[2] = {0, 0};
+    mutable bool r_released = false;   // a plan created with release_r_store freed side_alloc[1]: the store serves that plan only
     bool structure_only = false;   // loaded with values == NULL: planning / statistics only, no device memory
     int64_t nvalues_dev = 0;     // doubles allocated (stored + lincomb, padded)
     int64_t device_bytes = 0;

@@ -23,7 +23,7 @@ void set_error(const char* fmt, ...) {
     g_err = buf;
 }
 
-struct RepackDesc { int64_t src, dst; int32_t rows, cols, ld, pad_; };
+struct RepackDesc { int64_t src, dst; int32_t rows, cols, ld, side; };   // side: which of the store's two allocations dst lives in (host bookkeeping)
 
 // dst[r*ld + c] = c < cols ? src[r*cols + c] : 0      one CTA per block
 __global__ void __launch_bounds__(256) repack_kernel(const RepackDesc* __restrict__ desc, const double* __restrict__ src_base,
@@ -86,7 +86,9 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
 
     std::vector<RepackDesc> rep;
     rep.reserve(nblocks);
-    int64_t top = 0;   // device doubles
+    // L-side and R-side blocks live in two device allocations (the R side can be released once a plan has packed it,
+    // dmrg_plan_options.release_r_store); while the layout is computed, offsets are local to their side's allocation
+    int64_t tops[2] = {0, 0};   // device doubles per side
     for (int o = 0; o < nops; o++) {
         const dmrg_op_desc& d = ops[o];
         DMRG_REQUIRE(d.side == 0 || d.side == 1, "dmrg_ops_load: op %d has side %d", o, d.side);
@@ -110,14 +112,16 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             DMRG_REQUIRE(bd.offset >= 0 && bd.offset + (int64_t)rows * cols <= nvalues,
                          "dmrg_ops_load: block %lld exceeds values[]", (long long)b);
             const int ld = (int)round_up2(cols);
+            int64_t& top = tops[d.side];
             S->row_off[o][bd.row_sector] = top;
-            rep.push_back({bd.offset, top, rows, cols, ld, 0});
+            rep.push_back({bd.offset, top, rows, cols, ld, d.side});
             top += (int64_t)rows * ld;
         }
     }
     // linear combinations: block present where any summand has one
     std::vector<LinDesc> lind;
     std::vector<LinSummand> lins;
+    std::vector<int> lin_side;   // side of lind[i] (its summands are on the same side)
     for (int o = 0; o < nops; o++) {
         const dmrg_op_desc& d = ops[o];
         if (d.kind != DMRG_OP_LINCOMB) continue;
@@ -139,7 +143,9 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             for (int64_t i = i0; i < i1; i++) any = any || S->row_off[lin_op[i]][r] >= 0;
             if (!any) continue;
             const int64_t n = (int64_t)sec[r].dim * round_up2(sec[c].dim);
+            int64_t& top = tops[d.side];
             LinDesc ld{top, n, (int32_t)lins.size(), 0};
+            lin_side.push_back(d.side);
             for (int64_t i = i0; i < i1; i++) lins.push_back({S->row_off[lin_op[i]][r], lin_coef[i]});
             ld.sum_end = (int32_t)lins.size();
             lind.push_back(ld);
@@ -147,12 +153,35 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             top += n;
         }
     }
-    S->nvalues_dev = top;
-    S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
-    if (S->structure_only) return DMRG_OK;
-    DMRG_CUDA(cudaMalloc(&S->d_values, sizeof(double) * (size_t)std::max<int64_t>(top, 2)));
-    S->owned.push_back(S->d_values);
-    S->device_bytes = sizeof(double) * std::max<int64_t>(top, 2);
+    S->nvalues_dev = tops[0] + tops[1];
+    S->side_bytes[0] = tops[0] > 0 ? sizeof(double) * (size_t)std::max<int64_t>(tops[0], 2) : 0;
+    S->side_bytes[1] = tops[1] > 0 ? sizeof(double) * (size_t)std::max<int64_t>(tops[1], 2) : 0;
+    S->device_bytes = (int64_t)(S->side_bytes[0] + S->side_bytes[1]);
+    if (S->structure_only) {   // planning only: one linear numbering, R behind L
+        for (int o = 0; o < nops; o++)
+            if (ops[o].side == 1)
+                for (auto& off : S->row_off[o]) if (off >= 0) off += tops[0];
+        return DMRG_OK;
+    }
+    double* side_ptr[2] = {nullptr, nullptr};
+    for (int sd = 0; sd < 2; sd++)
+        if (S->side_bytes[sd]) {
+            DMRG_CUDA(cudaMalloc(&side_ptr[sd], S->side_bytes[sd]));
+            S->owned.push_back(side_ptr[sd]);
+            S->side_alloc[sd] = side_ptr[sd];
+        }
+    // one address space for both: offsets relative to the lower allocation (>= 0; both are cudaMalloc'ed, so the
+    // distance is a multiple of 32 doubles and every row keeps its 16-byte alignment)
+    S->d_values = side_ptr[0] && side_ptr[1] ? std::min(side_ptr[0], side_ptr[1]) : (side_ptr[0] ? side_ptr[0] : side_ptr[1]);
+    DMRG_REQUIRE(S->d_values != nullptr, "dmrg_ops_load: the store has no blocks");
+    const int64_t shift[2] = {side_ptr[0] ? (int64_t)(side_ptr[0] - S->d_values) : 0, side_ptr[1] ? (int64_t)(side_ptr[1] - S->d_values) : 0};
+    for (int o = 0; o < nops; o++)
+        for (auto& off : S->row_off[o]) if (off >= 0) off += shift[ops[o].side];
+    for (auto& r : rep) r.dst += shift[r.side];
+    for (size_t i = 0; i < lind.size(); i++) {
+        lind[i].dst += shift[lin_side[i]];
+        for (int q = lind[i].sum_begin; q < lind[i].sum_end; q++) if (lins[q].src >= 0) lins[q].src += shift[lin_side[i]];
+    }
 
     // ---- repack stored blocks (row padding) -------------------------------------------------
     if (!rep.empty()) {

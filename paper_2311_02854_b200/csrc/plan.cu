@@ -106,6 +106,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     const bool kTileOrder = pol.tile_order;
     const int kSplitSmall = pol.split_small;
     P->copy_mode = pol.copy_mode;
+    const bool kReleaseR = pol.release_r_store;
+    DMRG_REQUIRE(!P->ops->r_released, "dmrg_plan_create: the R-side blocks of this store were released to an earlier plan (release_r_store)");
     const dmrg_ops* S = P->ops;
     const auto& secL = S->sec[0];
     const auto& secR = S->sec[1];
@@ -377,6 +379,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         });
         std::unordered_map<int64_t, XLoc> xloc;
         xloc.reserve(req.size() * 2);
+        std::unordered_map<int64_t, int64_t> pack_loc;   // (R block, trans) -> chunk-local offset of its packed copy
         std::vector<TileRec> recs1[NUM_VARIANTS];
         std::vector<std::pair<int, int>> cut_m, cut_n;
         int64_t xtop = 0;
@@ -436,6 +439,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
             for (size_t c = c0; c < c1; c++) {
                 const XReq& r0 = req[runs[rblks[c].r0].i];
                 packs.push_back({r0.r_off, pack_top + col0 * ldp, r0.dRo, dRi, (int32_t)round_up2(r0.r_trans ? r0.dRo : dRi), r0.r_trans, ldp, 0});
+                pack_loc[r0.r_off * 2 + r0.r_trans] = pack_top + col0 * ldp;
                 col0s.push_back(col0);
                 col0 += round_up2(r0.dRo);
                 alg_bytes += 8.0 * (double)dRi * r0.dRo;
@@ -580,7 +584,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
                 }
                 (ident ? ident_segs : gemm_segs).push_back(s);
-                if (k.in_blk == k.out_blk) O.hd.push_back({(int32_t)ob, HdItem{k.l_off, k.r_off, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha}});
+                if (k.in_blk == k.out_blk) {
+                    // diagonal term: with release_r_store the R diagonal is read from the packed copy (same pitch; a
+                    // transposed copy has the same diagonal), addressed like the packed segments: kPackBase + offset
+                    const int64_t r_at = k.r_off < 0 ? kHdIdent : (kReleaseR ? kPackBase + pack_loc.at(k.r_off * 2 + k.r_trans) : k.r_off);
+                    O.hd.push_back({(int32_t)ob, HdItem{k.l_off < 0 ? kHdIdent : k.l_off, r_at, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha}});
+                }
             }
             cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
             cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
@@ -700,7 +709,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         }
         for (size_t q : O.pack_segs) { segs[seg_base + q].b_off += pack_top; pack_segs.push_back(seg_base + q); }
         for (PackDesc pd : O.packs) { pd.dst += pack_top; packs.push_back(pd); }
-        for (auto& h : O.hd) hd[h.first].push_back(h.second);
+        for (auto& h : O.hd) {
+            if (h.second.r_off >= kPackBase) h.second.r_off += pack_top;
+            hd[h.first].push_back(h.second);
+        }
         int stage = 1;
         for (TileList* tl : {&O.t1, &O.t2}) {
             PlanGroup grp{stage, (int)P->launches.size(), 0};
@@ -782,6 +794,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         for (size_t q : pack_segs) segs[q].b_off += delta - kPackBase;
     }
     for (Seg& sg : segs) sg.flags |= sg.alpha == 1.0 ? SEG_ALPHA_ONE : (sg.alpha == -1.0 ? SEG_ALPHA_NEG : 0u);
+    {
+        const int64_t delta = (int64_t)(P->d_pack - S->d_values);
+        for (HdItem& h : hd_items) if (h.r_off >= kPackBase) h.r_off += delta - kPackBase;
+    }
     int rc;
     if ((rc = up((void**)&P->d_jobs, jobs.data(), jobs.size() * sizeof(Job)))) return rc;
     if ((rc = up((void**)&P->d_segs, segs.data(), segs.size() * sizeof(Seg)))) return rc;
@@ -808,6 +824,16 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
         DMRG_CUDA(cudaGetLastError());
         DMRG_CUDA(cudaDeviceSynchronize());
         cudaFree(d_packs);
+    }
+    if (kReleaseR && S->side_alloc[1]) {
+        // nothing reads the R-side originals any more (stage 1 and the diagonal use the packed copy): give the memory back
+        dmrg_ops* Sm = const_cast<dmrg_ops*>(S);
+        cudaFree(Sm->side_alloc[1]);
+        Sm->owned.erase(std::remove(Sm->owned.begin(), Sm->owned.end(), Sm->side_alloc[1]), Sm->owned.end());
+        Sm->device_bytes -= (int64_t)Sm->side_bytes[1];
+        Sm->side_alloc[1] = nullptr;
+        Sm->side_bytes[1] = 0;
+        Sm->r_released = true;
     }
     return gemm_init();
 }
@@ -872,8 +898,8 @@ __global__ void __launch_bounds__(256) hdiag_kernel(const HdBlock* __restrict__ 
         for (int q = ty; q < nit; q += 8) {   // item q: lane tx fetches L[i0+tx][i0+tx] and R[j0+tx][j0+tx]
             const HdItem h = items[base + q];
             const int i = i0 + tx, j = j0 + tx;
-            sl[q][tx] = (h.l_off >= 0 && i < b.dl) ? ops[h.l_off + (int64_t)i * h.ldl + i] : 1.0;
-            sr[q][tx] = (h.r_off >= 0 && j < b.dr) ? ops[h.r_off + (int64_t)j * h.ldr + j] : 1.0;
+            sl[q][tx] = (h.l_off != kHdIdent && i < b.dl) ? ops[h.l_off + (int64_t)i * h.ldl + i] : 1.0;
+            sr[q][tx] = (h.r_off != kHdIdent && j < b.dr) ? ops[h.r_off + (int64_t)j * h.ldr + j] : 1.0;
             if (tx == 0) sa[q] = h.alpha;
         }
         __syncthreads();

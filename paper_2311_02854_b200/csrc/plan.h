@@ -2,7 +2,8 @@
 #pragma once
 #include "common.h"
 
-struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };   // offsets < 0: identity factor
+constexpr int64_t kHdIdent = INT64_MIN;   // HdItem offset of an identity factor (a packed R block can sit below the store: plain negatives are addresses)
+struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };
 struct HdTile { int32_t blk; int16_t ti, tj; };   // 32 x 32 tile of a psi block
 struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; int64_t pad_off; };   // pad_off: block in the padded psi copy
 

@@ -89,6 +89,7 @@ static int renormalize_impl(const dmrg_ops* in, int side, const dmrg_sector* new
                             const dmrg_rterm* terms, const double* site_ops, const int32_t* site_parity, int nsite,
                             const dmrg_renorm_options* opt, cudaStream_t st, dmrg_ops* out, dmrg_renorm_stats* stats) {
     DMRG_REQUIRE(in && !in->structure_only, "dmrg_renormalize: the input store has no values");
+    DMRG_REQUIRE(!in->r_released, "dmrg_renormalize: the R-side blocks of the input store were released to a plan");
     DMRG_REQUIRE(side == 0 || side == 1, "dmrg_renormalize: side must be 0 (block x site) or 1 (site x block)");
     DMRG_REQUIRE(new_sec && n_new > 0 && wb && n_wb > 0 && wvalues && new_ops && n_new_ops > 0 && term_ptr && site_ops && site_parity && nsite > 0,
                  "dmrg_renormalize: NULL or empty argument");
@@ -391,6 +392,7 @@ int64_t dmrg_ops_num_values(const dmrg_ops* S) {
 int dmrg_ops_export(const dmrg_ops* S, dmrg_op_desc* ops_out, dmrg_block_desc* blocks_out, double* values_out) {
     if (!S || !ops_out || !blocks_out || !values_out) { set_error("dmrg_ops_export: NULL argument"); return DMRG_EINVAL; }
     if (S->structure_only) { set_error("dmrg_ops_export: the store was loaded without values"); return DMRG_EINVAL; }
+    if (S->r_released) { set_error("dmrg_ops_export: the R-side blocks of this store were released to a plan"); return DMRG_EINVAL; }
     std::vector<UnpackDesc> desc;
     int64_t nb = 0, nv = 0;
     for (size_t o = 0; o < S->ops.size(); o++) {
@@ -462,6 +464,8 @@ int dmrg_ops_join(dmrg_ops* left, dmrg_ops* right, dmrg_ops** out) {
         J->row_off.push_back(right->row_off[o]);
     }
     J->d_values = base;
+    // release_r_store needs the R side in ONE allocation of its own: true when `right` is a single-allocation store
+    if (right->owned.size() == 1) { J->side_alloc[1] = right->owned[0]; J->side_bytes[1] = (size_t)right->device_bytes; }
     J->owned = left->owned;
     J->owned.insert(J->owned.end(), right->owned.begin(), right->owned.end());
     J->nvalues_dev = left->nvalues_dev + right->nvalues_dev;
@@ -553,7 +557,7 @@ static int form_lincombs(const dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t
 int dmrg_ops_add_lincombs(dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
                           const double* lin_coef, const int32_t* lin_trans, int32_t nlin) {
     if (!S || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_add_lincombs: NULL or empty argument"); return DMRG_EINVAL; }
-    if (S->structure_only || S->owned.empty()) { set_error("dmrg_ops_add_lincombs: the store holds no device values"); return DMRG_EINVAL; }
+    if (S->structure_only || S->owned.empty() || S->r_released) { set_error("dmrg_ops_add_lincombs: the store holds no device values (or its R side was released)"); return DMRG_EINVAL; }
     std::vector<std::vector<int64_t>> new_off;
     std::vector<std::vector<int32_t>> new_colsec;
     double* d_new = nullptr;
@@ -584,7 +588,7 @@ int dmrg_ops_derive(const dmrg_ops* src, const dmrg_op_desc* lin_ops, int32_t n_
     if (!out) { set_error("dmrg_ops_derive: out is NULL"); return DMRG_EINVAL; }
     *out = nullptr;
     if (!src || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_derive: NULL or empty argument"); return DMRG_EINVAL; }
-    if (src->structure_only || src->owned.empty()) { set_error("dmrg_ops_derive: the source store holds no device values"); return DMRG_EINVAL; }
+    if (src->structure_only || src->owned.empty() || src->r_released) { set_error("dmrg_ops_derive: the source store holds no device values (or its R side was released)"); return DMRG_EINVAL; }
     dmrg_ops* D = new (std::nothrow) dmrg_ops();
     if (!D) { set_error("dmrg_ops_derive: out of host memory"); return DMRG_ENOMEM; }
     double* d_new = nullptr;

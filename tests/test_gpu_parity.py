@@ -220,3 +220,32 @@ def test_plan_options_give_the_same_sigma():
         assert np.abs(out - orc).max() / np.linalg.norm(orc) <= TOL_SIGMA, kw
     plan.destroy()
     ops.free()
+
+
+def test_release_r_store_frees_the_r_side_and_changes_nothing():
+    """dmrg_plan_options.release_r_store: once stage 1 and the diagonal read the plan's packed copy of the R blocks, the
+    store's R-side allocation is freed.  sigma is bitwise the same, the diagonal still matches the oracle, the store
+    shrinks, and it refuses to serve a second plan."""
+    g = _gpu()
+    from dmrg_workload.problem import make_direct_problem
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr)
+    psi = random_psi(pr.psi_size, 11)
+    ref = _sigma_gpu(plan, psi)
+    plan.destroy()
+    before = ops.device_bytes
+    plan2 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, release_r_store=1)
+    assert ops.device_bytes < 0.75 * before
+    assert np.array_equal(_sigma_gpu(plan2, psi), ref)
+    d = torch.empty(pr.psi_size, dtype=torch.float64, device="cuda")
+    plan2.hdiag(d, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    hd = oracle.opair_hdiag(pr)
+    assert np.abs(d.cpu().numpy() - hd).max() <= 1e-12 * max(1.0, np.abs(hd).max())
+    x = torch.from_numpy(psi).cuda()
+    res = plan2.davidson(x, max_iter=5, max_space=5, tol=0.0, stream=torch.cuda.current_stream())
+    assert res["iters"] == 5
+    with pytest.raises(g.DmrgError):
+        g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot)
+    plan2.destroy()
+    ops.free()
