@@ -142,6 +142,13 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *                      get a launch of their own (same tiles, same results, more launches)
  *   release_r_store    1 = after packing, free the store's R-side blocks (the plan's packed copy is then the only
  *                      one; the store can serve no further dmrg_plan_create); 0 = keep (default)
+ *   shard_rank, shard_count   operator parallelism ("distribute operators and partition mu"): with
+ *                      shard_count > 1 the plan evaluates only its share of the terms -- one contiguous range of the
+ *                      planner's ordered term list (ordered by R operator, so a range needs only its own complementary
+ *                      operators), cut where the running canonical cost crosses shard_rank/shard_count of the total;
+ *                      every rank derives the same cuts from the same inputs.  dmrg_sigma / dmrg_hdiag then return
+ *                      PARTIAL results: the caller sums them over ranks (one all-reduce of psi_size doubles per call;
+ *                      paper_2311_02854_b200/sharded.py).  dmrg_plan_shard_terms lists the terms of the share.
  */
 typedef struct {
     int64_t workspace_bytes;
@@ -152,7 +159,8 @@ typedef struct {
     int32_t cost_order_only;
     int32_t split_small;
     int32_t release_r_store;
-    int32_t reserved[8];
+    int32_t shard_rank, shard_count;
+    int32_t reserved[6];
 } dmrg_plan_options;
 
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,
@@ -165,6 +173,9 @@ int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t n
                           dmrg_plan** out);
 void    dmrg_plan_destroy(dmrg_plan* plan);
 int64_t dmrg_plan_psi_size(const dmrg_plan* plan);            /* doubles in psi / sigma         */
+/* indices (into the caller's terms[]) of the terms this plan evaluates, in plan order; copies up to `capacity` of them
+ * to out [host, may be NULL] and returns their number (= nterms unless the plan is a shard) */
+int64_t dmrg_plan_shard_terms(const dmrg_plan* plan, int64_t* out, int64_t capacity);
 int64_t dmrg_plan_num_psi_blocks(const dmrg_plan* plan);
 int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host], num_psi_blocks */);
 

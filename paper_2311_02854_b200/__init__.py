@@ -25,7 +25,7 @@ assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
 
 PLANOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("min_split_stages", "<i4"), ("split_waves", "<f8"),
                        ("max_merged_cols", "<i4"), ("cost_order_only", "<i4"), ("split_small", "<i4"), ("release_r_store", "<i4"),
-                       ("reserved", "<i4", (8,))], align=True)
+                       ("shard_rank", "<i4"), ("shard_count", "<i4"), ("reserved", "<i4", (6,))], align=True)
 assert PLANOPT_DT.itemsize == 72
 COPY_LDGSTS, COPY_TMA = 1, 2
 WBLOCK_DT = np.dtype([("old_sector", "<i4"), ("site_state", "<i4"), ("new_sector", "<i4"), ("reserved", "<i4"), ("offset", "<i8")], align=True)
@@ -40,7 +40,7 @@ STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_j
              "xws_elems", "tensor_maps")
 
 EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_create_opts", "dmrg_plan_destroy",
-           "dmrg_plan_psi_size", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",
+           "dmrg_plan_psi_size", "dmrg_plan_shard_terms", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",
            "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
            "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
@@ -78,6 +78,8 @@ def lib():
         L.dmrg_plan_destroy.restype = None
         L.dmrg_plan_psi_size.argtypes = [vp]
         L.dmrg_plan_psi_size.restype = i64
+        L.dmrg_plan_shard_terms.argtypes = [vp, vp, i64]
+        L.dmrg_plan_shard_terms.restype = i64
         L.dmrg_plan_num_psi_blocks.argtypes = [vp]
         L.dmrg_plan_num_psi_blocks.restype = i64
         L.dmrg_plan_psi_layout.argtypes = [vp, vp]
@@ -295,6 +297,13 @@ class Plan:
     @property
     def psi_size(self):
         return int(lib().dmrg_plan_psi_size(self._h))
+
+    def shard_terms(self):
+        """Indices (into the term arrays given to the constructor) of the terms this plan evaluates, in plan order."""
+        n = int(lib().dmrg_plan_shard_terms(self._h, None, 0))
+        out = np.zeros(max(n, 1), dtype=np.int64)
+        lib().dmrg_plan_shard_terms(self._h, _ptr(out), n)
+        return out[:n]
 
     def psi_layout(self):
         """int64 [nblk,7]: (iL, c1, c2, iR, dL, dR, offset)."""

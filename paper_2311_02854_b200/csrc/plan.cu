@@ -82,6 +82,7 @@ struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     bool tile_order;
     int split_small;
     bool release_r_store;
+    int shard_rank, shard_count;
 };
 
 static PlanPolicy make_policy(const dmrg_plan_options* o) {
@@ -94,12 +95,15 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
     p.release_r_store = o && o->release_r_store;
+    p.shard_count = (o && o->shard_count > 1) ? o->shard_count : 1;
+    p.shard_rank = (o && o->shard_count > 1) ? o->shard_rank : 0;
     return p;
 }
 
-static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, const double* site_ops,
+static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, const double* site_ops,
                       const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
                       const PlanPolicy& pol) {
+    int64_t nterms = nterms_in;   // shrinks to this rank's share when the plan is a shard
     const int64_t workspace_bytes = pol.workspace_bytes;
     const int64_t kMaxMergedCols = pol.max_merged_cols;
     const double kSplitWaves = pol.split_waves, kMinSplitStages = pol.min_split_stages;
@@ -182,6 +186,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
     // ---- enumerate tasks: (term, psi block, dot transition)  (Eq. 7 at the level of blocks) ------
     std::vector<Task> tasks;
     std::vector<int64_t> term_task_begin(nterms + 1, 0);
+    std::vector<double> term_flops(nterms, 0.0);
     double canon_flops = 0.0;
     for (int64_t to = 0; to < nterms; to++) {
         const dmrg_term& T = terms[order[to]];
@@ -222,13 +227,41 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms, cons
                     k.l_off = l_off; k.r_off = r_off;
                     k.alpha = T.coef * zeta * v1 * v2;
                     tasks.push_back(k);
-                    if (r_off >= 0) canon_flops += 2.0 * k.dLi * k.dRi * k.dRo;
-                    if (l_off >= 0) canon_flops += 2.0 * k.dLo * k.dLi * k.dRo;
+                    if (r_off >= 0) term_flops[to] += 2.0 * k.dLi * k.dRi * k.dRo;
+                    if (l_off >= 0) term_flops[to] += 2.0 * k.dLo * k.dLi * k.dRo;
                 }
             }
         }
     }
     term_task_begin[nterms] = (int64_t)tasks.size();
+    // ---- operator parallelism: this plan keeps one contiguous range of the ORDERED term list -----------
+    // The terms are ordered by R operator, so a range needs only its own complementary operators; ranges are cut where
+    // the running canonical cost crosses k/shard_count of the total.  Every rank computes the same cuts (no communication);
+    // sigma = sum over ranks of the partial sigmas (one all-reduce of |psi| doubles per H psi, done by the caller).
+    if (pol.shard_count > 1) {
+        std::vector<double> prefix(nterms + 1, 0.0);
+        for (int64_t to = 0; to < nterms; to++) prefix[to + 1] = prefix[to] + term_flops[to];
+        auto cut = [&](int r) -> int64_t {
+            if (r <= 0) return 0;
+            if (r >= pol.shard_count) return nterms;
+            const double target = prefix[nterms] * r / pol.shard_count;
+            return (int64_t)(std::lower_bound(prefix.begin(), prefix.end(), target) - prefix.begin());
+        };
+        const int64_t lo = std::min(cut(pol.shard_rank), nterms), hi = std::max(lo, std::min(cut(pol.shard_rank + 1), nterms));
+        const int64_t tb = term_task_begin[lo], te = term_task_begin[hi];
+        std::vector<Task> kept(tasks.begin() + tb, tasks.begin() + te);
+        for (Task& k : kept) k.term_ord -= (int32_t)lo;
+        tasks.swap(kept);
+        std::vector<int64_t> ttb(hi - lo + 1);
+        for (int64_t to = lo; to <= hi; to++) ttb[to - lo] = term_task_begin[to] - tb;
+        term_task_begin.swap(ttb);
+        P->shard_terms.assign(order.begin() + lo, order.begin() + hi);
+        term_flops = std::vector<double>(term_flops.begin() + lo, term_flops.begin() + hi);
+        nterms = hi - lo;
+    } else {
+        P->shard_terms.assign(order.begin(), order.end());
+    }
+    for (double f : term_flops) canon_flops += f;
     P->stats[ST_TASKS] = (double)tasks.size();
     P->stats[ST_CANON_FLOPS] = canon_flops;
 
@@ -939,6 +972,10 @@ int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t n
         set_error("dmrg_plan_create: NULL or empty argument");
         return DMRG_EINVAL;
     }
+    if (options && options->shard_count > 1 && (options->shard_rank < 0 || options->shard_rank >= options->shard_count)) {
+        set_error("dmrg_plan_create: shard_rank %d outside [0, %d)", options->shard_rank, options->shard_count);
+        return DMRG_EINVAL;
+    }
     dmrg_plan* P = new (std::nothrow) dmrg_plan();
     if (!P) { set_error("dmrg_plan_create: out of host memory"); return DMRG_ENOMEM; }
     P->ops = ops;
@@ -972,6 +1009,12 @@ int dmrg_plan_psi_layout(const dmrg_plan* P, dmrg_psi_block* out) {
     if (!P || !out) { set_error("dmrg_plan_psi_layout: NULL argument"); return DMRG_EINVAL; }
     std::copy(P->blocks.begin(), P->blocks.end(), out);
     return DMRG_OK;
+}
+int64_t dmrg_plan_shard_terms(const dmrg_plan* P, int64_t* out, int64_t capacity) {
+    if (!P) return 0;
+    const int64_t n = (int64_t)P->shard_terms.size();
+    if (out) std::copy(P->shard_terms.begin(), P->shard_terms.begin() + std::min(n, capacity), out);
+    return n;
 }
 double dmrg_plan_stat(const dmrg_plan* P, int32_t key) { return (P && key >= 0 && key < ST_COUNT) ? P->stats[key] : -1.0; }
 

@@ -24,6 +24,7 @@ struct DavidsonWs;
 struct dmrg_plan {
     const dmrg_ops* ops = nullptr;
     std::vector<dmrg_psi_block> blocks;
+    std::vector<int64_t> shard_terms;   // indices (into the caller's term array) of the terms this plan evaluates, in plan order
     int64_t psi_size = 0;
     dmrg::Job* d_jobs = nullptr;
     dmrg::Seg* d_segs = nullptr;
