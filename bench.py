@@ -32,7 +32,7 @@ if ROOT not in sys.path:
 METRIC = "fp64_tflops_per_hpsi"
 # dram__bytes_read.sum + dram__bytes_write.sum of all GEMM launches of one H psi, from a committed ncu launch list
 # (NOT measured by this run): config -> (bytes, source)
-NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (1.53e12, "profiles/r1_cfg5_launches.csv (round 1 kernel)")}
+NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (1.60e12, "profiles/r2_cfg5_launches.csv (round 2, TMA kernel; 42 GEMM launches of the second dmrg_sigma call)")}
 UNIT = "TFLOP/s"
 
 
@@ -124,30 +124,35 @@ def pick_sample_blocks(pr, layout, budget_flops):
 
 
 def oracle_sample(pr, psi, total_flops, seconds):
-    """The oracle (all terms) on a bounded sample of sigma blocks, for the parity check of the timed configuration."""
+    """The oracle (all terms) on a bounded sample of sigma blocks, for the parity check of the timed configuration:
+    the LARGEST sigma block (the 436 x 436 class at cfg 5: 7 x 7 tiles, the most split-K parts) whenever the oracle can
+    do it in about half a minute, plus seeded random blocks up to the budget."""
     import oracle
     ncores = oracle.num_threads()
     layout = np.asarray(pr.layout)
     order, sizes = pick_sample_blocks(pr, layout, 0)
-    # probe with one mid-sized block to calibrate, then size the sample to `seconds`
     share = sizes / sizes.sum()
     target_rate = 1.5e9 * ncores   # first guess, FLOP/s
     budget = target_rate * seconds
     chosen, acc = [], 0.0
+    big = int(np.argmax(sizes))
+    if share[big] * total_flops <= 30.0 * 3.5e9 * ncores:
+        chosen.append(big)
     for b in order:
-        if len(chosen) >= 4 and acc >= budget:
+        if len(chosen) >= 5 and acc >= budget:
             break
-        if chosen and acc + share[b] * total_flops > 4 * budget:
-            continue   # keep an outsized block out of a small sample
+        if int(b) in chosen or (chosen and acc + share[b] * total_flops > 4 * budget):
+            continue   # keep a second outsized block out of a small sample
         chosen.append(int(b))
         acc += share[b] * total_flops
     t0 = time.perf_counter()
     sig, st = oracle.opair_sigma(pr, psi, only_out=chosen, return_stats=True)
     dt = time.perf_counter() - t0
+    dims = [(int(layout[b][4]), int(layout[b][5])) for b in chosen]
     return {"value": st["flops"] / dt * 1e-12, "unit": UNIT, "cores": ncores, "kind": "oracle",
             "sample": f"{len(chosen)} of {len(layout)} sigma blocks ({st['flops']:.3e} of {total_flops:.3e} FLOP, "
                       f"{int(st['tasks'])} tasks) in {dt:.1f} s incl. term expansion and intermediates",
-            "seconds": dt, "flops": st["flops"], "blocks": chosen, "sigma": sig}
+            "seconds": dt, "flops": st["flops"], "blocks": chosen, "block_dims": dims, "sigma": sig}
 
 
 def oracle_term_sample(pr, psi, total_flops, seconds, k=0):
@@ -395,7 +400,8 @@ def main():
         for b in blocks:
             o, cnt = int(lay[b][6]), int(lay[b][4] * lay[b][5])
             err = max(err, float(np.abs(got[o:o + cnt] - refs[o:o + cnt]).max()))
-        parity = {"max_abs_err_over_norm": err / nrm, "blocks_checked": len(blocks), "tolerance": 1e-11, "oracle_seconds": chk["seconds"]}
+        parity = {"max_abs_err_over_norm": err / nrm, "blocks_checked": len(blocks), "largest_block": max(chk["block_dims"], key=lambda d: d[0] * d[1]),
+                  "tolerance": 1e-11, "oracle_seconds": chk["seconds"]}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
