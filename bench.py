@@ -50,6 +50,10 @@ def parse():
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="dmrg_plan_options field (copy_mode, split_waves, min_split_stages, max_merged_cols, "
                          "cost_order_only, split_small, release_r_store); repeatable")
+    ap.add_argument("--parallelism", default="replicas", choices=["replicas", "shard"],
+                    help="N > 1: replicas (default; BASELINE.json fixes the path to one GPU: N independent copies, weak scaling) or "
+                         "shard (operator parallelism, PAPER.md:81,162: the terms are partitioned over the ranks and every H psi ends "
+                         "with one NCCL all-reduce of sigma inside dmrg_sigma; strong scaling)")
     ap.add_argument("--sigma-only", type=int, default=0, metavar="N",
                     help="profiling mode: no Davidson, no oracle; N plain dmrg_sigma calls (after one warm-up call) and a short "
                          "JSON line with the per-stage device times -- the command the ncu captures under profiles/ wrap")
@@ -264,7 +268,14 @@ def main():
     ws = int(args.workspace_gib * 2 ** 30) if args.workspace_gib > 0 else int(min(24 * 2 ** 30, 0.25 * free1))
     t0 = time.perf_counter()
     popts = plan_options(args)
+    sharded = args.parallelism == "shard" and world > 1
+    comm = None
+    if sharded:
+        popts.update(shard_rank=rank, shard_count=world)
     plan = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, ws, **popts)
+    if sharded:
+        comm = g.Comm.from_torch_distributed(torch.device("cuda", local))
+        plan.set_comm(comm)
     t_plan = time.perf_counter() - t0
     st = plan.stats()
     n = plan.psi_size
@@ -319,8 +330,17 @@ def main():
     assert res["iters"] == K
     flops_canon = st["canon_flops"]
     flops = st["s1_flops"] + st["s2_flops"]       # executed: what the GEMM launches of one H psi compute (unpadded)
-    thr, ms_step = replicas.job_throughput(flops, ms_total / K, world, "cuda")   # max over ranks
-    value = thr * 1e-12
+    if sharded:
+        # one bond shared by all ranks: the job's work is the SUM of the shards' executed flops, its time the slowest rank's
+        import torch.distributed as dist
+        tot = torch.tensor([flops, flops_canon], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tot)
+        job_flops, job_canon = float(tot[0]), float(tot[1])
+        ms_step = replicas.max_over_ranks(ms_total / K, "cuda")
+        value = job_flops / (ms_step * 1e-3) * 1e-12
+    else:
+        thr, ms_step = replicas.job_throughput(flops, ms_total / K, world, "cuda")   # max over ranks
+        value = thr * 1e-12
 
     # ---- kernel-only H psi (no Davidson vector work) and the roofline of the GEMM kernel --------
     ts = []
@@ -405,15 +425,16 @@ def main():
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic", "config": {"workload": workload_name(args.config, pr), "l2": "inputs larger than L2 (operator store + X workspace stream through every step)",
-                                                "parallelism": "replicas only" if world > 1 else "single GPU",
+                                                "parallelism": ("operator-parallel shards + one NCCL all-reduce of sigma per H psi" if sharded else "replicas only") if world > 1 else "single GPU",
                                                 "psi_size": int(n), "psi_blocks": int(len(pr.layout)), "terms": int(len(pr.term_coef)),
                                                 "tasks": int(st["tasks"]), "chunks": int(st["chunks"])},
                 "clocks": clk, "e2e": e2e, "gpu_launches": int(K * (st["launches"] + 15) + 4),   # GEMM / reduce launches + 15 Davidson vector kernels per step, + hdiag, start-up
                 "roofline": roofline, "cpu_baseline": cpu,
                 "ms_per_hpsi_kernel_only": ms_sigma, "frac_of_fp64_peak_whole_step": value / world / peak_dmma,
-                "canonical_flops_per_hpsi": flops_canon, "canonical_tflops": world * flops_canon / (ms_step * 1e-3) * 1e-12,
+                "canonical_flops_per_hpsi": job_canon if sharded else flops_canon,
+                "canonical_tflops": (job_canon if sharded else world * flops_canon) / (ms_step * 1e-3) * 1e-12,
                 "plan_options": popts,
                 "parity_sampled": parity,
                 "footprint_gb": {"operator_store": ops.device_bytes / 1e9, "plan_and_workspace": st["plan_device_bytes"] / 1e9,
@@ -424,6 +445,8 @@ def main():
                 "context": "paper: ~13-15 TFLOP/s FP64-TC per A100 for the GEMM step at large D (PAPER.md:231); D=14000 on 48 A100-80GB (PAPER.md:17)"}
         print(json.dumps(line))
     plan.destroy()
+    if comm is not None:
+        comm.destroy()
     ops.free()
     if world > 1:
         import torch.distributed as dist

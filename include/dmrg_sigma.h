@@ -302,6 +302,26 @@ int     dmrg_ops_derive(const dmrg_ops* src, const dmrg_op_desc* lin_ops, int32_
                         const int32_t* lin_trans, int32_t nlin, dmrg_ops** out);
 
 /* ---------------------------------------------------------------------------------------------
+ * Operator parallelism over the GPUs of a node: the terms are partitioned over ranks
+ * (dmrg_plan_options.shard_rank / shard_count) and the partial sigma vectors are summed with ONE all-reduce of psi_size
+ * doubles per H psi (the paper: NCCL broadcast of the trial vector + reduce of sigma; here the Davidson vectors are
+ * replicated and deterministic, so the broadcast is not needed).  One process per GPU:
+ *   dmrg_comm_unique_id  rank 0: writes the NCCL unique id (returns its size in bytes, 128; id_out [host]); the caller
+ *                        ships it to the other ranks (torch.distributed, MPI, a file)
+ *   dmrg_comm_create     every rank, on its own device: ncclCommInitRank
+ *   dmrg_plan_set_comm   attaches the communicator to a plan created as shard (rank, world): from then on dmrg_sigma and
+ *                        dmrg_hdiag end with an in-place ncclAllReduce(SUM) on the caller's stream, right behind their
+ *                        last launch, and return COMPLETE results on every rank; dmrg_davidson needs no change.
+ *                        NULL detaches.  The plan borrows the communicator.
+ * NCCL is loaded at run time (the libnccl.so.2 the process already has, e.g. torch's); without it these calls fail
+ * with DMRG_ECUDA and everything single-GPU still works. */
+typedef struct dmrg_comm dmrg_comm;
+int  dmrg_comm_unique_id(void* id_out, int32_t capacity);
+int  dmrg_comm_create(const void* id, int32_t rank, int32_t world, dmrg_comm** out);
+void dmrg_comm_destroy(dmrg_comm* comm);
+int  dmrg_plan_set_comm(dmrg_plan* plan, dmrg_comm* comm);
+
+/* ---------------------------------------------------------------------------------------------
  * Per-stage device timing of the most recent dmrg_sigma with timing enabled (adds CUDA events
  * around each launch; off by default).  dmrg_plan_stage_ms synchronises and returns milliseconds:
  * which = 0 stage 1 (Eq. 11), 1 stage 2 + reduction (Eqs. 12-13), 2 whole call. */

@@ -44,7 +44,8 @@ EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan
            "dmrg_sigma_host", "dmrg_hdiag", "dmrg_davidson", "dmrg_plan_set_timing", "dmrg_plan_stage_ms",
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
            "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
-           "dmrg_ops_join", "dmrg_ops_add_lincombs", "dmrg_ops_derive")
+           "dmrg_ops_join", "dmrg_ops_add_lincombs", "dmrg_ops_derive",
+           "dmrg_comm_unique_id", "dmrg_comm_create", "dmrg_comm_destroy", "dmrg_plan_set_comm")
 
 _lib = None
 
@@ -115,6 +116,14 @@ def lib():
         L.dmrg_ops_add_lincombs.restype = C.c_int
         L.dmrg_ops_derive.argtypes = [vp, vp, i32, vp, vp, vp, vp, i32, C.POINTER(vp)]
         L.dmrg_ops_derive.restype = C.c_int
+        L.dmrg_comm_unique_id.argtypes = [vp, i32]
+        L.dmrg_comm_unique_id.restype = C.c_int
+        L.dmrg_comm_create.argtypes = [vp, i32, i32, C.POINTER(vp)]
+        L.dmrg_comm_create.restype = C.c_int
+        L.dmrg_comm_destroy.argtypes = [vp]
+        L.dmrg_comm_destroy.restype = None
+        L.dmrg_plan_set_comm.argtypes = [vp, vp]
+        L.dmrg_plan_set_comm.restype = C.c_int
         L.dmrg_last_error.restype = C.c_char_p
         L.dmrg_version.restype = C.c_char_p
         _lib = L
@@ -337,6 +346,11 @@ class Plan:
         return {"energy": e.value, "resid": r.value, "iters": it.value, "thetas": thetas[:it.value].copy(),
                 "converged": rc == 0}
 
+    def set_comm(self, comm):
+        """dmrg_plan_set_comm: a sharded plan's dmrg_sigma / dmrg_hdiag then end with the all-reduce over `comm`."""
+        _check(lib().dmrg_plan_set_comm(self._h, comm._h if comm is not None else None))
+        self._comm = comm   # keep it alive: the plan borrows it
+
     def set_timing(self, enable):
         _check(lib().dmrg_plan_set_timing(self._h, 1 if enable else 0))
 
@@ -346,6 +360,49 @@ class Plan:
     def destroy(self):
         if self._h is not None:
             lib().dmrg_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class Comm:
+    """dmrg_comm: the NCCL communicator of the operator-parallel sigma (one process per GPU)."""
+
+    def __init__(self, unique_id, rank, world):
+        self._h = None
+        uid = np.ascontiguousarray(unique_id, dtype=np.uint8)
+        h = C.c_void_p()
+        _check(lib().dmrg_comm_create(_ptr(uid), int(rank), int(world), C.byref(h)))
+        self._h = h
+        self.rank, self.world = int(rank), int(world)
+
+    @staticmethod
+    def unique_id():
+        buf = np.zeros(256, dtype=np.uint8)
+        n = _check_count(lib().dmrg_comm_unique_id(_ptr(buf), len(buf)))
+        return buf[:n].copy()
+
+    @classmethod
+    def from_torch_distributed(cls, device=None):
+        """Rank 0 creates the id, torch.distributed ships it (any backend), every rank joins on its current device."""
+        import torch
+        import torch.distributed as dist
+        rank, world = (dist.get_rank(), dist.get_world_size()) if dist.is_initialized() else (0, 1)
+        uid = cls.unique_id() if rank == 0 else np.zeros(128, dtype=np.uint8)
+        if world > 1:
+            dev = device if (device is not None and dist.get_backend() == "nccl") else "cpu"
+            t = torch.from_numpy(uid.copy()).to(dev)
+            dist.broadcast(t, 0)
+            uid = t.cpu().numpy()
+        return cls(uid, rank, world)
+
+    def destroy(self):
+        if self._h is not None:
+            lib().dmrg_comm_destroy(self._h)
             self._h = None
 
     def __del__(self):

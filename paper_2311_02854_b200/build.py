@@ -10,6 +10,7 @@ SRCS = sorted(glob.glob(os.path.join(HERE, "csrc", "*.cu")))
 DEPS = SRCS + sorted(glob.glob(os.path.join(HERE, "csrc", "*.h"))) + [os.path.join(HERE, "..", "include", "dmrg_sigma.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
+LINK_FLAGS = ["-ldl"]   # comm.cu loads NCCL at run time (dlopen); no link-time dependency on it
 
 
 def stale():
@@ -23,7 +24,7 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRCS
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRCS + LINK_FLAGS
     subprocess.check_call(cmd)
     return LIB
 

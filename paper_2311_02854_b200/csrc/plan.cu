@@ -110,6 +110,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     const bool kTileOrder = pol.tile_order;
     const int kSplitSmall = pol.split_small;
     P->copy_mode = pol.copy_mode;
+    P->shard_rank = pol.shard_rank;
+    P->shard_count = pol.shard_count;
     const bool kReleaseR = pol.release_r_store;
     DMRG_REQUIRE(!P->ops->r_released, "dmrg_plan_create: the R-side blocks of this store were released to an earlier plan (release_r_store)");
     const dmrg_ops* S = P->ops;
@@ -1078,6 +1080,7 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         }
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
     }
+    if (P->comm) { const int rc = comm_all_reduce(P->comm, sigma, P->psi_size, st); if (rc != DMRG_OK) return rc; }   // sharded plan: sum the partial sigmas
     if (P->timing) { DMRG_CUDA(cudaEventRecord(P->ev[2 * ng + 1], st)); P->timing_valid = true; }
     return DMRG_OK;
 }
@@ -1105,6 +1108,7 @@ int dmrg_hdiag(dmrg_plan* P, double* diag, void* cuda_stream) {
     if (P->n_hd_tiles > 0)
         hdiag_kernel<<<(unsigned)P->n_hd_tiles, 256, 0, st>>>(P->d_hd_blocks, P->d_hd_tiles, P->d_hd_items, P->ops->d_values, diag);
     DMRG_CUDA(cudaGetLastError());
+    if (P->comm) return comm_all_reduce(P->comm, diag, P->psi_size, st);
     return DMRG_OK;
 }
 

@@ -20,6 +20,7 @@ enum {
 };
 
 struct DavidsonWs;
+struct dmrg_comm;
 
 struct dmrg_plan {
     const dmrg_ops* ops = nullptr;
@@ -51,8 +52,11 @@ struct dmrg_plan {
     std::vector<cudaEvent_t> ev;   // 2 per group + 2
     bool timing_valid = false;
     DavidsonWs* dav = nullptr;
+    int shard_rank = 0, shard_count = 1;
+    const dmrg_comm* comm = nullptr;   // borrowed: all-reduce of the partial sigma / diagonal of a sharded plan
 };
 
 namespace dmrg {
 void davidson_ws_free(DavidsonWs* ws);
+int comm_all_reduce(const dmrg_comm* C, double* buf, int64_t n, cudaStream_t st);
 }

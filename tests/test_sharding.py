@@ -126,3 +126,36 @@ def test_gpu_partial_sigmas_add_up():
     assert np.abs(acc.cpu().numpy() - orc).max() <= 1e-11 * np.linalg.norm(orc)
     full.destroy()
     ops.free()
+
+
+@pytest.mark.gpu
+def test_gpu_comm_attached_plan_reduces_in_place():
+    """dmrg_comm on one device (world size 1: the only size this box can run): the NCCL communicator is created, attached
+    to a plan created as shard 0 of 1, and dmrg_sigma / dmrg_hdiag / dmrg_davidson go through ncclAllReduce on the caller's
+    stream; results are those of the plain plan.  A communicator that does not match the plan's shard is refused."""
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test needs a CUDA device")
+    pr = _problem()
+    ops, plain = g.load_problem(pr)
+    psi = torch.from_numpy(random_psi(pr.psi_size, 4)).cuda()
+    ref = torch.empty_like(psi)
+    plain.sigma(psi, ref, torch.cuda.current_stream())
+    comm = g.Comm(g.Comm.unique_id(), 0, 1)
+    p = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, shard_rank=0, shard_count=1)
+    p.set_comm(comm)
+    out = torch.empty_like(psi)
+    p.sigma(psi, out, torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    x1, x2 = psi.clone(), psi.clone()
+    r1 = plain.davidson(x1, max_iter=6, max_space=6, tol=0.0, stream=torch.cuda.current_stream())
+    r2 = p.davidson(x2, max_iter=6, max_space=6, tol=0.0, stream=torch.cuda.current_stream())
+    assert r1["energy"] == r2["energy"] and torch.equal(x1, x2)
+    half = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, shard_rank=0, shard_count=2)
+    with pytest.raises(g.DmrgError):
+        half.set_comm(comm)
+    half.destroy()
+    p.destroy()
+    comm.destroy()
+    plain.destroy()
+    ops.free()
