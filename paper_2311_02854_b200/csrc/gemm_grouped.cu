@@ -90,19 +90,14 @@ __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];\n" ::"l"(tmap) : "memory");
 }
 
-// fold alpha into the smaller fragment set; |alpha| = 1 flips the sign bit on the integer pipe
-// instead of spending an FP64 issue slot
+// fold alpha into the A fragments (always A, whatever the fragment counts: the rounding of alpha * a * b must not depend
+// on the tile specialisation or the kernel variant); |alpha| = 1 flips the sign bit on the integer pipe instead of spending
+// an FP64 issue slot
 template <int FM, int FN>
 __device__ __forceinline__ void scale_frags(double (&af)[FM], double (&bf)[FN], int mode, double alpha) {
-    if (FM <= FN) {
 #pragma unroll
-        for (int i = 0; i < FM; i++)
-            af[i] = mode == 1 ? __hiloint2double(__double2hiint(af[i]) ^ 0x80000000, __double2loint(af[i])) : af[i] * alpha;
-    } else {
-#pragma unroll
-        for (int j = 0; j < FN; j++)
-            bf[j] = mode == 1 ? __hiloint2double(__double2hiint(bf[j]) ^ 0x80000000, __double2loint(bf[j])) : bf[j] * alpha;
-    }
+    for (int i = 0; i < FM; i++)
+        af[i] = mode == 1 ? __hiloint2double(__double2hiint(af[i]) ^ 0x80000000, __double2loint(af[i])) : af[i] * alpha;
 }
 
 // ---- producer, cp.async path ----------------------------------------------------------------------------
@@ -497,9 +492,14 @@ constexpr size_t smem_bytes(int nst) {
 //   V0 64x64, 2x2 consumer warps, BK = 32, 2 stages (72 KB), 128 registers, no spills -> 3 CTAs/SM.  Measured
 //      against BK = 16 / 2 stages / 96 registers / 4 CTAs/SM: cfg 5 +1.7 %, cfg 3 +1.0 %, cfg 4 -1.6 %, cfg 2 -2.2 %;
 //      3 stages x BK = 16, 4 stages, a second producer warp, double-buffered fragments: all slower.
+//   V1 the same tile with 4x2 consumer warps of 16x32 (8 fragments each, 8 DMMA per 6 LDS.64 per k-step), 72 registers,
+//      still 3 CTAs/SM but twice the resident warps: better on launches whose tiles are mostly ragged / short (cfg 2 +4 %,
+//      cfg 4 +3 %), worse on well-filled ones (cfg 5 -2 %: more shared-memory operand traffic per DMMA).  The planner picks
+//      per launch from the mean tile fill (dmrg_plan_options.consumer_warps).
 #define V0 grouped_gemm_kernel<64, 64, 2, 2, 2, 128>
-constexpr int V0_T = 32 * 5;
-constexpr size_t V0_S = smem_bytes<64, 64>(2);
+#define V1 grouped_gemm_kernel<64, 64, 4, 2, 2, 72>
+constexpr int V0_T = 32 * 5, V1_T = 32 * 9;
+constexpr size_t V0_S = smem_bytes<64, 64>(2), V1_S = smem_bytes<64, 64>(2);
 
 }  // namespace
 
@@ -507,6 +507,7 @@ int gemm_init() {
     static bool done = false;
     if (done) return DMRG_OK;
     DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V1_S));
     done = true;
     return DMRG_OK;
 }
@@ -517,6 +518,7 @@ int launch_grouped_gemm(int variant, int copy_mode, const Job* jobs, const Seg* 
     const unsigned g = (unsigned)ntiles;
     switch (variant) {
         case 0: V0<<<g, V0_T, V0_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
+        case 1: V1<<<g, V1_T, V1_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
     const cudaError_t e = cudaGetLastError();

@@ -73,6 +73,11 @@ constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are
 // DESIGN.md section 9 was taken with 4 resident CTAs per SM; the BK = 32 kernel keeps 3, the unit is kept so that the
 // recorded numbers stay comparable)
 constexpr double kCtaSlots = 148.0 * 4;
+// Kernel variant per launch (measured): the 8-consumer-warp kernel wins where tiles are short-lived or
+// ragged -- stage 1 when the mean K of its tiles is below kMeanKFor8Warps (a tile is then a couple of pipeline stages: latency,
+// not the pipe, is what it waits for), stage 2 when the mean fill of its 64 x 64 tiles is below kFillFor8Warps.
+constexpr double kStagesFor8Warps = 160.0;   // stage 1: mean K (k-columns) per tile
+constexpr double kFillFor8Warps = 0.72;      // stage 2: mean tile fill
 
 struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     int64_t workspace_bytes;
@@ -83,6 +88,7 @@ struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     int split_small;
     bool release_r_store;
     int shard_rank, shard_count;
+    int consumer_warps;   // 0 = per launch from the mean tile fill, 4 or 8 = forced
 };
 
 static PlanPolicy make_policy(const dmrg_plan_options* o) {
@@ -95,6 +101,7 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
     p.release_r_store = o && o->release_r_store;
+    p.consumer_warps = (o && (o->consumer_warps == 4 || o->consumer_warps == 8)) ? o->consumer_warps : 0;
     p.shard_count = (o && o->shard_count > 1) ? o->shard_count : 1;
     p.shard_rank = (o && o->shard_count > 1) ? o->shard_rank : 0;
     return p;
@@ -338,7 +345,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     // The chunks are planned independently of each other by all host threads, each into its own ChunkOut with
     // chunk-local job / segment / tensor-map indices and pack offsets; they are then appended in chunk order (the
     // result does not depend on the thread count).
-    struct TileList { std::vector<Tile> tiles; size_t nbig = 0; };   // sorted tiles of one stage; [0, nbig) = large-block jobs (split_small)
+    struct TileList { std::vector<Tile> tiles; size_t nbig = 0; double frag_area = 0, cost = 0; };   // frag_area: 8x8 fragments of the tiles x 64   // sorted tiles of one stage; [0, nbig) = large-block jobs (split_small)
     struct ChunkOut {
         std::vector<Job> jobs;
         std::vector<Seg> segs;
@@ -379,7 +386,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                    }) - r.begin();
         out.nbig = nbig;
         out.tiles.reserve(r.size());
-        for (auto& x : r) out.tiles.push_back(x.t);
+        for (auto& x : r) { out.tiles.push_back(x.t); out.frag_area += frag_area(x.t.rows, x.t.cols); out.cost += x.cost; }
     };
 
     auto build_chunk = [&](int64_t ch, ChunkOut& O) -> int {
@@ -724,7 +731,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     std::vector<PackDesc> packs;   // packed R store (stage-1 B operands), filled on the device after upload
     std::vector<size_t> pack_segs;  // segments whose b_off is relative to the packed store
     MapTable maps;
-    int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0;
+    int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, tiles8 = 0;
+    double fill_acc1 = 0, fill_acc2 = 0, cost_acc1 = 0, cost_acc2 = 0;
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
     for (int64_t ch = 0; ch < nchunks; ch++) {
         ChunkOut& O = outs[ch];
@@ -753,10 +761,19 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
             PlanGroup grp{stage, (int)P->launches.size(), 0};
             size_t i = 0;
             const size_t n = tl->tiles.size();
+            // kernel variant of this launch: 8 consumer warps when the tiles are mostly ragged (mean fill of the 64 x 64
+            // tiles below kFillFor8Warps), 4 consumer warps with 32 x 32 warp tiles otherwise
+            const double fill = n ? tl->frag_area / (4096.0 * (double)n) : 1.0;
+            const double mean_stages = n ? tl->cost / (double)n : 0.0;   // pipeline stages (+1) per tile
+            const bool want8 = stage == 1 ? mean_stages < kStagesFor8Warps : fill < kFillFor8Warps;
+            const int variant = pol.consumer_warps == 8 ? 1 : (pol.consumer_warps == 4 ? 0 : (want8 ? 1 : 0));
+            (stage == 1 ? cost_acc1 : cost_acc2) += tl->cost;
+            (stage == 1 ? fill_acc1 : fill_acc2) += tl->frag_area;
+            if (variant == 1) tiles8 += (int64_t)n;
             auto push_range = [&](size_t lo, size_t hi) {
                 while (lo < hi) {   // grid.x limit: split very long lists
                     const size_t cnt = std::min<size_t>(hi - lo, (size_t)1 << 30);
-                    P->launches.push_back({0, stage, (int64_t)tiles.size(), (int64_t)cnt});
+                    P->launches.push_back({variant, stage, (int64_t)tiles.size(), (int64_t)cnt});
                     for (size_t j = lo; j < lo + cnt; j++) { Tile t = tl->tiles[j]; t.job += (int32_t)job_base; tiles.push_back(t); }
                     lo += cnt;
                 }
@@ -812,6 +829,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     P->xws_elems = std::max<int64_t>(ws_peak, 2);
     P->stats[ST_XWS_ELEMS] = (double)P->xws_elems;
     P->stats[ST_TENSOR_MAPS] = (double)maps.descs.size();
+    P->stats[ST_S1_FILL] = s1_tiles ? fill_acc1 / (4096.0 * s1_tiles) : 0.0;
+    P->stats[ST_S2_FILL] = s2_tiles ? fill_acc2 / (4096.0 * s2_tiles) : 0.0;
+    P->stats[ST_TILES_8W] = (double)tiles8;
+    P->stats[ST_S1_STAGES] = s1_tiles ? cost_acc1 / s1_tiles - 1.0 : 0.0;
+    P->stats[ST_S2_STAGES] = s2_tiles ? cost_acc2 / s2_tiles - 1.0 : 0.0;
     P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
                                          hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +
                                          8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems);
