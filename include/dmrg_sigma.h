@@ -236,6 +236,25 @@ int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_spac
                   void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * dmrg_dots_static: out[i] = sum_e V[i*stride + e] * w[e], i < m -- the block of dot products every Davidson
+ * iteration needs (G_ik = b_i . w_k, the Gram-Schmidt coefficients, |r|^2; PAPER.md:162 keeps them on CPU rank 0),
+ * for callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc).  Same two kernels, same fixed grid and summation tree as inside dmrg_davidson (bitwise the same
+ * result for the same data), but the per-CTA partial sums live in a file-scope device array of
+ * DMRG_DOTS_STATIC_MAX_VECTORS x 592 doubles (151552 bytes, held by every GPU that loads the library until exit)
+ * instead of a cudaMalloc'ed workspace: the call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   V [device] m vectors of n doubles, vector i at V + i*stride (stride >= n; ignored for m = 1); w [device] n doubles;
+ *   out [device] m doubles, overwritten; m in [1, DMRG_DOTS_STATIC_MAX_VECTORS], else DMRG_EINVAL (the message names
+ *   the limit); n >= 0 (n = 0 gives zeros).
+ * Asynchronous on `cuda_stream`, on the current device.  All calls on one GPU share the one scratch array: calls that
+ * may overlap on the GPU (different streams, no dependency between them) RACE on it -- keep them on one stream or
+ * order them with events.  Every slot a call reads it has written itself, so nothing carries over between calls.
+ */
+#define DMRG_DOTS_STATIC_MAX_VECTORS 32
+int dmrg_dots_static(const double* V, int64_t stride, int32_t m, const double* w, int64_t n, double* out,
+                     void* cuda_stream);
+
+/* ---------------------------------------------------------------------------------------------
  * dmrg_renormalize: the renormalization step that follows the Davidson step at every bond (Eq. 8),
  *     [O_new]_{r'r} = sum_{l'c'} sum_{lc} zeta A^{c'}_{l'r'} [O^blk]_{l'l} [O^site]_{c'c} A^{c}_{lr},
  * for every operator the enlarged block carries, evaluated block by block as Eqs. (15)-(18)

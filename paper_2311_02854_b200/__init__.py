@@ -45,7 +45,8 @@ EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
            "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
            "dmrg_ops_join", "dmrg_ops_add_lincombs", "dmrg_ops_derive",
-           "dmrg_comm_unique_id", "dmrg_comm_create", "dmrg_comm_destroy", "dmrg_plan_set_comm")
+           "dmrg_comm_unique_id", "dmrg_comm_create", "dmrg_comm_destroy", "dmrg_plan_set_comm", "dmrg_dots_static")
+DOTS_STATIC_MAX_VECTORS = 32
 
 _lib = None
 
@@ -124,6 +125,8 @@ def lib():
         L.dmrg_comm_destroy.restype = None
         L.dmrg_plan_set_comm.argtypes = [vp, vp]
         L.dmrg_plan_set_comm.restype = C.c_int
+        L.dmrg_dots_static.argtypes = [vp, i64, i32, vp, i64, vp, vp]
+        L.dmrg_dots_static.restype = C.c_int
         L.dmrg_last_error.restype = C.c_char_p
         L.dmrg_version.restype = C.c_char_p
         _lib = L
@@ -436,6 +439,14 @@ def renormalize(store, side, sec_new, wblocks, wvalues, new_ops, term_ptr, term_
     _check(lib().dmrg_renormalize(store._h, int(side), _ptr(sn), len(sn), _ptr(wb), len(wb), _ptr(wv), len(wv), _ptr(od), len(od),
                                   _ptr(tp), _ptr(td), _ptr(so), _ptr(sp), len(so), _ptr(opt), _stream_ptr(stream), C.byref(h), _ptr(st)))
     return OpsStore._from_handle(h), {k: (float(st[k][0]) if st.dtype[k].kind == "f" else int(st[k][0])) for k in st.dtype.names}
+
+
+def dots_static(V, w, out, stream=None):
+    """dmrg_dots_static: out[i] = V[i] . w for the rows of the 2-D CUDA float64 tensor V (m <= DOTS_STATIC_MAX_VECTORS);
+    allocates nothing -- the per-CTA partial sums live in the library's static device scratch."""
+    m, n = (1, V.shape[0]) if V.dim() == 1 else V.shape
+    stride = V.stride(0) if V.dim() == 2 else n
+    _check(lib().dmrg_dots_static(_ptr(V), int(stride), int(m), _ptr(w), int(n), _ptr(out), _stream_ptr(stream)))
 
 
 def fp64_peak_tflops(which, ms=200.0, stream=None):

@@ -4,6 +4,7 @@
 // O(n) work is done by the kernels below, and the host only sees the m x m subspace matrix.
 // Reductions use a fixed grid and a fixed summation tree, so results are reproducible run to run.
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <new>
 
@@ -282,4 +283,56 @@ extern "C" int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32
         dmrg::set_error("dmrg_davidson: out of host memory");
         return DMRG_ENOMEM;
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// dmrg_dots_static: the Davidson dot-product pair (dots_partial_kernel + dots_final_kernel above) for callers that
+// may not allocate: the per-CTA partial sums, which dmrg_davidson keeps in a cudaMalloc'ed workspace, live in a
+// file-scope device array instead.  In HOST code `g_dots_scratch` is only a stand-in for the symbol, not a device
+// address: the address is looked up once per device with cudaGetSymbolAddress and handed to the kernels.
+namespace dmrg {
+
+constexpr int DOTS_STATIC_MAX_VECTORS = DMRG_DOTS_STATIC_MAX_VECTORS;
+constexpr int DOTS_STATIC_MAX_DEVICES = 64;
+static __device__ __align__(256) double g_dots_scratch[(size_t)DOTS_STATIC_MAX_VECTORS * RED_GRID];   // 151552 bytes per GPU
+
+static std::atomic<double*> g_dots_scratch_ptr[DOTS_STATIC_MAX_DEVICES];   // device address of g_dots_scratch per device ordinal (null = not looked up yet)
+
+// Device address of the scratch array on the CURRENT device (looked up on first use there; idempotent, so two threads
+// racing on the first call store the same pointer).  No allocation: the array is part of the loaded module.
+static int dots_scratch_address(double** out) {
+    int dev = -1;
+    DMRG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= DOTS_STATIC_MAX_DEVICES) { set_error("dmrg_dots_static: device ordinal %d is outside [0, %d)", dev, DOTS_STATIC_MAX_DEVICES); return DMRG_EINVAL; }
+    double* p = g_dots_scratch_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        DMRG_CUDA(cudaGetSymbolAddress((void**)&p, g_dots_scratch));
+        if (!p) { set_error("dmrg_dots_static: cudaGetSymbolAddress returned a null address on device %d", dev); return DMRG_ECUDA; }
+        g_dots_scratch_ptr[dev].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return DMRG_OK;
+}
+
+}  // namespace dmrg
+
+extern "C" int dmrg_dots_static(const double* V, int64_t stride, int32_t m, const double* w, int64_t n, double* out, void* cuda_stream) {
+    using namespace dmrg;
+    if (!V || !w || !out) { set_error("dmrg_dots_static: null pointer"); return DMRG_EINVAL; }
+    if (m < 1 || m > DOTS_STATIC_MAX_VECTORS) {
+        set_error("dmrg_dots_static: m = %d vectors is outside [1, %d] (the static scratch holds %d x %d partial sums; use dmrg_davidson's own workspace path for more)",
+                  m, DOTS_STATIC_MAX_VECTORS, DOTS_STATIC_MAX_VECTORS, RED_GRID);
+        return DMRG_EINVAL;
+    }
+    if (n < 0 || (m > 1 && stride < n)) { set_error("dmrg_dots_static: bad n = %lld / stride = %lld", (long long)n, (long long)stride); return DMRG_EINVAL; }
+    double* scratch = nullptr;
+    const int rc = dots_scratch_address(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // every partial sum dots_final_kernel reads (m rows x RED_GRID CTAs) is written by dots_partial_kernel in this very
+    // call -- CTAs with an empty slice store 0 -- so nothing left behind by an earlier call is ever read and nothing needs clearing
+    dots_partial_kernel<<<RED_GRID, RED_BLOCK, 0, st>>>(V, stride, m, w, n, scratch);
+    dots_final_kernel<<<(m + 63) / 64, 64, 0, st>>>(scratch, m, out);
+    DMRG_CUDA(cudaGetLastError());
+    return DMRG_OK;
 }
