@@ -20,10 +20,15 @@ One of the two factors is always a single site; the block's complementary
 operators are formed from its carried A, B by  P_pq = sum_{s<r} V[p,q,s,r] A_sr^T,
 Q_ps = sum_{q,r} V[p,q,s,r] B_qr  (definitions).  Products inside a
 block are carried as their own renormalized operators, never recomposed.
+
+Every "transpose" below is the Hermitian conjugate (a_p = (a+_p)^H): the plain transpose for the real
+spin-free integrals, the conjugate transpose for the complex integrals of a spin-orbit Hamiltonian
+(PAPER.md:97), for which the bases carry N only (ints.sym == "N"), the isometries are complex and a
+single site has the three sectors N = 0, 1, 2 of dimensions 1, 2, 1.
 """
 import numpy as np
 
-from .conventions import SITE_Q
+from .conventions import site_q
 from .sectors import full_dim, kept_dims
 from .siteops import SiteOps
 
@@ -47,7 +52,7 @@ class RBlock:
 
     # ---- derived operators (block-sparse dicts) ------------------------
     def transpose(self, blocks):
-        return {(c, r): m.T for (r, c), m in blocks.items()}
+        return {(c, r): m.conj().T for (r, c), m in blocks.items()}
 
     def Bfull(self, p, t):
         return self.ops[("B", p, t)] if p <= t else self.transpose(self.ops[("B", t, p)])
@@ -61,7 +66,7 @@ class RBlock:
                 v = ints.V(p, q, s, r)
                 if v != 0.0:
                     for (rr, cc), m in self.ops[("A", s, r)].items():
-                        _acc(out, (cc, rr), v * m.T)
+                        _acc(out, (cc, rr), v * m.conj().T)
         return out
 
     def compl_Q(self, p, s, ints):
@@ -87,12 +92,28 @@ def _acc(d, key, m):
 def site_block(k, ints, outside):
     """Exact single-site block with all carried operators (S_p for p in `outside`)."""
     so = SiteOps(k, ints)
-    blk = RBlock(so.labels, list(SITE_Q), [1, 1, 1, 1])
+    sym = getattr(ints, "sym", "NSz")
+    a, b = so.labels
+    if sym == "NSz":
+        where = [(0, 0), (1, 0), (2, 0), (3, 0)]          # site state -> (sector, position inside it)
+        blk = RBlock(so.labels, list(site_q(sym)), [1, 1, 1, 1])
+        blk.dets = {0: [0], 1: [1 << b], 2: [1 << a], 3: [(1 << a) | (1 << b)]}
+    else:
+        where = [(0, 0), (1, 0), (1, 1), (2, 0)]
+        blk = RBlock(so.labels, [(0, 0), (1, 0), (2, 0)], [1, 2, 1])
+        blk.dets = {0: [0], 1: [1 << b, 1 << a], 2: [(1 << a) | (1 << b)]}
 
     def sparse(m):
-        return {(i, j): np.array([[m[i, j]]]) for i in range(4) for j in range(4) if m[i, j] != 0.0}
+        out = {}
+        for i in range(4):
+            for j in range(4):
+                if m[i, j] != 0.0:
+                    (si, pi), (sj, pj) = where[i], where[j]
+                    if (si, sj) not in out:
+                        out[(si, sj)] = np.zeros((blk.dims[si], blk.dims[sj]), dtype=np.asarray(m).dtype)
+                    out[(si, sj)][pi, pj] = m[i, j]
+        return out
 
-    a, b = so.labels
     for p in so.labels:
         blk.ops[("C", p)] = sparse(so.C(p))
     blk.ops[("A", a, b)] = sparse(so.A(a, b))
@@ -103,9 +124,8 @@ def site_block(k, ints, outside):
     for p in outside:
         blk.ops[("S", p)] = sparse(so.S(p))
     blk.ops[("H",)] = sparse(so.H())
-    # determinant bookkeeping (tiny-K pins): sector i = site state i, one determinant each
-    blk.dets = {0: [0], 1: [1 << b], 2: [1 << a], 3: [(1 << a) | (1 << b)]}
-    blk.E = {i: np.ones((1, 1)) for i in range(4)}
+    # determinant bookkeeping (tiny-K pins): the site states of each sector, one determinant each
+    blk.E = {i: np.eye(d) for i, d in enumerate(blk.dims)}
     return blk
 
 
@@ -151,7 +171,9 @@ class _Enlarged:
                 (b, co) = self.offset[(cl, cr)]
                 k = np.kron(ml, mr) * coef
                 if (a, b) not in out:
-                    out[(a, b)] = np.zeros((self.dims[a], self.dims[b]))
+                    out[(a, b)] = np.zeros((self.dims[a], self.dims[b]), dtype=k.dtype)
+                elif out[(a, b)].dtype != k.dtype and k.dtype.kind == "c":
+                    out[(a, b)] = out[(a, b)].astype(k.dtype)
                 out[(a, b)][ro:ro + k.shape[0], co:co + k.shape[1]] += k
 
 
@@ -164,6 +186,8 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
     rng: numpy Generator for the isometries; rotate=True applies a random orthogonal
     rotation even when nothing is truncated."""
     assert left.norb == 1 or right.norb == 1
+    sym = getattr(ints, "sym", "NSz")
+    cplx = np.dtype(getattr(ints, "dtype", np.float64)).kind == "c"
     if site_side is None:
         site_side = "right" if right.norb == 1 else "left"
     site_is_right = site_side == "right"
@@ -245,10 +269,10 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
     m_new = left.norb + right.norb
     if D is None:
         rest = K - m_new
-        keep = [d if full_dim(rest, N_tot - q[0], twoSz_tot - q[1]) > 0 else 0
+        keep = [d if full_dim(rest, N_tot - q[0], twoSz_tot - q[1], sym) > 0 else 0
                 for q, d in zip(E.sectors, E.dims)]
     else:
-        keep = list(kept_dims(E.sectors, E.dims, m_new, K, N_tot, twoSz_tot, D, force_dmax))
+        keep = list(kept_dims(E.sectors, E.dims, m_new, K, N_tot, twoSz_tot, D, force_dmax, sym))
     W = {}
     new_secs, new_dims, remap = [], [], {}
     for i, (q, d, k) in enumerate(zip(E.sectors, E.dims, keep)):
@@ -259,6 +283,8 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
             W[i] = None
         else:
             g = rng.standard_normal((d, d))
+            if cplx:
+                g = g + 1j * rng.standard_normal((d, d))
             qmat, _ = np.linalg.qr(g)
             W[i] = qmat[:, :k]
         remap[i] = len(new_secs)
@@ -269,7 +295,7 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
     # (old-block sector, site state) -> new sector, rows of the kept isometry W (identity where nothing is rotated)
     nb.site_tensor = []
     for (il, ir), (a, off) in sorted(E.offset.items()):
-        if a not in remap:
+        if a not in remap or sym != "NSz":   # (the renormalization step is built for the N, Sz bases only)
             continue
         d = left.dims[il] * right.dims[ir]
         Wa = np.eye(E.dims[a]) if W[a] is None else W[a]
@@ -280,7 +306,7 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
         for (a, b), m in blocks.items():
             if a not in remap or b not in remap:
                 continue
-            x = m if W[a] is None else W[a].T @ m
+            x = m if W[a] is None else W[a].conj().T @ m
             x = x if W[b] is None else x @ W[b]
             out[(remap[a], remap[b])] = x
         nb.ops[key] = out
@@ -299,7 +325,7 @@ def merge(left, right, ints, outside, K, N_tot, twoSz_tot, D, rng=None, rotate=F
                 dets += [dl | dr for dl in left.dets[il] for dr in right.dets[ir]]
                 mats.append(np.kron(left.E[il], right.E[ir]))
             nr = sum(m.shape[0] for m in mats)
-            Ee = np.zeros((nr, E.dims[a]))
+            Ee = np.zeros((nr, E.dims[a]), dtype=np.result_type(*[m.dtype for m in mats]))
             r0 = c0 = 0
             for m in mats:
                 Ee[r0:r0 + m.shape[0], c0:c0 + m.shape[1]] = m

@@ -9,6 +9,15 @@ Quantum numbers q = (N, 2Sz).
 import numpy as np
 
 SITE_Q = ((0, 0), (1, -1), (1, 1), (2, 0))  # (N, 2Sz) of site states 0..3
+# Spin-orbit Hamiltonians ("the spin projection is no longer a good quantum number"): only U(1)_N is
+# kept, every 2Sz label is 0 and the two singly occupied site states share the sector N = 1 (the "two-by-two" dot blocks).
+SITE_Q_N = ((0, 0), (1, 0), (1, 0), (2, 0))
+
+
+def site_q(sym):
+    """(N, 2Sz) labels of the four site states under symmetry `sym`: "NSz" (U(1)_N x U(1)_Sz) or "N" (U(1)_N only)."""
+    assert sym in ("NSz", "N")
+    return SITE_Q if sym == "NSz" else SITE_Q_N
 
 
 def site_annihilators():
@@ -32,6 +41,9 @@ class SpinOrbitalIntegrals:
 
     <PQ|RS> = (pr|qs) d(sP,sR) d(sQ,sS);  V = <PQ|RS> - <PQ|SR>.
     """
+
+    sym = "NSz"       # symmetry the bases built from these integrals carry
+    dtype = np.float64
 
     def __init__(self, h, eri):
         self.h_sp = np.asarray(h, dtype=np.float64)
@@ -91,3 +103,36 @@ class SpinOrbitalIntegrals:
             for sq in (0, 1):
                 coul[sp::2, sq::2, sp::2, sq::2] = e
         return coul - coul.transpose(0, 1, 3, 2)
+
+
+class GeneralSpinOrbitalIntegrals:
+    """Complex Hermitian h[P,Q] and V[P,Q,R,S] = <PQ||RS> given directly over spin orbitals, with no spin selection
+    rule: the Hamiltonian of Eq. (2) "including spin-orbit couplings".  Hermiticity:
+    h[P,Q] = conj(h[Q,P]), V[P,Q,R,S] = conj(V[R,S,P,Q]); antisymmetry in (P,Q) and in (R,S).  Dense storage
+    ((2K)^4 complex numbers): for the small and medium K of the spin-orbit cases."""
+
+    sym = "N"
+    dtype = np.complex128
+
+    def __init__(self, h, V):
+        self.h_so = np.asarray(h, dtype=np.complex128)
+        self.Vt = np.asarray(V, dtype=np.complex128)
+        self.K = self.h_so.shape[0] // 2
+
+    def h(self, P, Q):
+        return complex(self.h_so[P, Q])
+
+    def V(self, P, Q, R, S):
+        return complex(self.Vt[P, Q, R, S])
+
+    def V_pq(self, P, Q):
+        return self.Vt[P, Q, :, :]
+
+    def V_pt(self, P, T):
+        return self.Vt[P, :, T, :]
+
+    def dense_h(self):
+        return self.h_so
+
+    def dense_V(self):
+        return self.Vt

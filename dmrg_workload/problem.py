@@ -14,6 +14,13 @@ def random_psi(n, seed):
     return x / np.linalg.norm(x)
 
 
+def random_psi_z(n, seed):
+    """Complex start vector for the spin-orbit problems: n complex numbers, unit 2-norm."""
+    rng = np.random.Generator(np.random.Philox(seed))
+    x = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    return x / np.linalg.norm(x)
+
+
 def make_blocked_problem(K, nL, N_tot, twoSz_tot=0, D=None, seed=1, banded=False, rotate=False,
                          force_dmax=True, track=False, ints=None):
     """Honest blocking (cfg 1-2, tiny pins): L = orbitals [0,nL), dots nL, nL+1, R = the rest."""
@@ -41,8 +48,9 @@ def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False,
     operator is Hermitian but is NOT a projected physical Hamiltonian."""
     ints = ints if ints is not None else make_integrals(K, seed, banded=banded)
     part = Partition(K, nL)
-    secL = block_sector_model(nL, K, N_tot, twoSz_tot, D)
-    secR = block_sector_model(K - nL - 2, K, N_tot, twoSz_tot, D)
+    sym = getattr(ints, "sym", "NSz")
+    secL = block_sector_model(nL, K, N_tot, twoSz_tot, D, sym)
+    secR = block_sector_model(K - nL - 2, K, N_tot, twoSz_tot, D, sym)
     tt = TermTable(part, ints)
     dmax = max(max(s[2] for s in secL), max(s[2] for s in secR))
     pr = assemble(tt, secL, secR, None, N_tot, twoSz_tot, direct_seed=None if structure_only else seed + 104729,
@@ -97,9 +105,9 @@ def term_subset_problem(pr, term_ids):
     q.ops = new_ops
     q.lin_ptr = np.array(lin_ptr, dtype=np.int64)
     q.lin_op = np.array(lin_op, dtype=np.int32)
-    q.lin_coef = np.array(lin_coef, dtype=np.float64)
+    q.lin_coef = np.array(lin_coef, dtype=pr.lin_coef.dtype)
     q.term_idx = ti
-    q.term_coef = np.array(pr.term_coef[term_ids], dtype=np.float64)
+    q.term_coef = np.array(pr.term_coef[term_ids], dtype=pr.term_coef.dtype)
     return q
 
 
@@ -129,6 +137,6 @@ def determinant_map(pr):
                 vals += list(M[k, nz])
                 k += 1
     dets = np.array(sorted(det_index, key=det_index.get), dtype=np.uint64)
-    P = np.zeros((len(dets), pr.psi_size))
+    P = np.zeros((len(dets), pr.psi_size), dtype=np.result_type(np.float64, *[np.asarray(v).dtype for v in vals[:1]], bL.E[0].dtype if 0 in bL.E else np.float64, pr.dtype))
     P[rows, cols] = vals
     return dets, P

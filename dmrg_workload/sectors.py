@@ -12,8 +12,10 @@ from math import comb
 import numpy as np
 
 
-def full_dim(m, N, twoSz):
-    """Number of determinants with (N, 2Sz) on m spatial orbitals."""
+def full_dim(m, N, twoSz, sym="NSz"):
+    """Number of determinants with (N, 2Sz) on m spatial orbitals (sym "N": with N electrons, any spin)."""
+    if sym == "N":
+        return comb(2 * m, N) if (0 <= N <= 2 * m and twoSz == 0) else 0
     if (N + twoSz) % 2:
         return 0
     na, nb = (N + twoSz) // 2, (N - twoSz) // 2
@@ -58,7 +60,7 @@ def _round_lr(x, cap, total):
     return d
 
 
-def kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D, force_dmax=True):
+def kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D, force_dmax=True, sym="NSz"):
     """qs: list of (N, 2Sz); avail: available states per q in the (enlarged) basis.
 
     Returns integer kept dimensions (0 = sector dropped)."""
@@ -66,7 +68,7 @@ def kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D, force_dmax=True):
     big = 1 << 40
     avail = np.asarray([min(int(a), big) for a in avail], dtype=np.int64)
     m_rest = K - m_block
-    comp = np.array([min(full_dim(m_rest, N_tot - N, twoSz_tot - s), big) for (N, s) in qs], dtype=np.int64)
+    comp = np.array([min(full_dim(m_rest, N_tot - N, twoSz_tot - s, sym), big) for (N, s) in qs], dtype=np.int64)
     cap = np.minimum(avail, comp)
     total = int(min(D, cap.sum()))
     if cap.sum() <= D:
@@ -101,24 +103,25 @@ def kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D, force_dmax=True):
     return _round_lr(x, cap, total)
 
 
-def block_sector_model(m_block, K, N_tot, twoSz_tot, D):
+def block_sector_model(m_block, K, N_tot, twoSz_tot, D, sym="NSz"):
     """Final sector table of a block of m_block orbitals (direct-fill configs)."""
     qs, avail = [], []
     for N in range(0, 2 * m_block + 1):
-        for s in range(-m_block, m_block + 1):
-            fd = full_dim(m_block, N, s)
+        for s in (range(-m_block, m_block + 1) if sym == "NSz" else (0,)):
+            fd = full_dim(m_block, N, s, sym)
             if fd > 0:
                 qs.append((N, s))
                 avail.append(fd)
-    d = kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D)
+    d = kept_dims(qs, avail, m_block, K, N_tot, twoSz_tot, D, sym=sym)
     return [(q[0], q[1], int(x)) for q, x in zip(qs, d) if x > 0]
 
 
-def psi_layout(secL, secR, N_tot, twoSz_tot):
+def psi_layout(secL, secR, N_tot, twoSz_tot, sym="NSz"):
     """Block table of psi/sigma: rows (iL, c1, c2, iR, dL, dR, offset), sorted by
     (iR, c1, c2, iL) so that all blocks sharing q_R form one contiguous row panel
     (each block is a dense row-major dL x dR matrix)."""
-    from .conventions import SITE_Q
+    from .conventions import site_q
+    SITE_Q = site_q(sym)
     idxL = {(s[0], s[1]): i for i, s in enumerate(secL)}
     rows = []
     off = 0

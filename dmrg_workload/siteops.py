@@ -35,7 +35,7 @@ class SiteOps:
         return self.ints.V(p, q, s, r) * (self.ann[r] @ self.ann[s])
 
     def Q(self, p, s):  # sum_{q,r in X} V[p,q,s,r] a+_q a_r
-        out = np.zeros((4, 4))
+        out = np.zeros((4, 4), dtype=self.ints.dtype)
         for q in self.labels:
             for r in self.labels:
                 v = self.ints.V(p, q, s, r)
@@ -44,7 +44,7 @@ class SiteOps:
         return out
 
     def S(self, p):  # sum_q h_pq/2 a_q + sum_{q; s<r} V[p,q,s,r] a+_q a_r a_s
-        out = np.zeros((4, 4))
+        out = np.zeros((4, 4), dtype=self.ints.dtype)
         s, r = self.labels
         for q in self.labels:
             out += 0.5 * self.ints.h(p, q) * self.ann[q]
@@ -54,7 +54,7 @@ class SiteOps:
         return out
 
     def H(self):  # Eq. (2) restricted to the site
-        out = np.zeros((4, 4))
+        out = np.zeros((4, 4), dtype=self.ints.dtype)
         X = self.labels
         for p in X:
             for q in X:

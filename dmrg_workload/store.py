@@ -19,8 +19,10 @@ from .conventions import SITE_Q, spin_of
 KIND = {"H": 0, "C": 1, "A": 2, "B": 3, "P": 4, "Q": 5, "S": 6, "LIN": 7}
 
 
-def op_charge(op):
-    """(dN, d2Sz) of a stored operator."""
+def op_charge(op, sym="NSz"):
+    """(dN, d2Sz) of a stored operator; sym "N": only dN, d2Sz = 0."""
+    if sym == "N":
+        return (op_charge(op)[0], 0)
     k = op.kind
     if k == "H":
         return (0, 0)
@@ -51,6 +53,7 @@ class Problem:
         self.site_ops = self.site_parity = None
         self.term_coef = self.term_idx = None
         self.N_tot = self.twoSz_tot = 0
+        self.sym, self.dtype = "NSz", np.dtype(np.float64)   # "N" / complex128 for spin-orbit problems (psi_size counts complex numbers then)
         self.layout = None
         self.psi_size = 0
         self.meta = {}
@@ -92,7 +95,10 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
     operator stays Hermitian (the term table adds no h.c. for those)."""
     from .sectors import psi_layout
     from .terms import BlockOp, dot_parity
+    sym = getattr(tt.ints, "sym", "NSz")
+    dtype = np.dtype(getattr(tt.ints, "dtype", np.float64))
     pr = Problem()
+    pr.sym, pr.dtype = sym, dtype
     pr.N_tot, pr.twoSz_tot = N_tot, twoSz_tot
     pr.secL = np.array(secL, dtype=np.int32).reshape(-1, 3)
     pr.secR = np.array(secR, dtype=np.int32).reshape(-1, 3)
@@ -105,7 +111,7 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
     sym_blocks = []   # direct fill: (offset, d) of square blocks to symmetrise
     off = 0
     for op in stored:
-        dq = op_charge(op)
+        dq = op_charge(op, sym)
         first = len(blk_rows)
         sl = secs[op.side]
         self_adjoint = op.kind == "H" or (op.kind in ("B", "Q") and op.p == op.q)
@@ -119,7 +125,7 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
                 if m is None:
                     continue
                 assert m.shape == shape
-                vals.append(np.ascontiguousarray(m, dtype=np.float64).ravel())
+                vals.append(np.ascontiguousarray(m, dtype=dtype).ravel())
             elif self_adjoint:
                 assert ir == ic
                 sym_blocks.append((off, shape[0]))
@@ -131,18 +137,24 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
     if block_values is None and direct_seed is None:
         values = None   # structure only (sizing / planning without the 8-byte-per-element store)
     elif block_values is None:
-        values = np.empty(off, dtype=np.float64)
-        _fill_normal(values, int(direct_seed))
-        if direct_scale != 1.0:
-            values *= direct_scale
+        if dtype.kind == "c":   # real and imaginary parts N(0, 1/2) each: |entry|^2 has mean 1 as in the real fill
+            raw = np.empty(2 * off, dtype=np.float64)
+            _fill_normal(raw, int(direct_seed))
+            raw *= direct_scale * np.sqrt(0.5)
+            values = raw.view(np.complex128)
+        else:
+            values = np.empty(off, dtype=np.float64)
+            _fill_normal(values, int(direct_seed))
+            if direct_scale != 1.0:
+                values *= direct_scale
         for o, d in sym_blocks:
             m = values[o:o + d * d].reshape(d, d)
-            m[:] = (m + m.T) * 0.5
+            m[:] = (m + m.conj().T) * 0.5
     lin_ptr, lin_op, lin_coef = [0], [], []
     for side in "LR":
         for j, lc in enumerate(tt.lincombs[side]):
             op = BlockOp(side, "LIN", j, -1)
-            charges = {op_charge(BlockOp(side, "C", lab, -1)) for lab, _ in lc}
+            charges = {op_charge(BlockOp(side, "C", lab, -1), sym) for lab, _ in lc}
             assert len(charges) == 1, "lincomb mixes charges"
             dq = charges.pop()
             op_id[op] = len(ops_rows)
@@ -154,15 +166,16 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
     pr.ops = np.array(ops_rows, dtype=np.int64).reshape(-1, 8)
     pr.blocks = np.array(blk_rows, dtype=np.int64).reshape(-1, 3)
     if block_values is not None:
-        values = np.concatenate(vals) if vals else np.zeros(0)
+        values = np.concatenate(vals) if vals else np.zeros(0, dtype=dtype)
     pr.values = values
     pr.lin_ptr = np.array(lin_ptr, dtype=np.int64)
     pr.lin_op = np.array(lin_op, dtype=np.int32)
-    pr.lin_coef = np.array(lin_coef, dtype=np.float64)
+    pr.lin_coef = np.array(lin_coef, dtype=dtype)
     # site operators, deduplicated by value
     site_index, site_ops, site_par = {}, [], []
 
     def site_id(m):
+        m = np.ascontiguousarray(m, dtype=dtype)
         key = m.tobytes()
         if key not in site_index:
             site_index[key] = len(site_ops)
@@ -170,18 +183,18 @@ def assemble(tt, secL, secR, block_values, N_tot, twoSz_tot, direct_seed=None, d
             site_par.append(dot_parity(m))
         return site_index[key]
 
-    site_id(np.eye(4))
+    site_id(np.eye(4, dtype=dtype))
     coefs, idx = [], []
     for coef, Ls, c, d, Rs in tt.terms:
         ol, tl = (-1, 0) if Ls is None else (op_id[Ls[0]], int(Ls[1]))
         orr, trr = (-1, 0) if Rs is None else (op_id[Rs[0]], int(Rs[1]))
         coefs.append(coef)
         idx.append((ol, tl, site_id(c), site_id(d), orr, trr))
-    pr.term_coef = np.array(coefs, dtype=np.float64)
+    pr.term_coef = np.array(coefs, dtype=dtype)
     pr.term_idx = np.array(idx, dtype=np.int32).reshape(-1, 6)
-    pr.site_ops = np.array(site_ops, dtype=np.float64).reshape(-1, 16)
+    pr.site_ops = np.array(site_ops, dtype=dtype).reshape(-1, 16)
     pr.site_parity = np.array(site_par, dtype=np.int32)
-    pr.layout, pr.psi_size = psi_layout(secL, secR, N_tot, twoSz_tot)
+    pr.layout, pr.psi_size = psi_layout(secL, secR, N_tot, twoSz_tot, sym)
     pr.op_id = op_id
     pr.stored_ops = stored
     return pr

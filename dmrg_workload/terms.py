@@ -13,9 +13,12 @@ op on R).  This module is symbolic: it emits slot descriptors and coefficients t
 from the integrals; it performs no contraction.
 
 Storage conventions referenced here: A_pq, P_pq stored for p<q (P_qp = -P_pq);
-B_pt, Q_pt stored for p<=t (B_tp = B_pt^T, Q_tp = Q_pt^T, real integrals).
-A 'LIN' operator is sum_s coef_s a+_s on one block; used transposed it is
-sum_s coef_s a_s (the paper's "intermediates").
+B_pt, Q_pt stored for p<=t (B_tp = B_pt^H, Q_tp = Q_pt^H by Hermiticity of the integrals).
+A 'LIN' operator is sum_s coef_s a+_s on one block; used "transposed" it is its Hermitian
+conjugate sum_s conj(coef_s) a_s (the paper's "intermediates").
+Throughout, a transposed use (trans flag) means the Hermitian conjugate of the stored operator:
+the plain transpose for the real spin-free integrals, the conjugate transpose for the complex
+integrals of a spin-orbit Hamiltonian, to which the same table applies.
 """
 from collections import namedtuple
 
@@ -66,14 +69,23 @@ class TermTable:
         self._lin_index = {}
         self.terms = []
         self.tags = []
+        self.complex = np.dtype(getattr(ints, "dtype", np.float64)).kind == "c"
         self.sc = SiteOps(part.nL, ints)
         self.sd = SiteOps(part.nL + 1, ints)
         self._build()
 
     # ---- helpers -------------------------------------------------------
+    def _num(self, c):
+        return complex(c) if self.complex else float(c)
+
+    def linT(self, side, coefs):
+        """Slot whose operator is sum_s coefs[s] a_s: the LIN operator sum_s conj(coefs[s]) a+_s, used transposed."""
+        lin = self.lin(side, [(s, np.conj(c)) for s, c in coefs])
+        return None if lin is None else (lin, True)
+
     def lin(self, side, coefs):
         """Register sum_s coefs[s] a+_s on `side`; returns BlockOp or None if all zero."""
-        items = tuple((s, float(c)) for s, c in coefs if c != 0.0)
+        items = tuple((s, self._num(c)) for s, c in coefs if c != 0.0)
         if not items:
             return None
         key = (side, items)
@@ -112,13 +124,13 @@ class TermTable:
             return
         n_odd = block_parity(L) + pc + pd + block_parity(R)
         assert n_odd % 2 == 0, f"odd term in {tag}"
-        self.terms.append((float(coef), L, c.copy(), d.copy(), R))
+        self.terms.append((self._num(coef), L, c.copy(), d.copy(), R))
         self.tags.append(tag)
         if hc:
             sgn = -1.0 if (n_odd * (n_odd - 1) // 2) % 2 else 1.0
             Lh = None if L is None else (L[0], not L[1])
             Rh = None if R is None else (R[0], not R[1])
-            self.terms.append((float(coef) * sgn, Lh, c.T.copy(), d.T.copy(), Rh))
+            self.terms.append((self._num(np.conj(coef)) * sgn, Lh, c.conj().T.copy(), d.conj().T.copy(), Rh))
             self.tags.append(tag + "+")
 
     # ---- the table -----------------------------------------------------
@@ -185,9 +197,9 @@ class TermTable:
                 add("G3e", 1.0, FL, Fc, sd.D(t), (op, tr), True)
             for q in d:
                 for t in d:
-                    lin = self.lin("R", [(r, V(p, q, r, t)) for r in R])
+                    lin = self.linT("R", [(r, V(p, q, r, t)) for r in R])
                     if lin is not None:
-                        add("G3f", 1.0, FL, Fc, sd.B(q, t), T(lin), True)
+                        add("G3f", 1.0, FL, Fc, sd.B(q, t), lin, True)
         # G4: sum_{p in d u R} a+_p S_p^{Lc}  (ordered: S_p^{Lc} to the left => -1)
         for p in d + R:
             if p in d:
@@ -204,9 +216,9 @@ class TermTable:
                 add("G4d", -1.0 * sg, N(op), sc.C(q), Gd, GR, True)
             for q in c:
                 for t in c:
-                    lin = self.lin("L", [(s, V(p, q, s, t)) for s in L])
+                    lin = self.linT("L", [(s, V(p, q, s, t)) for s in L])
                     if lin is not None:
-                        add("G4e", -1.0, T(lin), sc.B(q, t), Gd, GR, True)
+                        add("G4e", -1.0, lin, sc.B(q, t), Gd, GR, True)
             for r in c:
                 op, tr = self.Qop("L", p, r)
                 add("G4f", -1.0, (op, tr), sc.D(r), Gd, GR, True)
@@ -231,15 +243,15 @@ class TermTable:
         for p in L:
             for q in c:
                 for t in d:
-                    lin = self.lin("R", [(r, V(p, q, t, r)) for r in R])
+                    lin = self.linT("R", [(r, V(p, q, t, r)) for r in R])
                     if lin is not None:
-                        add("G5f", -1.0, N(Cr("L", p)), sc.C(q), sd.D(t), T(lin), True)
+                        add("G5f", -1.0, N(Cr("L", p)), sc.C(q), sd.D(t), lin, True)
         add("G5g", 1.0, None, Ac, None, N(BlockOp("R", "P", c0, c1)), True)
         add("G5h", V(c0, c1, d0, d1), None, Ac, ddn, None, True)
         for t in d:
-            lin = self.lin("R", [(r, V(c0, c1, t, r)) for r in R])
+            lin = self.linT("R", [(r, V(c0, c1, t, r)) for r in R])
             if lin is not None:
-                add("G5i", -1.0, None, Ac, sd.D(t), T(lin), True)
+                add("G5i", -1.0, None, Ac, sd.D(t), lin, True)
         # G6: sum_{p,t in L u c} B_pt Q_pt^{dR}
         for i, p in enumerate(L):
             add("G6a", 1.0, N(BlockOp("L", "B", p, p)), None, None,
@@ -267,9 +279,9 @@ class TermTable:
         for p in L:
             for t in c:
                 for q in d:
-                    lin = self.lin("R", [(r, V(p, q, t, r)) for r in R])
+                    lin = self.linT("R", [(r, V(p, q, t, r)) for r in R])
                     if lin is not None:
-                        add("G6g", 1.0, N(Cr("L", p)), sc.D(t), sd.C(q), T(lin), True)
+                        add("G6g", 1.0, N(Cr("L", p)), sc.D(t), sd.C(q), lin, True)
                     lin = self.lin("R", [(r, V(p, r, t, q)) for r in R])
                     if lin is not None:
                         add("G6h", -1.0, N(Cr("L", p)), sc.D(t), sd.D(q), N(lin), True)
@@ -279,9 +291,9 @@ class TermTable:
                 add("G6i", 1.0, None, sc.B(p, t), None, (op, tr), False)
                 add("G6j", 1.0, None, sc.B(p, t), sd.Q(p, t), None, False)
                 for q in d:
-                    lin = self.lin("R", [(r, V(p, q, t, r)) for r in R])
+                    lin = self.linT("R", [(r, V(p, q, t, r)) for r in R])
                     if lin is not None:
-                        add("G6k", 1.0, None, sc.B(p, t), sd.C(q), T(lin), False)
+                        add("G6k", 1.0, None, sc.B(p, t), sd.C(q), lin, False)
                     lin = self.lin("R", [(r, V(p, r, t, q)) for r in R])
                     if lin is not None:
                         add("G6l", -1.0, None, sc.B(p, t), sd.D(q), N(lin), False)

@@ -5,7 +5,7 @@ import pytest
 import scipy.sparse as sp
 
 import fockdense as fd
-from dmrg_workload.integrals import make_integrals
+from dmrg_workload.integrals import make_integrals, make_so_integrals
 from dmrg_workload.terms import Partition, TermTable, block_parity, dot_parity
 
 
@@ -17,12 +17,15 @@ def slot_matrix(slot, blk, lincombs):
         m = blk.op("LIN", lin=lincombs[op.side][op.p])
     else:
         m = blk.op(op.kind, op.p, op.q)
-    return m.T.tocsr() if tr else m
+    return m.conj().T.tocsr() if tr else m   # a transposed use is the Hermitian conjugate (terms.py)
 
 
-@pytest.mark.parametrize("K,nL", [(4, 1), (5, 2), (5, 1), (6, 2)])
-def test_term_table_reproduces_H(K, nL):
-    ints = make_integrals(K, seed=100 + K + nL)
+@pytest.mark.parametrize("K,nL,spin_orbit", [(4, 1, False), (5, 2, False), (5, 1, False), (6, 2, False),
+                                             (4, 1, True), (5, 2, True), (5, 1, True)])
+def test_term_table_reproduces_H(K, nL, spin_orbit):
+    """spin_orbit: complex Hermitian integrals without spin selection rules -- the same table with
+    every transposed use read as a Hermitian conjugate."""
+    ints = (make_so_integrals if spin_orbit else make_integrals)(K, seed=100 + K + nL)
     part = Partition(K, nL)
     tt = TermTable(part, ints)
     bL, bR = fd.DenseBlock(part.L, ints), fd.DenseBlock(part.R, ints)
@@ -48,4 +51,8 @@ def test_term_table_reproduces_H(K, nL):
     Href = fd.hamiltonian(a, ints, dim)
     diff = abs(Hsum - Href).max()
     assert diff < 1e-12, diff
-    assert abs(Href - Href.T).max() < 1e-12
+    assert abs(Href - Href.conj().T).max() < 1e-12
+    if spin_orbit:   # the coupling is really there: H is complex and does not commute with Sz
+        assert abs(Href.imag).max() > 1e-3
+        Sz = sum(0.5 * (1 if P % 2 == 0 else -1) * (a[P].T @ a[P]) for P in a)
+        assert abs(Href @ Sz - Sz @ Href).max() > 1e-3
