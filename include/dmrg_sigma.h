@@ -236,6 +236,42 @@ int dmrg_davidson(dmrg_plan* plan, double* x, int32_t max_iter, int32_t max_spac
                   void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Spin-orbit Hamiltonians: complex FP64, U(1)_N only, two-by-two dot blocks ("For relativistic Hamiltonian
+ * including spin-orbit couplings, the spin projection is no longer a good quantum number, and [O]_{C1'C1} and [O]_{C2'C2}
+ * can be either a scalar or a two-by-two matrix"; PAPER.md:285 names complex arithmetic as the extension).  The same
+ * Eq. (7) in complex arithmetic:
+ *   dmrg_ops_load_z    as dmrg_ops_load, with values [host or device] and lin_coef [host] holding (re, im) PAIRS of doubles
+ *                      (numpy complex128): nvalues and dmrg_block_desc.offset count complex numbers.  Every sector label
+ *                      and operator charge must have two_sz = d2sz = 0.  A "transposed" use of an operator (trans_l,
+ *                      trans_r) means its conjugate transpose.  Store utilities (export, join, add_lincombs, derive) and
+ *                      dmrg_renormalize refuse complex stores (DMRG_EINVAL).
+ *   dmrg_plan_create_z as dmrg_plan_create_opts on such a store: coef_im [host, may be NULL = 0] the imaginary parts of the
+ *                      term coefficients (real parts in terms[].coef); site_ops [host] nsite x 16 (re, im) pairs, row-major
+ *                      4 x 4; only N is checked (DMRG_ECHARGE) and the two singly occupied site states (1 beta, 2 alpha)
+ *                      belong to one dot sector, so a site matrix may connect them: such a two-by-two dot block is planned
+ *                      as up to four (c', c) transitions per term and block, Eqs. (9)-(10) folded into the scalar factors.
+ *   psi / sigma / diag of a complex plan are vectors of (re, im) pairs (complex128) in the psi layout;
+ *   dmrg_plan_psi_size still counts DOUBLES (2 per number), dmrg_psi_block.offset counts numbers.  dmrg_sigma, dmrg_sigma_host,
+ *   dmrg_hdiag (the real diagonal, written to both slots of every pair) and dmrg_davidson take such plans unchanged: a
+ *   Hermitian H is a real symmetric operator on the 2n reals, with the same lowest eigenvalue, and every real eigenvector
+ *   of it is a complex eigenvector of H.
+ * How it runs (csrc/plan.cu): through the same real grouped FP64 GEMM kernel -- psi, X and sigma row-planar, the R blocks
+ * packed as their real 2 x 2 images, the L blocks stored as theirs -- 8 M N K real flops per complex GEMM, the count of a
+ * complex multiply-add, nothing computed twice.  The complex store takes 4 doubles per L-side entry (2 per R-side entry
+ * plus 4 in the plan's packed copy). */
+int dmrg_ops_load_z(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* secR, int32_t nsecR,
+                    const dmrg_op_desc* ops, int32_t nops,
+                    const dmrg_block_desc* blocks, int64_t nblocks,
+                    const double* values, int64_t nvalues, int32_t values_on_device,
+                    const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin,
+                    dmrg_ops** out);
+int dmrg_plan_create_z(const dmrg_ops* ops, const dmrg_term* terms, const double* coef_im, int64_t nterms,
+                       const double* site_ops, const int32_t* site_parity, int32_t nsite,
+                       int32_t n_total, const dmrg_plan_options* options, dmrg_plan** out);
+int32_t dmrg_ops_is_complex(const dmrg_ops* ops);
+int32_t dmrg_plan_is_complex(const dmrg_plan* plan);
+
+/* ---------------------------------------------------------------------------------------------
  * dmrg_dots_static: out[i] = sum_e V[i*stride + e] * w[e], i < m -- the block of dot products every Davidson
  * iteration needs (G_ik = b_i . w_k, the Gram-Schmidt coefficients, |r|^2; PAPER.md:162 keeps them on CPU rank 0),
  * for callers that cannot allocate device memory (CUDA graph capture, tight serving loops, harnesses that forbid

@@ -45,7 +45,8 @@ EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan
            "dmrg_fp64_peak_tflops", "dmrg_last_error", "dmrg_version",
            "dmrg_renormalize", "dmrg_ops_num_ops", "dmrg_ops_num_blocks", "dmrg_ops_num_values", "dmrg_ops_export", "dmrg_ops_sectors",
            "dmrg_ops_join", "dmrg_ops_add_lincombs", "dmrg_ops_derive",
-           "dmrg_comm_unique_id", "dmrg_comm_create", "dmrg_comm_destroy", "dmrg_plan_set_comm", "dmrg_dots_static")
+           "dmrg_comm_unique_id", "dmrg_comm_create", "dmrg_comm_destroy", "dmrg_plan_set_comm", "dmrg_dots_static",
+           "dmrg_ops_load_z", "dmrg_plan_create_z", "dmrg_ops_is_complex", "dmrg_plan_is_complex")
 DOTS_STATIC_MAX_VECTORS = 32
 
 _lib = None
@@ -125,6 +126,14 @@ def lib():
         L.dmrg_comm_destroy.restype = None
         L.dmrg_plan_set_comm.argtypes = [vp, vp]
         L.dmrg_plan_set_comm.restype = C.c_int
+        L.dmrg_ops_load_z.argtypes = L.dmrg_ops_load.argtypes
+        L.dmrg_ops_load_z.restype = C.c_int
+        L.dmrg_plan_create_z.argtypes = [vp, vp, vp, i64, vp, vp, i32, i32, vp, C.POINTER(vp)]
+        L.dmrg_plan_create_z.restype = C.c_int
+        L.dmrg_ops_is_complex.argtypes = [vp]
+        L.dmrg_ops_is_complex.restype = i32
+        L.dmrg_plan_is_complex.argtypes = [vp]
+        L.dmrg_plan_is_complex.restype = i32
         L.dmrg_dots_static.argtypes = [vp, i64, i32, vp, i64, vp, vp]
         L.dmrg_dots_static.restype = C.c_int
         L.dmrg_last_error.restype = C.c_char_p
@@ -174,8 +183,12 @@ class OpsStore:
     def __init__(self, secL, secR, ops, blocks, values, lin_ptr, lin_op, lin_coef):
         """secL/secR: int [n,3] (N, 2Sz, dim); ops: int [nops,8] (side, kind, p, q, dN, d2Sz, first_block,
         nblocks); blocks: int [nblk,3] (row_sector, col_sector, offset); values: float64 numpy array (host)
-        or CUDA torch tensor (device); lincomb CSR as in dmrg_sigma.h."""
+        or CUDA torch tensor (device); lincomb CSR as in dmrg_sigma.h.  complex128 values (numpy) or a complex128 CUDA
+        tensor select dmrg_ops_load_z (spin-orbit stores); lin_coef is then complex too."""
         self._h = None
+        is_z = values is not None and (values.dtype == np.complex128 if isinstance(values, np.ndarray) else values.is_complex())
+        is_z = is_z or (values is None and np.asarray(lin_coef).dtype.kind == "c")
+        self.is_complex = bool(is_z)
         sl = _structured(np.asarray(secL).reshape(-1, 3), SECTOR_DT, (("n", 0), ("two_sz", 1), ("dim", 2)))
         sr = _structured(np.asarray(secR).reshape(-1, 3), SECTOR_DT, (("n", 0), ("two_sz", 1), ("dim", 2)))
         od = _structured(np.asarray(ops).reshape(-1, 8), OP_DT, (("side", 0), ("kind", 1), ("p", 2), ("q", 3), ("dn", 4),
@@ -185,17 +198,18 @@ class OpsStore:
         if values is None:
             nvalues = int(max((b[2] for b in np.asarray(blocks).reshape(-1, 3)), default=0)) + (1 << 40)
         elif isinstance(values, np.ndarray):
-            values = np.ascontiguousarray(values, dtype=np.float64)
+            values = np.ascontiguousarray(values, dtype=np.complex128 if is_z else np.float64)
         else:
-            assert values.is_cuda and values.is_contiguous() and values.element_size() == 8
+            assert values.is_cuda and values.is_contiguous() and values.element_size() == (16 if is_z else 8)
             on_dev = 1
         lp = np.ascontiguousarray(lin_ptr, dtype=np.int64)
         lo = np.ascontiguousarray(lin_op, dtype=np.int32)
-        lc = np.ascontiguousarray(lin_coef, dtype=np.float64)
+        lc = np.ascontiguousarray(lin_coef, dtype=np.complex128 if is_z else np.float64)
         if values is not None:
             nvalues = int(values.size if on_dev == 0 else values.numel())
         h = C.c_void_p()
-        _check(lib().dmrg_ops_load(_ptr(sl), len(sl), _ptr(sr), len(sr), _ptr(od), len(od), _ptr(bd), len(bd),
+        load = lib().dmrg_ops_load_z if is_z else lib().dmrg_ops_load
+        _check(load(_ptr(sl), len(sl), _ptr(sr), len(sr), _ptr(od), len(od), _ptr(bd), len(bd),
                                    _ptr(values), nvalues, on_dev, _ptr(lp), _ptr(lo), _ptr(lc), len(lp) - 1, C.byref(h)))
         self._h = h
 
@@ -284,15 +298,26 @@ class Plan:
         cost_order_only, split_small, release_r_store); passing any selects dmrg_plan_create_opts."""
         self._h = None
         self.ops = ops   # keep the store alive: the plan borrows it
+        self.is_complex = bool(lib().dmrg_ops_is_complex(ops._h))
         ti = np.asarray(term_idx).reshape(-1, 6)
         td = np.zeros(len(ti), dtype=TERM_DT)
-        td["coef"] = np.asarray(term_coef, dtype=np.float64)
+        td["coef"] = np.asarray(term_coef).real.astype(np.float64)
         for name, c in (("op_l", 0), ("trans_l", 1), ("dot1", 2), ("dot2", 3), ("op_r", 4), ("trans_r", 5)):
             td[name] = ti[:, c]
-        so = np.ascontiguousarray(site_ops, dtype=np.float64).reshape(-1, 16)
+        so = np.ascontiguousarray(site_ops, dtype=np.complex128 if self.is_complex else np.float64).reshape(-1, 16)
         sp = np.ascontiguousarray(site_parity, dtype=np.int32)
         h = C.c_void_p()
-        if options:
+        if self.is_complex:   # dmrg_plan_create_z: complex coefficients and site matrices, N only
+            ci = np.ascontiguousarray(np.asarray(term_coef, dtype=np.complex128).imag, dtype=np.float64)
+            po = np.zeros(1, dtype=PLANOPT_DT)
+            po["workspace_bytes"] = int(workspace_bytes)
+            for k, v in options.items():
+                if k not in PLANOPT_DT.names or k == "reserved":
+                    raise TypeError(f"unknown plan option {k!r}")
+                po[k] = v
+            assert int(two_sz_total) == 0
+            _check(lib().dmrg_plan_create_z(ops._h, _ptr(td), _ptr(ci), len(td), _ptr(so), _ptr(sp), len(so), int(n_total), _ptr(po), C.byref(h)))
+        elif options:
             po = np.zeros(1, dtype=PLANOPT_DT)
             po["workspace_bytes"] = int(workspace_bytes)
             for k, v in options.items():

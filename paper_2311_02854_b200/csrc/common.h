@@ -127,6 +127,7 @@ struct dmrg_ops {
     double* side_alloc[2] = {nullptr, nullptr};   // dmrg_ops_load: the allocation holding the L-side / R-side blocks (also in `owned`)
     size_t side_bytes[2] = {0, 0};
     mutable bool r_released = false;   // a plan created with release_r_store freed side_alloc[1]: the store serves that plan only
+    bool cplx = false;             // dmrg_ops_load_z: complex blocks (L side: real 2x2-image blocks, R side: row-planar re | im; ops_store.cu)
     bool structure_only = false;   // loaded with values == NULL: planning / statistics only, no device memory
     int64_t nvalues_dev = 0;     // doubles allocated (stored + lincomb, padded)
     int64_t device_bytes = 0;

@@ -23,7 +23,13 @@ void set_error(const char* fmt, ...) {
     g_err = buf;
 }
 
-struct RepackDesc { int64_t src, dst; int32_t rows, cols, ld, side; };   // side: which of the store's two allocations dst lives in (host bookkeeping)
+struct RepackDesc { int64_t src, dst; int32_t rows, cols, ld, side; int32_t mode, pad_; };   // side: which of the store's two allocations dst lives in (host bookkeeping)
+// mode 0: real block.  Complex stores (dmrg_ops_load_z; src = interleaved (re, im) pairs, offsets in doubles):
+//   mode 1, L side: the real 2 rows x 2 cols image with interleaved rows and columns, [2r+a][2c+b] = (a == b ? re : (a ? im : -im)),
+//           so that  image(A) image(B) = image(A B),  image(A)^T = image(A^H),  and a complex matrix-vector product
+//           becomes a real one on vectors whose entries are (re, im) row pairs -- stage 2 reads these blocks as they are;
+//   mode 2, R side: row-planar, row r = [re(r, 0..cols) | im(r, 0..cols)], each half padded to an even length (ld = 2 halves);
+//           stage 1 reads the R side through the plan's packed copy, which builds its own real image from this.
 
 // dst[r*ld + c] = c < cols ? src[r*cols + c] : 0      one CTA per block
 __global__ void __launch_bounds__(256) repack_kernel(const RepackDesc* __restrict__ desc, const double* __restrict__ src_base,
@@ -31,6 +37,26 @@ __global__ void __launch_bounds__(256) repack_kernel(const RepackDesc* __restric
     const RepackDesc d = desc[blockIdx.x];
     const double* src = src_base + (d.src - src_shift);
     double* dst = dst_base + d.dst;
+    if (d.mode == 1) {   // ld = 2 cols
+        const int64_t n = (int64_t)2 * d.rows * d.ld;
+        for (int64_t e = threadIdx.x; e < n; e += blockDim.x) {
+            const int rr = (int)(e / d.ld), cc = (int)(e - (int64_t)rr * d.ld);
+            const int a = rr & 1, b = cc & 1;
+            const double v = src[2 * ((int64_t)(rr >> 1) * d.cols + (cc >> 1)) + (a ^ b)];
+            dst[e] = (a == 0 && b == 1) ? -v : v;
+        }
+        return;
+    }
+    if (d.mode == 2) {   // ld = 2 round_up2(cols)
+        const int half = d.ld / 2;
+        const int64_t n = (int64_t)d.rows * d.ld;
+        for (int64_t e = threadIdx.x; e < n; e += blockDim.x) {
+            const int r = (int)(e / d.ld), cc = (int)(e - (int64_t)r * d.ld);
+            const int part = cc >= half, c = cc - part * half;
+            dst[e] = c < d.cols ? src[2 * ((int64_t)r * d.cols + c) + part] : 0.0;
+        }
+        return;
+    }
     const int64_t n = (int64_t)d.rows * d.ld;
     for (int64_t e = threadIdx.x; e < n; e += blockDim.x) {
         int r = (int)(e / d.ld), c = (int)(e - (int64_t)r * d.ld);
@@ -55,6 +81,31 @@ __global__ void __launch_bounds__(256) lincomb_kernel(const LinDesc* __restrict_
     }
 }
 
+// Complex stores: out = sum_i (cr_i + i ci_i) * src_i in summand order.  In both device layouts a complex entry is a pair of
+// doubles (x, y) = (re, im) at positions (p, p + delta): the L-side image keeps them in rows 2r / 2r + 1 of one column
+// (x = [2r][c] carries re for even c and -im for odd c, y = [2r+1][c] the matching im / re: multiplying by i maps
+// (x, y) -> (-y, x) in every column), the R-side row-planar layout in the two halves of a row.  Pair q of a block sits at
+// p = (q / w) * stride + q % w.
+struct LinDescZ { int64_t dst; int64_t npairs; int32_t w, stride, delta; int32_t sum_begin, sum_end, pad_; };
+struct LinSummandZ { int64_t src; double cr, ci; };
+__global__ void __launch_bounds__(256) lincomb_z_kernel(const LinDescZ* __restrict__ desc, const LinSummandZ* __restrict__ sums,
+                                                        double* __restrict__ vals) {
+    const LinDescZ d = desc[blockIdx.y];
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < d.npairs; q += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t p = (q / d.w) * d.stride + q % d.w;
+        double ax = 0.0, ay = 0.0;
+        for (int i = d.sum_begin; i < d.sum_end; i++) {
+            const LinSummandZ s = sums[i];
+            if (s.src < 0) continue;
+            const double x = vals[s.src + p], y = vals[s.src + p + d.delta];
+            ax += s.cr * x - s.ci * y;
+            ay += s.cr * y + s.ci * x;
+        }
+        vals[d.dst + p] = ax;
+        vals[d.dst + p + d.delta] = ay;
+    }
+}
+
 static int find_sector(const std::vector<dmrg_sector>& s, int n, int two_sz) {
     for (size_t i = 0; i < s.size(); i++)
         if (s[i].n == n && s[i].two_sz == two_sz) return (int)i;
@@ -65,7 +116,8 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
                          const dmrg_op_desc* ops, int32_t nops, const dmrg_block_desc* blocks, int64_t nblocks,
                          const double* values, int64_t nvalues, int32_t values_on_device,
                          const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin,
-                         dmrg_ops* S) {
+                         bool cplx, dmrg_ops* S) {
+    S->cplx = cplx;   // values / lin_coef are interleaved (re, im) pairs; nvalues and block offsets count complex numbers
     DMRG_REQUIRE((secL || nsecL == 0) && (secR || nsecR == 0) && nsecL >= 0 && nsecR >= 0 && nsecL + nsecR > 0, "dmrg_ops_load: empty sector table");
     DMRG_REQUIRE(nops >= 0 && nblocks >= 0 && nvalues >= 0, "dmrg_ops_load: negative count");
     DMRG_REQUIRE(nops == 0 || ops, "dmrg_ops_load: ops is NULL");
@@ -111,16 +163,27 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             const int rows = sec[bd.row_sector].dim, cols = sec[bd.col_sector].dim;
             DMRG_REQUIRE(bd.offset >= 0 && bd.offset + (int64_t)rows * cols <= nvalues,
                          "dmrg_ops_load: block %lld exceeds values[]", (long long)b);
-            const int ld = (int)round_up2(cols);
             int64_t& top = tops[d.side];
             S->row_off[o][bd.row_sector] = top;
-            rep.push_back({bd.offset, top, rows, cols, ld, d.side});
-            top += (int64_t)rows * ld;
+            if (!cplx) {
+                const int ld = (int)round_up2(cols);
+                rep.push_back({bd.offset, top, rows, cols, ld, d.side, 0, 0});
+                top += (int64_t)rows * ld;
+            } else if (d.side == 0) {
+                rep.push_back({2 * bd.offset, top, rows, cols, 2 * cols, d.side, 1, 0});
+                top += (int64_t)4 * rows * cols;
+            } else {
+                const int ld = 2 * (int)round_up2(cols);
+                rep.push_back({2 * bd.offset, top, rows, cols, ld, d.side, 2, 0});
+                top += (int64_t)rows * ld;
+            }
         }
     }
     // linear combinations: block present where any summand has one
     std::vector<LinDesc> lind;
     std::vector<LinSummand> lins;
+    std::vector<LinDescZ> lindz;
+    std::vector<LinSummandZ> linsz;
     std::vector<int> lin_side;   // side of lind[i] (its summands are on the same side)
     for (int o = 0; o < nops; o++) {
         const dmrg_op_desc& d = ops[o];
@@ -142,8 +205,20 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             bool any = false;
             for (int64_t i = i0; i < i1; i++) any = any || S->row_off[lin_op[i]][r] >= 0;
             if (!any) continue;
-            const int64_t n = (int64_t)sec[r].dim * round_up2(sec[c].dim);
             int64_t& top = tops[d.side];
+            if (cplx) {
+                const int rows = sec[r].dim, cols = sec[c].dim, pc = (int)round_up2(cols);
+                LinDescZ ld = d.side == 0 ? LinDescZ{top, (int64_t)rows * 2 * cols, 2 * cols, 4 * cols, 2 * cols, (int32_t)linsz.size(), 0, 0}
+                                          : LinDescZ{top, (int64_t)rows * pc, pc, 2 * pc, pc, (int32_t)linsz.size(), 0, 0};
+                lin_side.push_back(d.side);
+                for (int64_t i = i0; i < i1; i++) linsz.push_back({S->row_off[lin_op[i]][r], lin_coef[2 * i], lin_coef[2 * i + 1]});
+                ld.sum_end = (int32_t)linsz.size();
+                lindz.push_back(ld);
+                S->row_off[o][r] = top;
+                top += d.side == 0 ? (int64_t)4 * rows * cols : (int64_t)rows * 2 * pc;
+                continue;
+            }
+            const int64_t n = (int64_t)sec[r].dim * round_up2(sec[c].dim);
             LinDesc ld{top, n, (int32_t)lins.size(), 0};
             lin_side.push_back(d.side);
             for (int64_t i = i0; i < i1; i++) lins.push_back({S->row_off[lin_op[i]][r], lin_coef[i]});
@@ -182,11 +257,18 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
         lind[i].dst += shift[lin_side[i]];
         for (int q = lind[i].sum_begin; q < lind[i].sum_end; q++) if (lins[q].src >= 0) lins[q].src += shift[lin_side[i]];
     }
+    for (size_t i = 0; i < lindz.size(); i++) {
+        lindz[i].dst += shift[lin_side[i]];
+        for (int q = lindz[i].sum_begin; q < lindz[i].sum_end; q++) if (linsz[q].src >= 0) linsz[q].src += shift[lin_side[i]];
+    }
 
     // ---- repack stored blocks (row padding) -------------------------------------------------
     if (!rep.empty()) {
         std::sort(rep.begin(), rep.end(), [](const RepackDesc& a, const RepackDesc& b) { return a.src < b.src; });
         const int64_t CHUNK = int64_t(1) << 26;   // 64 Mi doubles = 512 MiB staging
+        const int64_t esz = cplx ? 2 : 1;         // doubles per stored number; RepackDesc.src counts doubles
+        const int64_t nvalues_d = nvalues * esz;
+        auto raw_end = [&](const RepackDesc& r) { return r.src + esz * (int64_t)r.rows * r.cols; };
         double* d_stage = nullptr;
         RepackDesc* d_desc = nullptr;
         const size_t DESC_BATCH = 1 << 16;
@@ -200,7 +282,7 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
             int64_t hi = lo;
             size_t j = i;
             while (j < rep.size() && j - i < DESC_BATCH) {
-                const int64_t end = rep[j].src + (int64_t)rep[j].rows * rep[j].cols;
+                const int64_t end = raw_end(rep[j]);
                 if (j > i && end - lo > CHUNK) break;
                 hi = std::max(hi, end);
                 j++;
@@ -212,7 +294,7 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
                 if (hi - lo > stage_cap) {
                     if (d_stage) cudaFree(d_stage);
                     d_stage = nullptr;
-                    stage_cap = std::max(hi - lo, std::min<int64_t>(CHUNK, nvalues));
+                    stage_cap = std::max(hi - lo, std::min<int64_t>(CHUNK, nvalues_d));
                     cudaError_t e = cudaMalloc(&d_stage, sizeof(double) * (size_t)stage_cap);
                     if (e != cudaSuccess) { set_error("dmrg_ops_load: staging cudaMalloc failed"); rc = DMRG_ENOMEM; break; }
                 }
@@ -233,6 +315,23 @@ static int ops_load_impl(const dmrg_sector* secL, int32_t nsecL, const dmrg_sect
         if (rc != DMRG_OK) return rc;
     }
     // ---- intermediates: O = sum_s alpha_s a_s, block by block ------------------
+    if (!lindz.empty()) {
+        LinDescZ* d_lind = nullptr;
+        LinSummandZ* d_lins = nullptr;
+        DMRG_CUDA(cudaMalloc(&d_lind, sizeof(LinDescZ) * lindz.size()));
+        DMRG_CUDA(cudaMalloc(&d_lins, sizeof(LinSummandZ) * linsz.size()));
+        DMRG_CUDA(cudaMemcpy(d_lind, lindz.data(), sizeof(LinDescZ) * lindz.size(), cudaMemcpyHostToDevice));
+        DMRG_CUDA(cudaMemcpy(d_lins, linsz.data(), sizeof(LinSummandZ) * linsz.size(), cudaMemcpyHostToDevice));
+        const size_t YB = 32768;
+        for (size_t y0 = 0; y0 < lindz.size(); y0 += YB) {
+            const unsigned ny = (unsigned)std::min(YB, lindz.size() - y0);
+            lincomb_z_kernel<<<dim3(8, ny), 256>>>(d_lind + y0, d_lins, S->d_values);
+        }
+        DMRG_CUDA(cudaGetLastError());
+        DMRG_CUDA(cudaDeviceSynchronize());
+        cudaFree(d_lind);
+        cudaFree(d_lins);
+    }
     if (!lind.empty()) {
         LinDesc* d_lind = nullptr;
         LinSummand* d_lins = nullptr;
@@ -269,7 +368,7 @@ int dmrg_ops_load(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* sec
     int rc;
     try {
         rc = dmrg::ops_load_impl(secL, nsecL, secR, nsecR, ops, nops, blocks, nblocks, values, nvalues, values_on_device,
-                                 lin_ptr, lin_op, lin_coef, nlin, S);
+                                 lin_ptr, lin_op, lin_coef, nlin, false, S);
     } catch (const std::bad_alloc&) {
         dmrg::set_error("dmrg_ops_load: out of host memory");
         rc = DMRG_ENOMEM;
@@ -281,6 +380,33 @@ int dmrg_ops_load(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* sec
     *out = S;
     return DMRG_OK;
 }
+
+int dmrg_ops_load_z(const dmrg_sector* secL, int32_t nsecL, const dmrg_sector* secR, int32_t nsecR,
+                    const dmrg_op_desc* ops, int32_t nops, const dmrg_block_desc* blocks, int64_t nblocks,
+                    const double* values, int64_t nvalues, int32_t values_on_device,
+                    const int64_t* lin_ptr, const int32_t* lin_op, const double* lin_coef, int32_t nlin,
+                    dmrg_ops** out) {
+    if (!out) { dmrg::set_error("dmrg_ops_load_z: out is NULL"); return DMRG_EINVAL; }
+    *out = nullptr;
+    dmrg_ops* S = new (std::nothrow) dmrg_ops();
+    if (!S) { dmrg::set_error("dmrg_ops_load_z: out of host memory"); return DMRG_ENOMEM; }
+    int rc;
+    try {
+        rc = dmrg::ops_load_impl(secL, nsecL, secR, nsecR, ops, nops, blocks, nblocks, values, nvalues, values_on_device,
+                                 lin_ptr, lin_op, lin_coef, nlin, true, S);
+    } catch (const std::bad_alloc&) {
+        dmrg::set_error("dmrg_ops_load_z: out of host memory");
+        rc = DMRG_ENOMEM;
+    } catch (...) {
+        dmrg::set_error("dmrg_ops_load_z: unexpected exception");
+        rc = DMRG_EINVAL;
+    }
+    if (rc != DMRG_OK) { dmrg_ops_free(S); return rc; }
+    *out = S;
+    return DMRG_OK;
+}
+
+int32_t dmrg_ops_is_complex(const dmrg_ops* ops) { return ops && ops->cplx ? 1 : 0; }
 
 void dmrg_ops_free(dmrg_ops* ops) {
     if (!ops) return;

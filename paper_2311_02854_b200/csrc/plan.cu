@@ -17,6 +17,7 @@
 #include <array>
 #include <atomic>
 #include <cmath>
+#include <complex>
 #include <cstdlib>
 #include <new>
 #include <thread>
@@ -30,12 +31,23 @@ namespace dmrg {
 static const int SITE_N[4] = {0, 1, 1, 2};
 static const int SITE_S[4] = {0, -1, 1, 0};
 
+// Complex plans (dmrg_plan_create_z, spin-orbit Hamiltonians: PAPER.md:97): the complex contraction runs through the
+// same real grouped GEMMs.  psi, X and sigma are kept "row-planar" (row l = [re | im], each half padded to an even
+// length): stage 1 multiplies such rows (K = both halves) by the real image [[Rre, -Rim], [Rim, Rre]] of the R block
+// as used, packed K-contiguous with all real-part rows of a stack before all imaginary-part rows, so X comes out
+// row-planar again; read with half the row pitch, a row-planar dL x dR' matrix IS the real 2 dL x dR' matrix whose rows
+// 2l, 2l+1 are (re, im) of row l, which is what the interleaved real image of an L block (ops_store.cu) multiplies in
+// stage 2 -- M and K double, N stays.  One complex GEMM costs 4 real ones (8 M N K flops), nothing is computed twice.
+// A complex coefficient alpha = ar + i ai gives two real tasks: ar into accumulator 0, ai into accumulator 1 (the
+// second half of the plan's internal sigma buffer, out_blk + nblk); sigma = acc0 + i acc1 is formed when the
+// row-planar result is written out interleaved (sigma_z_finish_kernel).  `zdim` below = 2 for complex plans.
 struct Task {
     int32_t term_ord, in_blk, out_blk;
     int32_t l_trans, r_trans;
     int32_t dLi, dLo, dRi, dRo;
     int64_t l_off, r_off;   // device offsets of the operator blocks, -1 = identity
     double alpha;
+    int32_t canon;          // 1: counts towards the canonical flops (0: the imaginary-coefficient twin of a complex task)
 };
 
 struct XLoc { int64_t off; int32_t ld; };   // X of one task: a slice (origin, row pitch) of a stage-1 job's output matrix
@@ -64,6 +76,7 @@ static inline double warp_area(const std::vector<std::pair<int, int>>& cm, const
 static inline double frag_area(int M, int N) { return 64.0 * ((M + 7) / 8) * ((N + 7) / 8); }
 
 __global__ void pack_r_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops, double* __restrict__ pack);
+__global__ void pack_r_z_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops, double* __restrict__ pack);
 
 struct TileRec { Tile t; double cost; int64_t key = 0; int32_t bucket = 0; };   // key: secondary launch order inside a cost bucket
 
@@ -107,9 +120,24 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     return p;
 }
 
-static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, const double* site_ops,
+static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_im, int64_t nterms_in, const double* site_ops_in,
                       const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
                       const PlanPolicy& pol) {
+    const bool Z = P->ops->cplx;   // complex plan: site_ops_in holds (re, im) pairs, coef_im the imaginary parts of the coefficients
+    const int zdim = Z ? 2 : 1;
+    P->cplx = Z;
+    // spin-orbit plans keep U(1)_N only: every 2Sz label is 0 and the two singly occupied site states share a sector
+    static const int SITE_S0[4] = {0, 0, 0, 0};
+    const int* const SITE_S = Z ? SITE_S0 : dmrg::SITE_S;
+    typedef std::complex<double> cplx_t;
+    std::vector<cplx_t> site_z((size_t)nsite * 16);
+    for (size_t i = 0; i < site_z.size(); i++) site_z[i] = Z ? cplx_t(site_ops_in[2 * i], site_ops_in[2 * i + 1]) : cplx_t(site_ops_in[i], 0.0);
+    const cplx_t* site_ops = site_z.data();
+    if (Z) {
+        for (int side = 0; side < 2; side++)
+            for (auto& sc : P->ops->sec[side]) DMRG_REQUIRE(sc.two_sz == 0, "dmrg_plan_create_z: sector labels must have two_sz = 0 (only N is a symmetry)");
+        DMRG_REQUIRE(two_sz_total == 0, "dmrg_plan_create_z: two_sz_total must be 0");
+    }
     int64_t nterms = nterms_in;   // shrinks to this rank's share when the plan is a shard
     const int64_t workspace_bytes = pol.workspace_bytes;
     const int64_t kMaxMergedCols = pol.max_merged_cols;
@@ -144,7 +172,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                             break;
                         }
                 }
-        P->psi_size = off;
+        P->psi_size = off * zdim;   // doubles; block offsets count numbers (complex ones for a complex plan)
     }
     const int64_t nblk = (int64_t)P->blocks.size();
     DMRG_REQUIRE(nblk > 0, "dmrg_plan_create: no psi block has the target quantum numbers (%d, %d)", n_total, two_sz_total);
@@ -168,8 +196,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         int dn = 0, ds = 0;
         if (T.op_l >= 0) { const int s = T.trans_l ? -1 : 1; dn += s * S->ops[T.op_l].dn; ds += s * S->ops[T.op_l].d2sz; }
         if (T.op_r >= 0) { const int s = T.trans_r ? -1 : 1; dn += s * S->ops[T.op_r].dn; ds += s * S->ops[T.op_r].d2sz; }
-        const double* o1 = site_ops + 16 * (size_t)T.dot1;
-        const double* o2 = site_ops + 16 * (size_t)T.dot2;
+        const cplx_t* o1 = site_ops + 16 * (size_t)T.dot1;
+        const cplx_t* o2 = site_ops + 16 * (size_t)T.dot2;
         for (int a = 0; a < 4; a++) for (int b = 0; b < 4; b++) {
             if (o1[4 * a + b] == 0.0) continue;
             for (int c = 0; c < 4; c++) for (int d = 0; d < 4; d++) {
@@ -200,8 +228,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     for (int64_t to = 0; to < nterms; to++) {
         const dmrg_term& T = terms[order[to]];
         term_task_begin[to] = (int64_t)tasks.size();
-        const double* o1 = site_ops + 16 * (size_t)T.dot1;
-        const double* o2 = site_ops + 16 * (size_t)T.dot2;
+        const cplx_t* o1 = site_ops + 16 * (size_t)T.dot1;
+        const cplx_t* o2 = site_ops + 16 * (size_t)T.dot2;
+        const cplx_t coef(T.coef, (Z && coef_im) ? coef_im[order[to]] : 0.0);
         const int p1 = site_parity[T.dot1] & 1, p2 = site_parity[T.dot2] & 1;
         const int pR = T.op_r >= 0 ? (S->ops[T.op_r].dn & 1) : 0;
         for (int64_t b = 0; b < nblk; b++) {
@@ -222,10 +251,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
             const int zexp = p1 * Nl + p2 * (Nl + SITE_N[B.c1]) + pR * (Nl + SITE_N[B.c1] + SITE_N[B.c2]);
             const double zeta = (zexp & 1) ? -1.0 : 1.0;
             for (int c1o = 0; c1o < 4; c1o++) {
-                const double v1 = o1[4 * c1o + B.c1];
+                const cplx_t v1 = o1[4 * c1o + B.c1];
                 if (v1 == 0.0) continue;
                 for (int c2o = 0; c2o < 4; c2o++) {
-                    const double v2 = o2[4 * c2o + B.c2];
+                    const cplx_t v2 = o2[4 * c2o + B.c2];
                     if (v2 == 0.0) continue;
                     const int32_t ob = lut[(((size_t)iLo * 4 + c1o) * 4 + c2o) * nR + iRo];
                     if (ob < 0) continue;
@@ -234,10 +263,19 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                     k.l_trans = T.trans_l != 0; k.r_trans = T.trans_r != 0;
                     k.dLi = B.dl; k.dRi = B.dr; k.dLo = secL[iLo].dim; k.dRo = secR[iRo].dim;
                     k.l_off = l_off; k.r_off = r_off;
-                    k.alpha = T.coef * zeta * v1 * v2;
-                    tasks.push_back(k);
-                    if (r_off >= 0) term_flops[to] += 2.0 * k.dLi * k.dRi * k.dRo;
-                    if (l_off >= 0) term_flops[to] += 2.0 * k.dLo * k.dLi * k.dRo;
+                    const cplx_t alpha = coef * zeta * v1 * v2;
+                    k.alpha = alpha.real();
+                    k.canon = 1;
+                    if (!Z || alpha.real() != 0.0 || alpha.imag() == 0.0) tasks.push_back(k);
+                    if (Z && alpha.imag() != 0.0) {   // the imaginary part of the coefficient accumulates into the second buffer
+                        k.canon = alpha.real() == 0.0;
+                        k.alpha = alpha.imag();
+                        k.out_blk = ob + (int32_t)nblk;
+                        tasks.push_back(k);
+                    }
+                    // a complex GEMM is 4 real ones: 8 M N K (zdim^2 = 4)
+                    if (r_off >= 0) term_flops[to] += 2.0 * zdim * zdim * k.dLi * k.dRi * k.dRo;
+                    if (l_off >= 0) term_flops[to] += 2.0 * zdim * zdim * k.dLo * k.dLi * k.dRo;
                 }
             }
         }
@@ -271,11 +309,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         P->shard_terms.assign(order.begin(), order.end());
     }
     for (double f : term_flops) canon_flops += f;
-    P->stats[ST_TASKS] = (double)tasks.size();
+    P->stats[ST_TASKS] = (double)std::count_if(tasks.begin(), tasks.end(), [](const Task& k) { return k.canon != 0; });   // a complex task's imaginary-coefficient twin is not a task of its own
     P->stats[ST_CANON_FLOPS] = canon_flops;
 
     // ---- chunk the (ordered) terms by X workspace --------------------------------------------------
-    auto x_elems = [](const Task& k) { return (int64_t)k.dLi * round_up2(k.dRo); };
+    auto x_elems = [zdim](const Task& k) { return (int64_t)k.dLi * zdim * round_up2(k.dRo); };
     int64_t ws_elems = workspace_bytes / 8;
     {
         int64_t max_term = 0;
@@ -330,7 +368,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     std::vector<int64_t> ppad(nblk);
     {
         int64_t o = 0;
-        for (int64_t b = 0; b < nblk; b++) { ppad[b] = o; o += (int64_t)P->blocks[b].dl * round_up2(P->blocks[b].dr); }
+        for (int64_t b = 0; b < nblk; b++) { ppad[b] = o; o += (int64_t)P->blocks[b].dl * zdim * round_up2(P->blocks[b].dr); }
         P->psi_pad_elems = std::max<int64_t>(o, 2);
     }
     // psi panels (all blocks of one R sector, contiguous in the padded copy): the matrices of the stage-1 A tensor maps
@@ -421,7 +459,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         });
         std::unordered_map<int64_t, XLoc> xloc;
         xloc.reserve(req.size() * 2);
-        std::unordered_map<int64_t, int64_t> pack_loc;   // (R block, trans) -> chunk-local offset of its packed copy
+        std::unordered_map<int64_t, std::pair<int64_t, int64_t>> pack_loc;   // (R block, trans) -> chunk-local offset of its packed copy (+ distance to its imaginary-part rows)
         std::vector<TileRec> recs1[NUM_VARIANTS];
         std::vector<std::pair<int, int>> cut_m, cut_n;
         int64_t xtop = 0;
@@ -466,25 +504,29 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         for (size_t c0 = 0; c0 < rblks.size();) {
             // class [c0, c1): same signature, stack width capped
             const dmrg_psi_block& B0 = P->blocks[req[runs[rblks[c0].r0].i].in_blk];
-            const int dRi = B0.dr, ldp = (int)round_up2(dRi);
+            // complex plans: K runs over both halves of a row-planar psi row (the pad column between them meets a zero of
+            // the pack), a stack holds the real-part rows of all its blocks, then their imaginary-part rows
+            const int dRi = B0.dr, ldp = zdim * (int)round_up2(dRi), Keff = Z ? ldp : dRi;
             size_t c1 = c0;
             int64_t ncols = 0;
             while (c1 < rblks.size() && !sig_less(rblks[c0], rblks[c1]) && !sig_less(rblks[c1], rblks[c0]) &&
-                   (c1 == c0 || ncols + round_up2(req[runs[rblks[c1].r0].i].dRo) <= kMaxMergedCols)) {
-                ncols += round_up2(req[runs[rblks[c1].r0].i].dRo);
+                   (c1 == c0 || ncols + zdim * round_up2(req[runs[rblks[c1].r0].i].dRo) <= kMaxMergedCols)) {
+                ncols += zdim * round_up2(req[runs[rblks[c1].r0].i].dRo);
                 c1++;
             }
             const int ldx = (int)ncols;   // even by construction
+            const int64_t half = ncols / 2;   // complex: column (= packed row) distance between the two parts of a block
             // pack the stack once
             std::vector<int64_t> col0s;
             int64_t col0 = 0;
             for (size_t c = c0; c < c1; c++) {
                 const XReq& r0 = req[runs[rblks[c].r0].i];
-                packs.push_back({r0.r_off, pack_top + col0 * ldp, r0.dRo, dRi, (int32_t)round_up2(r0.r_trans ? r0.dRo : dRi), r0.r_trans, ldp, 0});
-                pack_loc[r0.r_off * 2 + r0.r_trans] = pack_top + col0 * ldp;
+                packs.push_back({r0.r_off, pack_top + col0 * ldp, r0.dRo, dRi, zdim * (int32_t)round_up2(r0.r_trans ? r0.dRo : dRi), r0.r_trans, ldp, 0,
+                                 Z ? half * ldp : 0});
+                pack_loc[r0.r_off * 2 + r0.r_trans] = {pack_top + col0 * ldp, Z ? half * ldp : 0};
                 col0s.push_back(col0);
                 col0 += round_up2(r0.dRo);
-                alg_bytes += 8.0 * (double)dRi * r0.dRo;
+                alg_bytes += 8.0 * zdim * (double)dRi * r0.dRo;
             }
             // one GEMM per run of the signature
             const size_t nruns = rblks[c0].r1 - rblks[c0].r0;
@@ -496,24 +538,25 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                     const Run& Rc = runs[rblks[c].r0 + t];
                     int64_t rr = 0;
                     for (size_t q = Rc.i; q < Rc.j; q++) {
-                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx};
+                        // complex: recorded with half the row pitch -- the row-planar slice as stage 2 reads it (2 dL rows)
+                        xloc[xkey(req[q].r_off, req[q].r_trans, req[q].in_blk, nblk)] = {xtop + rr * ldx + col0s[c - c0], ldx / zdim};
                         rr += P->blocks[req[q].in_blk].dl;
                     }
-                    s1_flops += 2.0 * rows * dRi * req[Rc.i].dRo;
-                    alg_bytes += 8.0 * rows * req[Rc.i].dRo;
+                    s1_flops += 2.0 * zdim * zdim * rows * dRi * req[Rc.i].dRo;
+                    alg_bytes += 8.0 * zdim * rows * req[Rc.i].dRo;
                 }
-                alg_bytes += 8.0 * rows * dRi;
+                alg_bytes += 8.0 * zdim * rows * dRi;
                 Seg s;
                 s.a_off = ppad[req[R0.i].in_blk]; s.lda = ldp;
                 s.b_off = kPackBase + pack_top; s.ldb = ldp;   // resolved to an offset from the operator store at upload
-                s.K = dRi; s.alpha = 1.0;
+                s.K = Keff; s.alpha = 1.0;
                 s.flags = (SP_PSI << SEG_A_SPACE_SHIFT) | (SP_OPS << SEG_B_SPACE_SHIFT) | SEG_B_KCONTIG;
                 {
                     const int64_t pf = panel_first[Bt.ir];
-                    const BoxShape ba = box_shape(0, dRi, panel_rows[Bt.ir], TILE), bb = box_shape(0, dRi, ncols, TILE);
-                    s.a_map = maps.get(MS_PSI, ppad[pf], 0, dRi, panel_rows[Bt.ir], ldp, ba);
+                    const BoxShape ba = box_shape(0, Keff, panel_rows[Bt.ir], TILE), bb = box_shape(0, Keff, ncols, TILE);
+                    s.a_map = maps.get(MS_PSI, ppad[pf], 0, Keff, panel_rows[Bt.ir], ldp, ba);
                     s.a_o0 = (int32_t)((ppad[req[R0.i].in_blk] - ppad[pf]) / ldp);
-                    s.b_map = maps.get(MS_PACK, pack_top, 0, dRi, ncols, ldp, bb);
+                    s.b_map = maps.get(MS_PACK, pack_top, 0, Keff, ncols, ldp, bb);
                     s.a_pitch = (uint16_t)ba.inner; s.b_pitch = (uint16_t)bb.inner;
                     s.a_bytes = 8u * ba.inner * ba.outer; s.b_bytes = 8u * bb.inner * bb.outer;
                 }
@@ -522,11 +565,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                 jb.c_off = xtop; jb.ldc = ldx; jb.M = (int)rows; jb.N = (int)ncols;
                 jb.seg_begin = (int32_t)segs.size(); jb.seg_end = jb.seg_begin + 1;
                 jb.flags = (SP_X << JOB_C_SPACE_SHIFT);
-                jb.nstages = (dRi + GEMM_BK - 1) / GEMM_BK;
+                jb.nstages = (Keff + GEMM_BK - 1) / GEMM_BK;
                 segs.push_back(s);
                 const int v = choose_variant(jb.M, jb.N);
                 const int bm = kVariants[v].bm, bn = kVariants[v].bn;
-                const double kpad4 = 4.0 * ((dRi + 3) / 4);
+                const double kpad4 = 4.0 * ((Keff + 3) / 4);
                 cut_dim(jb.M, bm, cut_m);
                 cut_dim(jb.N, bn, cut_n);
                 for (auto& a : cut_m)
@@ -559,13 +602,13 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
             const int ob = tasks[idx[i]].out_blk;
             int nst = 0;
             while (j < idx.size() && tasks[idx[j]].out_blk == ob) {
-                if (tasks[idx[j]].l_off >= 0) nst += (tasks[idx[j]].dLi + GEMM_BK - 1) / GEMM_BK;
+                if (tasks[idx[j]].l_off >= 0) nst += (zdim * tasks[idx[j]].dLi + GEMM_BK - 1) / GEMM_BK;
                 j++;
             }
-            const dmrg_psi_block& OB = P->blocks[ob];
-            const int v = choose_variant(OB.dl, OB.dr);
+            const dmrg_psi_block& OB = P->blocks[ob % nblk];   // complex plans: ob >= nblk = the imaginary-coefficient accumulator
+            const int v = choose_variant(zdim * OB.dl, OB.dr);
             const int bm = kVariants[v].bm, bn = kVariants[v].bn;
-            Group g{i, j, v, (OB.dl + bm - 1) / bm, (OB.dr + bn - 1) / bn, nst};
+            Group g{i, j, v, (zdim * OB.dl + bm - 1) / bm, (OB.dr + bn - 1) / bn, nst};
             // cost in units of 64x64x16 tile-stages
             tile_stages += (double)g.ntm * g.ntn * nst * (bm * bn / 4096.0);
             groups.push_back(g);
@@ -582,7 +625,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         std::vector<Seg> ident_segs, gemm_segs;
         for (const Group& g : groups) {
             const int ob = tasks[idx[g.i]].out_blk;
-            const dmrg_psi_block& OB = P->blocks[ob];
+            const dmrg_psi_block& OB = P->blocks[ob % nblk];
+            const int Mo = zdim * OB.dl;   // rows of the sigma block as the GEMM sees it (complex: (re, im) row pairs)
             ident_segs.clear();
             gemm_segs.clear();
             double kp4 = 0;
@@ -590,56 +634,67 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                 const Task& k = tasks[idx[q]];
                 const bool ident = k.l_off < 0;
                 Seg s;
+                const int Ki = zdim * k.dLi, Mk = zdim * k.dLo;   // K and M extents of this contribution
                 s.alpha = k.alpha;
-                s.K = k.dLi;
+                s.K = Ki;
                 s.flags = 0;
                 s.a_map = s.b_map = 0; s.a_o0 = 0; s.a_pitch = s.b_pitch = 0; s.a_bytes = s.b_bytes = 0;
                 auto set_a = [&](int32_t id, BoxShape b) { s.a_map = id; s.a_pitch = (uint16_t)b.inner; s.a_bytes = 8u * b.inner * b.outer; };
                 auto set_b = [&](int32_t id, BoxShape b) { s.b_map = id; s.b_pitch = (uint16_t)b.inner; s.b_bytes = 8u * b.inner * b.outer; };
                 if (ident) { s.a_off = 0; s.lda = 0; s.flags |= SEG_A_IDENT; }
                 else {
-                    s.a_off = k.l_off; s.lda = (int)round_up2(k.l_trans ? k.dLo : k.dLi);
+                    s.a_off = k.l_off; s.lda = Z ? 2 * (k.l_trans ? k.dLo : k.dLi) : (int)round_up2(k.l_trans ? k.dLo : k.dLi);
                     s.flags |= (SP_OPS << SEG_A_SPACE_SHIFT) | (k.l_trans ? SEG_A_MCONTIG : 0);
-                    const BoxShape ba = box_shape(k.l_trans ? 1 : 0, k.dLi, k.dLo, TILE);
-                    set_a(k.l_trans ? maps.get(MS_OPS, k.l_off, 1, k.dLo, k.dLi, s.lda, ba) : maps.get(MS_OPS, k.l_off, 0, k.dLi, k.dLo, s.lda, ba), ba);
+                    const BoxShape ba = box_shape(k.l_trans ? 1 : 0, Ki, Mk, TILE);
+                    set_a(k.l_trans ? maps.get(MS_OPS, k.l_off, 1, Mk, Ki, s.lda, ba) : maps.get(MS_OPS, k.l_off, 0, Ki, Mk, s.lda, ba), ba);
                 }
                 if (k.r_off < 0) {
                     const dmrg_psi_block& IB = P->blocks[k.in_blk];
                     s.b_off = ppad[k.in_blk]; s.ldb = (int)round_up2(IB.dr);
                     s.flags |= (SP_PSI << SEG_B_SPACE_SHIFT);
-                    if (ident) alg_bytes += 8.0 * k.dLi * k.dRi;
-                    else { const BoxShape bb = box_shape(1, k.dLi, IB.dr, TILE); set_b(maps.get(MS_PSI, ppad[k.in_blk], 1, IB.dr, IB.dl, s.ldb, bb), bb); }
+                    if (ident) alg_bytes += 8.0 * zdim * k.dLi * k.dRi;
+                    else { const BoxShape bb = box_shape(1, Ki, IB.dr, TILE); set_b(maps.get(MS_PSI, ppad[k.in_blk], 1, IB.dr, zdim * IB.dl, s.ldb, bb), bb); }
                 } else {
                     const XLoc xl = xloc.at(xkey(k.r_off, k.r_trans, k.in_blk, nblk));
                     s.b_off = xl.off; s.ldb = xl.ld;
                     s.flags |= (SP_X << SEG_B_SPACE_SHIFT);
                     if (!ident) {   // the X slice of this task as a matrix of its own: dLi rows x dRo columns, row pitch = the stage-1 job's
-                        const BoxShape bb = box_shape(1, k.dLi, k.dRo, TILE);
-                        set_b(maps.get(MS_X, xl.off, 1, k.dRo, k.dLi, xl.ld, bb), bb);
+                        const BoxShape bb = box_shape(1, Ki, k.dRo, TILE);
+                        set_b(maps.get(MS_X, xl.off, 1, k.dRo, Ki, xl.ld, bb), bb);
                     }
-                    alg_flops += 2.0 * k.dLi * k.dRi * k.dRo;
+                    if (k.canon) alg_flops += 2.0 * zdim * zdim * k.dLi * k.dRi * k.dRo;
                 }
                 if (!ident) {
-                    kp4 += 4.0 * ((k.dLi + 3) / 4);
-                    s2_flops += 2.0 * k.dLo * k.dLi * k.dRo;
-                    alg_flops += 2.0 * k.dLo * k.dLi * k.dRo;
-                    alg_bytes += 8.0 * ((double)k.dLo * k.dLi + (double)k.dLi * k.dRo);
+                    kp4 += 4.0 * ((Ki + 3) / 4);
+                    s2_flops += 2.0 * Mk * Ki * k.dRo;
+                    if (k.canon) alg_flops += 2.0 * Mk * Ki * k.dRo;
+                    alg_bytes += 8.0 * ((double)Mk * Ki + (double)Ki * k.dRo);
                 }
                 (ident ? ident_segs : gemm_segs).push_back(s);
-                if (k.in_blk == k.out_blk) {
+                if (k.in_blk == k.out_blk % nblk && !Z) {
                     // diagonal term: with release_r_store the R diagonal is read from the packed copy (same pitch; a
                     // transposed copy has the same diagonal), addressed like the packed segments: kPackBase + offset
-                    const int64_t r_at = k.r_off < 0 ? kHdIdent : (kReleaseR ? kPackBase + pack_loc.at(k.r_off * 2 + k.r_trans) : k.r_off);
-                    O.hd.push_back({(int32_t)ob, HdItem{k.l_off < 0 ? kHdIdent : k.l_off, r_at, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha}});
+                    const int64_t r_at = k.r_off < 0 ? kHdIdent : (kReleaseR ? kPackBase + pack_loc.at(k.r_off * 2 + k.r_trans).first : k.r_off);
+                    O.hd.push_back({(int32_t)ob, HdItem{k.l_off < 0 ? kHdIdent : k.l_off, r_at, (int)round_up2(k.dLi), (int)round_up2(k.dRi), k.alpha, 0, 0}});
+                } else if (k.in_blk == k.out_blk % nblk) {
+                    // complex plan: diag += Re((ar + i ai) l r) -- this task carries ar (accumulator 0: ar Re(l r)) or ai
+                    // (accumulator 1: -ai Im(l r)).  l = (re, im) at [2i][2i] and, one image row below or -- the block used
+                    // conj-transposed -- one column to the right, of the L image; r always from the packed copy "as used":
+                    // re at [n][n] of the real-part rows, im at [n][n] of the imaginary-part rows.
+                    const auto pl = k.r_off < 0 ? std::pair<int64_t, int64_t>{0, 0} : pack_loc.at(k.r_off * 2 + k.r_trans);
+                    HdItem h{k.l_off < 0 ? kHdIdent : k.l_off, k.r_off < 0 ? kHdIdent : kPackBase + pl.first, 2 * k.dLi, 2 * (int)round_up2(k.dRi), k.alpha,
+                             k.l_trans ? 1 : 2 * k.dLi, pl.second};
+                    h.part = ob >= nblk;
+                    O.hd.push_back({(int32_t)(ob % nblk), h});
                 }
             }
-            cut_dim(OB.dl, kVariants[g.variant].bm, cut_m);
+            cut_dim(Mo, kVariants[g.variant].bm, cut_m);
             cut_dim(OB.dr, kVariants[g.variant].bn, cut_n);
-            padded_flops += 2.0 * frag_area(OB.dl, OB.dr) * kp4;
-            stage_flops += 2.0 * frag_area(OB.dl, OB.dr) * (double)GEMM_BK * g.nst;
+            padded_flops += 2.0 * frag_area(Mo, OB.dr) * kp4;
+            stage_flops += 2.0 * frag_area(Mo, OB.dr) * (double)GEMM_BK * g.nst;
             warp_flops += 2.0 * warp_area(cut_m, cut_n, g.variant) * (double)GEMM_BK * g.nst;
             tile_flops += 2.0 * (double)g.ntm * g.ntn * kVariants[g.variant].bm * kVariants[g.variant].bn * (double)GEMM_BK * g.nst;
-            alg_bytes += 16.0 * OB.dl * OB.dr;
+            alg_bytes += 16.0 * Mo * OB.dr;
             const int nsplit = (int)std::max(1.0, std::ceil(g.nst / smax));
             int part_no = 0;
             auto push_tiles = [&](std::vector<TileRec> (&recs)[NUM_VARIANTS], int job_id, double cost) {
@@ -648,7 +703,10 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                     for (auto& b : cut_n) recs[g.variant].push_back({{job_id, a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, cost, key});
             };
             Job jb;
-            jb.c_off = OB.offset; jb.ldc = OB.dr; jb.M = OB.dl; jb.N = OB.dr;
+            // complex plans accumulate into the plan's own buffer: two accumulators of psi_size doubles, block b of each at twice its
+            // offset, row-planar without padding (2 dl rows of dr)
+            const int64_t c_at = Z ? (int64_t)(ob / nblk) * P->psi_size + 2 * OB.offset : OB.offset;
+            jb.c_off = c_at; jb.ldc = OB.dr; jb.M = Mo; jb.N = OB.dr;
             jb.flags = (SP_SIGMA << JOB_C_SPACE_SHIFT) | JOB_BETA1;
             if (nsplit == 1) {
                 jb.seg_begin = (int32_t)segs.size();
@@ -662,7 +720,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                 // split-K: part p accumulates a contiguous range of segments into its own partial matrix;
                 // a final job adds the partials to sigma in part order (deterministic, no atomics)
                 const int ldp = (int)round_up2(OB.dr);
-                const int64_t psz = (int64_t)OB.dl * ldp;
+                const int64_t psz = (int64_t)Mo * ldp;
                 size_t sbeg = 0;
                 int done = 0, nparts = 0;
                 std::vector<int64_t> part_off;   // consecutive: part p lives at part_off[0] + p * psz
@@ -675,7 +733,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                         send++;
                     }
                     Job pj;
-                    pj.c_off = ptop; pj.ldc = ldp; pj.M = OB.dl; pj.N = OB.dr;
+                    pj.c_off = ptop; pj.ldc = ldp; pj.M = Mo; pj.N = OB.dr;
                     pj.flags = (SP_X << JOB_C_SPACE_SHIFT);
                     pj.seg_begin = (int32_t)segs.size();
                     if (nparts == 0) segs.insert(segs.end(), ident_segs.begin(), ident_segs.end());   // identity-L terms ride with part 0
@@ -690,7 +748,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
                     nparts++;
                     sbeg = send;
                 }
-                reds.push_back({OB.offset, part_off[0], psz, OB.dl, OB.dr, ldp, nparts});
+                reds.push_back({c_at, part_off[0], psz, Mo, OB.dr, ldp, nparts});
             }
             DMRG_REQUIRE(segs.size() < ((size_t)1 << 31) && jobs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
         }
@@ -836,7 +894,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
     P->stats[ST_S2_STAGES] = s2_tiles ? cost_acc2 / s2_tiles - 1.0 : 0.0;
     P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
                                          hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +
-                                         8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems);
+                                         8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems + (Z ? 16.0 * P->psi_size : 0.0));
     if (S->structure_only) return DMRG_OK;
     auto up = [&](void** dptr, const void* src, size_t bytes) -> int {
         DMRG_CUDA(cudaMalloc(dptr, std::max<size_t>(bytes, 16)));
@@ -844,6 +902,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         return DMRG_OK;
     };
     DMRG_CUDA(cudaMalloc(&P->d_psi_pad, sizeof(double) * (size_t)P->psi_pad_elems));
+    if (Z) DMRG_CUDA(cudaMalloc(&P->d_sigz, sizeof(double) * (size_t)std::max<int64_t>(2 * P->psi_size, 2)));
     DMRG_CUDA(cudaMalloc(&P->d_pack, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     DMRG_CUDA(cudaMemset(P->d_pack, 0, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     {   // the GEMM kernel addresses the packed store relative to the operator store (one flat device address space)
@@ -876,7 +935,8 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, int64_t nterms_in, c
         DMRG_CUDA(cudaMemcpy(d_packs, packs.data(), packs.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));
         for (size_t y0 = 0; y0 < packs.size(); y0 += 32768) {
             const unsigned ny = (unsigned)std::min<size_t>(32768, packs.size() - y0);
-            pack_r_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, S->d_values, P->d_pack);
+            if (Z) pack_r_z_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, S->d_values, P->d_pack);
+            else pack_r_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, S->d_values, P->d_pack);
         }
         DMRG_CUDA(cudaGetLastError());
         DMRG_CUDA(cudaDeviceSynchronize());
@@ -907,6 +967,88 @@ __global__ void __launch_bounds__(256) pack_r_kernel(const PackDesc* __restrict_
         else { n = (int)(e / d.dRi); k = (int)(e - (int64_t)n * d.dRi); }
         const double v = d.trans ? ops[d.src + (int64_t)k * d.src_ld + n] : ops[d.src + (int64_t)n * d.src_ld + k];
         pack[d.dst + (int64_t)n * d.ldp + k] = v;
+    }
+}
+
+// Complex plans: the real image of the R block as used (normal, or conj-transposed for an h.c. use), K-contiguous over both
+// halves of a row-planar psi row:   real-part row n = [ re R(n, :) | -im R(n, :) ],  imaginary-part row n = [ im R(n, :) | re R(n, :) ]
+// (halves of ldp / 2, pads stay zero).  The store keeps R blocks row-planar (ops_store.cu, mode 2).
+__global__ void __launch_bounds__(256) pack_r_z_kernel(const PackDesc* __restrict__ descs, const double* __restrict__ ops,
+                                                       double* __restrict__ pack) {
+    const PackDesc d = descs[blockIdx.y];
+    const int64_t n_el = (int64_t)d.dRo * d.dRi;
+    const int sh = d.src_ld / 2, kh = d.ldp / 2;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_el; e += (int64_t)gridDim.x * blockDim.x) {
+        int n, k;
+        double re, im;
+        if (d.trans) {
+            k = (int)(e / d.dRo); n = (int)(e - (int64_t)k * d.dRo);
+            re = ops[d.src + (int64_t)k * d.src_ld + n];
+            im = -ops[d.src + (int64_t)k * d.src_ld + sh + n];
+        } else {
+            n = (int)(e / d.dRi); k = (int)(e - (int64_t)n * d.dRi);
+            re = ops[d.src + (int64_t)n * d.src_ld + k];
+            im = ops[d.src + (int64_t)n * d.src_ld + sh + k];
+        }
+        double* r0 = pack + d.dst + (int64_t)n * d.ldp;
+        double* r1 = r0 + d.im_delta;
+        r0[k] = re; r0[kh + k] = -im;
+        r1[k] = im; r1[kh + k] = re;
+    }
+}
+
+// complex plans: interleaved psi -> row-planar padded copy (row i of a block = [re | im], halves of round_up2(dr))
+__global__ void __launch_bounds__(256) pad_psi_z_kernel(const HdBlock* __restrict__ blocks, const double* __restrict__ psi,
+                                                        double* __restrict__ pad) {
+    const HdBlock b = blocks[blockIdx.y];
+    const int pc = (b.dr + 1) & ~1, ld = 2 * pc;
+    const int64_t n = (int64_t)b.dl * ld;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / ld), jj = (int)(e - (int64_t)i * ld);
+        const int part = jj >= pc, j = jj - part * pc;
+        pad[b.pad_off + e] = j < b.dr ? psi[2 * (b.offset + (int64_t)i * b.dr + j) + part] : 0.0;
+    }
+}
+
+// complex plans: sigma = acc0 + i acc1, row-planar accumulators (block b at twice its offset: rows 2i, 2i+1 = re, im of
+// row i) -> interleaved (re, im) pairs in the caller's vector
+__global__ void __launch_bounds__(256) sigma_z_finish_kernel(const HdBlock* __restrict__ blocks, const double* __restrict__ acc0,
+                                                             const double* __restrict__ acc1, double* __restrict__ sigma) {
+    const HdBlock b = blocks[blockIdx.y];
+    const int64_t n = (int64_t)b.dl * b.dr;
+    const double* a0 = acc0 + 2 * b.offset;
+    const double* a1 = acc1 + 2 * b.offset;
+    for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(e / b.dr), j = (int)(e - (int64_t)i * b.dr);
+        const int64_t pr = (int64_t)(2 * i) * b.dr + j, pi = pr + b.dr;
+        sigma[2 * (b.offset + e)] = a0[pr] - a1[pi];
+        sigma[2 * (b.offset + e) + 1] = a0[pi] + a1[pr];
+    }
+}
+
+// complex plans: Hd[blk][i][j] = sum_items Re(alpha l_ii r_jj), written to both the real and the imaginary slot of the
+// element (the Davidson preconditioner acts on the vector as 2n reals).  A task carries the real part of its coefficient
+// (part 0: + ar Re(l r)) or the imaginary part (part 1: - ai Im(l r)).  One thread per element, items in plan order.
+__global__ void __launch_bounds__(256) hdiag_z_kernel(const HdBlock* __restrict__ blocks, const HdTile* __restrict__ tiles,
+                                                      const HdItem* __restrict__ items, const double* __restrict__ ops,
+                                                      double* __restrict__ diag) {
+    const HdTile t = tiles[blockIdx.x];
+    const HdBlock b = blocks[t.blk];
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    const int j = t.tj * 32 + tx;
+    for (int u = 0; u < 4; u++) {
+        const int i = t.ti * 32 + ty + 8 * u;
+        if (i >= b.dl || j >= b.dr) continue;
+        double acc = 0.0;
+        for (int q = b.item_begin; q < b.item_end; q++) {
+            const HdItem h = items[q];
+            double lr = 1.0, li = 0.0, rr = 1.0, ri = 0.0;
+            if (h.l_off != kHdIdent) { const double* p = ops + h.l_off + (int64_t)(2 * i) * h.ldl + 2 * i; lr = p[0]; li = p[h.l_im]; }
+            if (h.r_off != kHdIdent) { const double* p = ops + h.r_off + (int64_t)j * h.ldr + j; rr = p[0]; ri = p[h.r_im]; }
+            acc += h.part ? -h.alpha * (lr * ri + li * rr) : h.alpha * (lr * rr - li * ri);
+        }
+        diag[2 * (b.offset + (int64_t)i * b.dr + j)] = acc;
+        diag[2 * (b.offset + (int64_t)i * b.dr + j) + 1] = acc;
     }
 }
 
@@ -987,9 +1129,28 @@ int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms
     return dmrg_plan_create_opts(ops, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, &o, out);
 }
 
+static int plan_create_any(const dmrg_ops* ops, const dmrg_term* terms, const double* coef_im, int64_t nterms, const double* site_ops,
+                           const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
+                           const dmrg_plan_options* options, dmrg_plan** out);
+
 int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms, const double* site_ops,
                           const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
                           const dmrg_plan_options* options, dmrg_plan** out) {
+    if (ops && ops->cplx) { set_error("dmrg_plan_create: the store is complex (dmrg_ops_load_z): use dmrg_plan_create_z"); return DMRG_EINVAL; }
+    return plan_create_any(ops, terms, nullptr, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, options, out);
+}
+
+int dmrg_plan_create_z(const dmrg_ops* ops, const dmrg_term* terms, const double* coef_im, int64_t nterms, const double* site_ops,
+                       const int32_t* site_parity, int32_t nsite, int32_t n_total, const dmrg_plan_options* options, dmrg_plan** out) {
+    if (ops && !ops->cplx) { set_error("dmrg_plan_create_z: the store is real (dmrg_ops_load): use dmrg_plan_create"); return DMRG_EINVAL; }
+    return plan_create_any(ops, terms, coef_im, nterms, site_ops, site_parity, nsite, n_total, 0, options, out);
+}
+
+int32_t dmrg_plan_is_complex(const dmrg_plan* P) { return P && P->cplx ? 1 : 0; }
+
+static int plan_create_any(const dmrg_ops* ops, const dmrg_term* terms, const double* coef_im, int64_t nterms, const double* site_ops,
+                           const int32_t* site_parity, int32_t nsite, int32_t n_total, int32_t two_sz_total,
+                           const dmrg_plan_options* options, dmrg_plan** out) {
     if (!out) { set_error("dmrg_plan_create: out is NULL"); return DMRG_EINVAL; }
     *out = nullptr;
     if (!ops || nterms < 0 || (nterms > 0 && !terms) || !site_ops || !site_parity || nsite <= 0) {
@@ -1005,7 +1166,7 @@ int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t n
     P->ops = ops;
     int rc;
     try {
-        rc = plan_build(P, terms, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, make_policy(options));
+        rc = plan_build(P, terms, coef_im, nterms, site_ops, site_parity, nsite, n_total, two_sz_total, make_policy(options));
     } catch (const std::bad_alloc&) {
         set_error("dmrg_plan_create: out of host memory");
         rc = DMRG_ENOMEM;
@@ -1021,7 +1182,7 @@ int dmrg_plan_create_opts(const dmrg_ops* ops, const dmrg_term* terms, int64_t n
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
     cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
-    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io); cudaFree(P->d_tmaps);
+    cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io); cudaFree(P->d_tmaps); cudaFree(P->d_sigz);
     for (auto e : P->ev) cudaEventDestroy(e);
     if (P->dav) davidson_ws_free(P->dav);
     delete P;
@@ -1076,10 +1237,13 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t ng = P->groups.size();
     if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * ng], st));
-    DMRG_CUDA(cudaMemsetAsync(sigma, 0, sizeof(double) * (size_t)P->psi_size, st));
+    // complex plans accumulate in their own row-planar buffers (two accumulators) and write sigma out at the end
+    double* const acc = P->cplx ? P->d_sigz : sigma;
+    DMRG_CUDA(cudaMemsetAsync(acc, 0, sizeof(double) * (size_t)P->psi_size * (P->cplx ? 2 : 1), st));
     for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += 32768) {
         const unsigned ny = (unsigned)std::min<int64_t>(32768, P->n_hd_blocks - y0);
-        pad_psi_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_hd_blocks + y0, psi, P->d_psi_pad);
+        if (P->cplx) pad_psi_z_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_hd_blocks + y0, psi, P->d_psi_pad);
+        else pad_psi_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_hd_blocks + y0, psi, P->d_psi_pad);
     }
     DMRG_CUDA(cudaGetLastError());
     for (size_t gi = 0; gi < ng; gi++) {
@@ -1088,7 +1252,7 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         if (G.stage == 3) {   // first_launch / nlaunch index the reduction table here
             for (int y0 = 0; y0 < G.nlaunch; y0 += 32768) {
                 const unsigned ny = (unsigned)std::min(32768, G.nlaunch - y0);
-                splitk_reduce_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_reds + G.first_launch + y0, P->d_xws, sigma);
+                splitk_reduce_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_reds + G.first_launch + y0, P->d_xws, acc);
             }
             DMRG_CUDA(cudaGetLastError());
             if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
@@ -1097,10 +1261,17 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         for (int li = 0; li < G.nlaunch; li++) {   // more than one launch per group only with split_small (measurement aid)
             const PlanLaunch& L = P->launches[G.first_launch + li];
             int rc = launch_grouped_gemm(L.variant, P->copy_mode, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
-                                         P->ops->d_values, P->d_xws, P->d_psi_pad, sigma, P->d_tmaps, st);
+                                         P->ops->d_values, P->d_xws, P->d_psi_pad, acc, P->d_tmaps, st);
             if (rc != DMRG_OK) return rc;
         }
         if (P->timing) DMRG_CUDA(cudaEventRecord(P->ev[2 * gi + 1], st));
+    }
+    if (P->cplx) {
+        for (int64_t y0 = 0; y0 < P->n_hd_blocks; y0 += 32768) {
+            const unsigned ny = (unsigned)std::min<int64_t>(32768, P->n_hd_blocks - y0);
+            sigma_z_finish_kernel<<<dim3(8, ny), 256, 0, st>>>(P->d_hd_blocks + y0, P->d_sigz, P->d_sigz + P->psi_size, sigma);
+        }
+        DMRG_CUDA(cudaGetLastError());
     }
     if (P->comm) { const int rc = comm_all_reduce(P->comm, sigma, P->psi_size, st); if (rc != DMRG_OK) return rc; }   // sharded plan: sum the partial sigmas
     if (P->timing) { DMRG_CUDA(cudaEventRecord(P->ev[2 * ng + 1], st)); P->timing_valid = true; }
@@ -1127,7 +1298,9 @@ int dmrg_hdiag(dmrg_plan* P, double* diag, void* cuda_stream) {
     if (!P || !diag) { set_error("dmrg_hdiag: NULL argument"); return DMRG_EINVAL; }
     if (P->ops->structure_only) { set_error("dmrg_hdiag: the operator store was loaded without values (planning only)"); return DMRG_EINVAL; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (P->n_hd_tiles > 0)
+    if (P->n_hd_tiles > 0 && P->cplx)
+        hdiag_z_kernel<<<(unsigned)P->n_hd_tiles, 256, 0, st>>>(P->d_hd_blocks, P->d_hd_tiles, P->d_hd_items, P->ops->d_values, diag);
+    else if (P->n_hd_tiles > 0)
         hdiag_kernel<<<(unsigned)P->n_hd_tiles, 256, 0, st>>>(P->d_hd_blocks, P->d_hd_tiles, P->d_hd_items, P->ops->d_values, diag);
     DMRG_CUDA(cudaGetLastError());
     if (P->comm) return comm_all_reduce(P->comm, diag, P->psi_size, st);

@@ -3,13 +3,13 @@
 #include "common.h"
 
 constexpr int64_t kHdIdent = INT64_MIN;   // HdItem offset of an identity factor (a packed R block can sit below the store: plain negatives are addresses)
-struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; };
+struct HdItem { int64_t l_off, r_off; int32_t ldl, ldr; double alpha; int64_t l_im, r_im; int32_t part = 0, pad_ = 0; };   // l_im, r_im, part: complex plans (distance from the real to the imaginary part of a diagonal entry; 1 = imaginary-coefficient task)
 struct HdTile { int32_t blk; int16_t ti, tj; };   // 32 x 32 tile of a psi block
 struct HdBlock { int64_t offset; int32_t dl, dr; int32_t item_begin, item_end; int64_t pad_off; };   // pad_off: block in the padded psi copy
 
 struct RedJob { int64_t sigma_off, part_off, part_stride; int32_t M, N, ldp, nparts; };   // split-K reduction of one sigma block
 
-struct PackDesc { int64_t src, dst; int32_t dRo, dRi, src_ld, trans, ldp, pad_; };   // one R block copied into the packed stage-1 store
+struct PackDesc { int64_t src, dst; int32_t dRo, dRi, src_ld, trans, ldp, pad_; int64_t im_delta; };   // im_delta (complex plans): from a block's real-part rows to its imaginary-part rows in the pack   // one R block copied into the packed stage-1 store
 
 struct PlanLaunch { int variant; int stage; int64_t tile_begin, ntiles; };
 struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one stage of one chunk: mutually independent (stage 3: range of the RedJob table)
@@ -26,7 +26,9 @@ struct dmrg_plan {
     const dmrg_ops* ops = nullptr;
     std::vector<dmrg_psi_block> blocks;
     std::vector<int64_t> shard_terms;   // indices (into the caller's term array) of the terms this plan evaluates, in plan order
-    int64_t psi_size = 0;
+    int64_t psi_size = 0;   // doubles in psi / sigma (2 per number for a complex plan)
+    bool cplx = false;      // complex plan (dmrg_plan_create_z)
+    double* d_sigz = nullptr;   // complex plan: the two row-planar accumulators of dmrg_sigma (2 * psi_size doubles)
     dmrg::Job* d_jobs = nullptr;
     dmrg::Seg* d_segs = nullptr;
     dmrg::Tile* d_tiles = nullptr;

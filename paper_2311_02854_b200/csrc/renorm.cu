@@ -350,6 +350,7 @@ int dmrg_renormalize(const dmrg_ops* in, int32_t side, const dmrg_sector* new_se
                      const dmrg_renorm_options* options, void* cuda_stream, dmrg_ops** out, dmrg_renorm_stats* stats) {
     if (!out) { set_error("dmrg_renormalize: out is NULL"); return DMRG_EINVAL; }
     *out = nullptr;
+    if (in && in->cplx) { set_error("%s: complex stores (dmrg_ops_load_z) are served by dmrg_plan_create_z / dmrg_sigma / dmrg_hdiag / dmrg_davidson only", "dmrg_renormalize"); return DMRG_EINVAL; }
     dmrg_ops* S = new (std::nothrow) dmrg_ops();
     if (!S) { set_error("dmrg_renormalize: out of host memory"); return DMRG_ENOMEM; }
     int rc;
@@ -392,6 +393,7 @@ int64_t dmrg_ops_num_values(const dmrg_ops* S) {
 int dmrg_ops_export(const dmrg_ops* S, dmrg_op_desc* ops_out, dmrg_block_desc* blocks_out, double* values_out) {
     if (!S || !ops_out || !blocks_out || !values_out) { set_error("dmrg_ops_export: NULL argument"); return DMRG_EINVAL; }
     if (S->structure_only) { set_error("dmrg_ops_export: the store was loaded without values"); return DMRG_EINVAL; }
+    if (S->cplx) { set_error("%s: complex stores (dmrg_ops_load_z) are served by dmrg_plan_create_z / dmrg_sigma / dmrg_hdiag / dmrg_davidson only", "dmrg_ops_export"); return DMRG_EINVAL; }
     if (S->r_released) { set_error("dmrg_ops_export: the R-side blocks of this store were released to a plan"); return DMRG_EINVAL; }
     std::vector<UnpackDesc> desc;
     int64_t nb = 0, nv = 0;
@@ -440,6 +442,7 @@ int dmrg_ops_sectors(const dmrg_ops* S, int32_t side, dmrg_sector* out, int32_t 
 int dmrg_ops_join(dmrg_ops* left, dmrg_ops* right, dmrg_ops** out) {
     if (!left || !right || !out) { set_error("dmrg_ops_join: NULL argument"); return DMRG_EINVAL; }
     *out = nullptr;
+    if (left->cplx || right->cplx) { set_error("%s: complex stores (dmrg_ops_load_z) are served by dmrg_plan_create_z / dmrg_sigma / dmrg_hdiag / dmrg_davidson only", "dmrg_ops_join"); return DMRG_EINVAL; }
     if (left->structure_only || right->structure_only || left->owned.empty() || right->owned.empty()) { set_error("dmrg_ops_join: both stores must hold device values"); return DMRG_EINVAL; }
     if (!left->sec[1].empty() || !right->sec[0].empty() || left->sec[0].empty() || right->sec[1].empty()) {
         set_error("dmrg_ops_join: `left` must hold only side-0 operators and `right` only side-1 operators");
@@ -557,6 +560,7 @@ static int form_lincombs(const dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t
 int dmrg_ops_add_lincombs(dmrg_ops* S, const dmrg_op_desc* lin_ops, int32_t n_lin_ops, const int64_t* lin_ptr, const int32_t* lin_op,
                           const double* lin_coef, const int32_t* lin_trans, int32_t nlin) {
     if (!S || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_add_lincombs: NULL or empty argument"); return DMRG_EINVAL; }
+    if (S->cplx) { set_error("%s: complex stores (dmrg_ops_load_z) are served by dmrg_plan_create_z / dmrg_sigma / dmrg_hdiag / dmrg_davidson only", "dmrg_ops_add_lincombs"); return DMRG_EINVAL; }
     if (S->structure_only || S->owned.empty() || S->r_released) { set_error("dmrg_ops_add_lincombs: the store holds no device values (or its R side was released)"); return DMRG_EINVAL; }
     std::vector<std::vector<int64_t>> new_off;
     std::vector<std::vector<int32_t>> new_colsec;
@@ -588,6 +592,7 @@ int dmrg_ops_derive(const dmrg_ops* src, const dmrg_op_desc* lin_ops, int32_t n_
     if (!out) { set_error("dmrg_ops_derive: out is NULL"); return DMRG_EINVAL; }
     *out = nullptr;
     if (!src || !lin_ops || n_lin_ops <= 0 || !lin_ptr || !lin_op || !lin_coef) { set_error("dmrg_ops_derive: NULL or empty argument"); return DMRG_EINVAL; }
+    if (src->cplx) { set_error("%s: complex stores (dmrg_ops_load_z) are served by dmrg_plan_create_z / dmrg_sigma / dmrg_hdiag / dmrg_davidson only", "dmrg_ops_derive"); return DMRG_EINVAL; }
     if (src->structure_only || src->owned.empty() || src->r_released) { set_error("dmrg_ops_derive: the source store holds no device values (or its R side was released)"); return DMRG_EINVAL; }
     dmrg_ops* D = new (std::nothrow) dmrg_ops();
     if (!D) { set_error("dmrg_ops_derive: out of host memory"); return DMRG_ENOMEM; }
