@@ -41,7 +41,8 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=8)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 of BASELINE.json (default: the headline K=73 D=3000)")
+    ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 of BASELINE.json (default: the headline K=73 D=3000); so2 / so3: the spin-orbit "
+                                                     "variants (complex FP64, N only; SURVEY section 8(f) NEXT-4) of cfg2 / cfg3, --sigma-only only")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="X workspace (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -279,7 +280,14 @@ def main():
     t_plan = time.perf_counter() - t0
     st = plan.stats()
     n = plan.psi_size
-    psi_h = random_psi(n, 5)
+    is_z = np.dtype(getattr(pr, "dtype", np.float64)).kind == "c"
+    if is_z:
+        from dmrg_workload.problem import random_psi_z
+        if args.sigma_only <= 0:
+            raise SystemExit("bench.py: the spin-orbit configs are measured with --sigma-only N (the headline metric is BASELINE.json's real cfg5)")
+        psi_h = random_psi_z(n // 2, 5)   # psi_size counts doubles
+    else:
+        psi_h = random_psi(n, 5)
     x = torch.from_numpy(psi_h).cuda()
     sig = torch.empty_like(x)
 
@@ -293,7 +301,20 @@ def main():
             rows.append(plan.stage_ms())
         med = [float(np.median([r[i] for r in rows])) for i in range(3)]
         fl = st["s1_flops"] + st["s2_flops"]
-        print(json.dumps({"mode": "sigma-only", "config": workload_name(args.config, pr), "calls": args.sigma_only, "plan_options": popts,
+        zpar = None
+        if is_z and not args.no_cpu_baseline:
+            # parity of this launch configuration against the complex oracle on sampled sigma blocks (largest one first)
+            from oracle import zsigma
+            lay = np.asarray(pr.layout)
+            sizes = lay[:, 4] * lay[:, 5]
+            blocks = [int(np.argmax(sizes)), int(np.argmin(sizes))] + [int(b) for b in np.random.Generator(np.random.Philox(1234)).permutation(len(lay))[:3]]
+            t0 = time.perf_counter()
+            ref = zsigma.zopair_sigma(pr, psi_h, only_out=blocks)
+            got = sig.cpu().numpy()
+            err = max(float(np.abs(got[int(lay[b][6]):int(lay[b][6] + sizes[b])] - ref[int(lay[b][6]):int(lay[b][6] + sizes[b])]).max()) for b in blocks)
+            zpar = {"max_abs_err_over_norm": err / float(np.linalg.norm(got)), "blocks_checked": len(blocks), "largest_block": [int(lay[blocks[0]][4]), int(lay[blocks[0]][5])],
+                    "tolerance": 1e-11, "oracle": "oracle/zsigma.py", "oracle_seconds": time.perf_counter() - t0}
+        print(json.dumps({"mode": "sigma-only", "dtype": "c128 (as real FP64 GEMMs, 8 MNK flops per complex GEMM)" if is_z else "f64", "parity_sampled": zpar, "config": workload_name(args.config, pr), "calls": args.sigma_only, "plan_options": popts,
                           "stage1_ms": med[0], "stage2_ms": med[1], "hpsi_ms": med[2], "executed_tflops": fl / med[2] * 1e-9,
                           "s1_tflops": st["s1_flops"] / med[0] * 1e-9, "s2_tflops": st["s2_flops"] / med[1] * 1e-9,
                           "launches_per_hpsi": int(st["launches"]), "chunks": int(st["chunks"]),

@@ -2,7 +2,7 @@
 import numpy as np
 
 from .blocking import build_block
-from .integrals import make_integrals
+from .integrals import make_integrals, make_so_integrals
 from .sectors import block_sector_model
 from .store import assemble, block_values_from_rblocks, sectors_of
 from .terms import Partition, TermTable
@@ -56,6 +56,8 @@ def make_direct_problem(K, nL, N_tot, twoSz_tot=0, D=1000, seed=1, banded=False,
     pr = assemble(tt, secL, secR, None, N_tot, twoSz_tot, direct_seed=None if structure_only else seed + 104729,
                   direct_scale=dmax ** -0.5)
     pr.meta = dict(K=K, nL=nL, nR=K - nL - 2, D=D, seed=seed, mode="direct", banded=banded)
+    if pr.dtype.kind == "c":
+        pr.meta["mode"] = "spin-orbit: complex, N only, direct"
     pr.ints, pr.part, pr.tt = ints, part, tt
     return pr
 
@@ -67,6 +69,10 @@ CONFIGS = {
     "cfg3": dict(gen="direct", K=36, nL=17, N_tot=36, D=1500, seed=1),
     "cfg4": dict(gen="direct", K=73, nL=35, N_tot=114, D=1000, seed=1, banded=True),
     "cfg5": dict(gen="direct", K=73, nL=35, N_tot=114, D=3000, seed=1, banded=True),
+    # spin-orbit variants (not BASELINE.json configs): complex integrals without spin
+    # selection rules (integrals.make_so_integrals), U(1)_N sectors only, direct fill with complex blocks
+    "so2": dict(gen="direct", K=24, nL=11, N_tot=24, D=500, seed=1, spin_orbit=True),
+    "so3": dict(gen="direct", K=36, nL=17, N_tot=36, D=1500, seed=1, spin_orbit=True),
 }
 
 
@@ -74,6 +80,8 @@ def make_config(name, **over):
     kw = dict(CONFIGS[name])
     kw.update(over)
     gen = kw.pop("gen")
+    if kw.pop("spin_orbit", False):
+        kw["ints"] = make_so_integrals(kw["K"], kw["seed"], banded=kw.get("banded", False))
     return make_blocked_problem(**kw) if gen == "blocked" else make_direct_problem(**kw)
 
 
