@@ -93,6 +93,45 @@ struct Tile {
 };
 static_assert(sizeof(Tile) == 16, "Tile layout");
 
+// What the kernel reads per CTA: the tile and everything it needs of its job in ONE 64-byte record, so that a CTA's first
+// global round trip is its only descriptor fetch before the segment list (tile -> job -> first non-identity segment used
+// to be three dependent loads, which short tiles -- a couple of pipeline stages -- cannot hide).  a_map0 / b_map0: the
+// tensor maps of the first GEMM segment, prefetched while that segment's descriptor is still on its way.
+struct alignas(64) TileDesc {
+    int64_t  c_off;
+    int32_t  ldc;
+    int32_t  m0, n0;
+    uint16_t rows, cols;
+    int32_t  seg_begin, seg_gemm, seg_end;   // [seg_begin, seg_gemm): identity-A segments, [seg_gemm, seg_end): GEMM segments
+    uint32_t flags;                          // JOB_*
+    int32_t  nstages;
+    int32_t  a_map0, b_map0;
+    int32_t  pad_[3];
+};
+static_assert(sizeof(TileDesc) == 64, "TileDesc layout");
+
+inline std::vector<TileDesc> make_tile_descs(const std::vector<Tile>& tiles, const std::vector<Job>& jobs, const std::vector<Seg>& segs) {
+    std::vector<int32_t> first_gemm(jobs.size());
+    for (size_t j = 0; j < jobs.size(); j++) {
+        int32_t s = jobs[j].seg_begin;
+        while (s < jobs[j].seg_end && (segs[s].flags & SEG_A_IDENT)) s++;
+        first_gemm[j] = s;
+    }
+    std::vector<TileDesc> out(tiles.size());
+    for (size_t t = 0; t < tiles.size(); t++) {
+        const Tile& T = tiles[t];
+        const Job& J = jobs[T.job];
+        TileDesc& d = out[t];
+        d.c_off = J.c_off; d.ldc = J.ldc; d.m0 = T.m0; d.n0 = T.n0; d.rows = T.rows; d.cols = T.cols;
+        d.seg_begin = J.seg_begin; d.seg_gemm = first_gemm[T.job]; d.seg_end = J.seg_end;
+        d.flags = J.flags; d.nstages = J.nstages;
+        const bool has = d.seg_gemm < d.seg_end;
+        d.a_map0 = has ? segs[d.seg_gemm].a_map : 0; d.b_map0 = has ? segs[d.seg_gemm].b_map : 0;
+        d.pad_[0] = d.pad_[1] = d.pad_[2] = 0;
+    }
+    return out;
+}
+
 // tile-shape variants of the grouped GEMM kernel
 struct TileShape { int bm, bn; };
 constexpr int NUM_VARIANTS = 1;
@@ -108,7 +147,7 @@ struct GemmLaunch {       // one launch of one kernel variant
     int64_t ntiles;
 };
 
-int launch_grouped_gemm(int variant, int copy_mode, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+int launch_grouped_gemm(int variant, int copy_mode, const Seg* segs, const TileDesc* tiles, int64_t ntiles,
                         const double* ops, double* xws, const double* psi, double* sigma, const TensorMap* tmaps, cudaStream_t st);
 int gemm_init();   // sets shared-memory attributes once
 

@@ -238,21 +238,20 @@ __device__ __forceinline__ void compute_stage(double (&acc)[FMe][FNe][2], uint32
 }
 
 struct ConsumerCtx {
-    const Job* job; const Seg* segs; const double* ops; double* xws; const double* psi; double* sigma;
+    const TileDesc* td; const Seg* segs; const double* ops; double* xws; const double* psi; double* sigma;
     uint32_t smem_u32; const StageMeta* meta; uint32_t full_u32, empty_u32;
     int m0, n0, m_lim, n_lim, nstages, lane, wm0, wn0, fm_eff, fn_eff;
 };
 
 // Everything one consumer warp does for one tile, with FMe x FNe accumulator fragments (<= the 4 x 4 of a 32x32
-// warp tile): identity-A segments, the mbarrier-paced main loop, the epilogue.  Fragments (i, j) with
-// i >= fm_eff or j >= fn_eff (a warp ragged in both directions keeps all its columns) are computed on
-// stale or neighbouring data and never stored.
+// warp tile): identity-A segments, the mbarrier-paced main loop, the epilogue.  FMe x FNe = the warp's fragment
+// counts (fm_eff, fn_eff), except for a warp without fragments, which runs the 1 x 1 body with any_frag = false.
 template <int BM, int BN, int NST, int FMe, int FNe>
 __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
     constexpr int A_ELEMS = (BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4);
     constexpr int B_ELEMS = (BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4);
     constexpr int STAGE_ELEMS = A_ELEMS + B_ELEMS;
-    const Job& job = *cx.job;
+    const TileDesc& job = *cx.td;
     const int lane = cx.lane, lr = lane >> 2, lc = lane & 3;
     const int m0 = cx.m0, n0 = cx.n0, wm0 = cx.wm0, wn0 = cx.wn0;
     const int fm_eff = cx.fm_eff, fn_eff = cx.fn_eff;
@@ -266,9 +265,8 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
         for (int j = 0; j < FNe; j++) acc[i][j][0] = acc[i][j][1] = 0.0;
 
     // ---- identity-A segments (planner puts them first): acc += alpha * B tile ---------------------
-    for (int sg = job.seg_begin; sg < job.seg_end; sg++) {
+    for (int sg = job.seg_begin; sg < job.seg_gemm; sg++) {
         const Seg s = cx.segs[sg];
-        if (!(s.flags & SEG_A_IDENT)) break;
         const double* b = space_r((s.flags >> SEG_B_SPACE_SHIFT) & 3u) + s.b_off;
 #pragma unroll
         for (int i = 0; i < FMe; i++) {
@@ -330,6 +328,23 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
     }
 }
 
+template <int BM, int BN, int NST, int FMe, int FN, int J>
+__device__ __forceinline__ void dispatch_cols(const ConsumerCtx& cx) {
+    if constexpr (J <= 1) consumer_body<BM, BN, NST, FMe, 1>(cx);
+    else {
+        if (cx.fn_eff >= J) consumer_body<BM, BN, NST, FMe, J>(cx);
+        else dispatch_cols<BM, BN, NST, FMe, FN, J - 1>(cx);
+    }
+}
+template <int BM, int BN, int NST, int FM, int FN, int I>
+__device__ __forceinline__ void dispatch_rows(const ConsumerCtx& cx) {
+    if constexpr (I <= 1) dispatch_cols<BM, BN, NST, 1, FN, FN>(cx);
+    else {
+        if (cx.fm_eff >= I) dispatch_cols<BM, BN, NST, I, FN, FN>(cx);
+        else dispatch_rows<BM, BN, NST, FM, FN, I - 1>(cx);
+    }
+}
+
 // Warp-specialised kernel.  Warps 0 .. WM*WN-1 are CONSUMERS (LDS + DMMA only, one TM x TN warp tile
 // each); the last warp is the PRODUCER, which walks the job's segment list and stages every operand tile.
 // The two sides meet only through per-stage mbarriers (full: one expect_tx arrival of the elected lane + the
@@ -338,7 +353,7 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
 // there is no CTA-wide barrier in the main loop and the consumer warps drift freely against each other.
 template <int BM, int BN, int WM, int WN, int NST, int MAXREG>
 __global__ void __launch_bounds__(32 * (WM * WN + 1)) __maxnreg__(MAXREG)
-grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, const Tile* __restrict__ tiles,
+grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ tiles,
                     const double* __restrict__ ops, double* __restrict__ xws, const double* __restrict__ psi,
                     double* __restrict__ sigma, const TensorMap* __restrict__ tmaps, int copy_mode) {
     constexpr int NCW = WM * WN;   // consumer warps
@@ -355,10 +370,9 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
-    const Tile tile = tiles[blockIdx.x];
-    const Job job = jobs[tile.job];
-    const int m0 = tile.m0, n0 = tile.n0;
-    const int m_lim = tile.rows, n_lim = tile.cols;   // <= BM, BN and inside the matrix (planner)
+    const TileDesc job = tiles[blockIdx.x];   // the tile and its job: one 64-byte record
+    const int m0 = job.m0, n0 = job.n0;
+    const int m_lim = job.rows, n_lim = job.cols;   // <= BM, BN and inside the matrix (planner)
     const int nstages = job.nstages;
     auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
 
@@ -376,14 +390,17 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
 
     if (warp >= NCW) {
         // =============================== producer warp ==============================================
-        int lseg = job.seg_begin;
-        while (lseg < job.seg_end && (segs[lseg].flags & SEG_A_IDENT)) lseg++;   // identity segments need no staging
+        int lseg = job.seg_gemm;   // identity segments need no staging
         if (lseg >= job.seg_end) return;
+        if (copy_mode == COPY_TMA) {
+            if (lane != 0) return;
+            tma_prefetch_desc(tmaps + job.a_map0);   // while the segment descriptor is on its way
+            tma_prefetch_desc(tmaps + job.b_map0);
+        }
         Seg ls = segs[lseg];
         int lk0 = 0;
         if (copy_mode == COPY_TMA) {
             // ---- TMA: one elected lane, two tensor copies per stage ------------------------------------
-            if (lane != 0) return;
             for (int it = 0; it < nstages; it++) {
                 const int slot = it % NST;
                 if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
@@ -450,35 +467,23 @@ grouped_gemm_kernel(const Job* __restrict__ jobs, const Seg* __restrict__ segs, 
     }
 
     // =================================== consumer warps ================================================
-    // The tile's 8x8 fragments are dealt out evenly to the WM x WN consumer warps (a 56 x 48 tile gives the
-    // 2 x 2 warps 4+3 by 3+3 fragments): the stage buffers couple the warps of a CTA, so the CTA advances at
-    // the pace of its most loaded warp.
+    // The tile's 8x8 fragments are dealt out to the WM x WN consumer warps (a 56 x 48 tile gives the 2 x 2 warps
+    // 4+3 by 3+3 fragments): the stage buffers couple the warps of a CTA, so the CTA advances at the pace of its
+    // most loaded warp.
     ConsumerCtx cx;
-    cx.job = &job; cx.segs = segs; cx.ops = ops; cx.xws = xws; cx.psi = psi; cx.sigma = sigma;
+    cx.td = &job; cx.segs = segs; cx.ops = ops; cx.xws = xws; cx.psi = psi; cx.sigma = sigma;
     cx.smem_u32 = smem_u32; cx.meta = meta; cx.full_u32 = full_u32; cx.empty_u32 = empty_u32;
     cx.m0 = m0; cx.n0 = n0; cx.m_lim = m_lim; cx.n_lim = n_lim; cx.nstages = nstages; cx.lane = lane;
+    // deal the tile's fragment rows / columns to the WM x WN warps as evenly as possible: the first (fr % W) warp rows get one more
     const int fr_m = (m_lim + 7) >> 3, fr_n = (n_lim + 7) >> 3;
-    const int per_m = (fr_m + WM - 1) / WM, per_n = (fr_n + WN - 1) / WN;
-    cx.wm0 = (warp / WN) * per_m * 8; cx.wn0 = (warp % WN) * per_n * 8;
-    cx.fm_eff = max(0, min(per_m, fr_m - (warp / WN) * per_m));
-    cx.fn_eff = max(0, min(per_n, fr_n - (warp % WN) * per_n));
-    // The whole consumer body (accumulators, main loop, epilogue) is specialised on the number of fragment rows
-    // OR columns of this warp, so a partly filled tile costs in proportion to its fragments.  (Specialising on
-    // both counts at once made ptxas spill; a warp ragged in both directions pads its columns to the warp tile.)
-    if (cx.fm_eff == FM || cx.fm_eff == 0) {
-        switch (cx.fn_eff) {
-            case 1: consumer_body<BM, BN, NST, FM, 1>(cx); break;
-            case 2: if constexpr (FN >= 2) consumer_body<BM, BN, NST, FM, 2>(cx); break;
-            case 3: if constexpr (FN >= 3) consumer_body<BM, BN, NST, FM, 3>(cx); break;
-            default: consumer_body<BM, BN, NST, FM, FN>(cx); break;   // full warp tile, or a warp with no fragment
-        }
-    } else {
-        switch (cx.fm_eff) {
-            case 1: consumer_body<BM, BN, NST, 1, FN>(cx); break;
-            case 2: if constexpr (FM >= 2) consumer_body<BM, BN, NST, 2, FN>(cx); break;
-            default: if constexpr (FM >= 3) consumer_body<BM, BN, NST, 3, FN>(cx); break;
-        }
-    }
+    const int wr = warp / WN, wc = warp % WN;
+    const int base_m = fr_m / WM, rem_m = fr_m % WM, base_n = fr_n / WN, rem_n = fr_n % WN;
+    cx.wm0 = (wr * base_m + min(wr, rem_m)) * 8; cx.wn0 = (wc * base_n + min(wc, rem_n)) * 8;
+    cx.fm_eff = base_m + (wr < rem_m ? 1 : 0);
+    cx.fn_eff = base_n + (wc < rem_n ? 1 : 0);
+    // The whole consumer body (accumulators, main loop, epilogue) is specialised on the warp's fragment rows AND columns, so a
+    // partly filled tile costs exactly its 8 x 8 fragments (a warp without fragments still walks the barriers).
+    dispatch_rows<BM, BN, NST, FM, FN, FM>(cx);
 }
 
 template <int BM, int BN>
@@ -512,13 +517,13 @@ int gemm_init() {
     return DMRG_OK;
 }
 
-int launch_grouped_gemm(int variant, int copy_mode, const Job* jobs, const Seg* segs, const Tile* tiles, int64_t ntiles,
+int launch_grouped_gemm(int variant, int copy_mode, const Seg* segs, const TileDesc* tiles, int64_t ntiles,
                         const double* ops, double* xws, const double* psi, double* sigma, const TensorMap* tmaps, cudaStream_t st) {
     if (ntiles <= 0) return DMRG_OK;
     const unsigned g = (unsigned)ntiles;
     switch (variant) {
-        case 0: V0<<<g, V0_T, V0_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
-        case 1: V1<<<g, V1_T, V1_S, st>>>(jobs, segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
+        case 0: V0<<<g, V0_T, V0_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
+        case 1: V1<<<g, V1_T, V1_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
     const cudaError_t e = cudaGetLastError();

@@ -892,7 +892,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     P->stats[ST_TILES_8W] = (double)tiles8;
     P->stats[ST_S1_STAGES] = s1_tiles ? cost_acc1 / s1_tiles - 1.0 : 0.0;
     P->stats[ST_S2_STAGES] = s2_tiles ? cost_acc2 / s2_tiles - 1.0 : 0.0;
-    P->stats[ST_DEVICE_BYTES] = (double)(jobs.size() * sizeof(Job) + segs.size() * sizeof(Seg) + tiles.size() * sizeof(Tile) +
+    P->stats[ST_DEVICE_BYTES] = (double)(segs.size() * sizeof(Seg) + tiles.size() * sizeof(TileDesc) +
                                          hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +
                                          8.0 * P->xws_elems + 8.0 * pack_top + 8.0 * P->psi_pad_elems + (Z ? 16.0 * P->psi_size : 0.0));
     if (S->structure_only) return DMRG_OK;
@@ -915,9 +915,11 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
         for (HdItem& h : hd_items) if (h.r_off >= kPackBase) h.r_off += delta - kPackBase;
     }
     int rc;
-    if ((rc = up((void**)&P->d_jobs, jobs.data(), jobs.size() * sizeof(Job)))) return rc;
     if ((rc = up((void**)&P->d_segs, segs.data(), segs.size() * sizeof(Seg)))) return rc;
-    if ((rc = up((void**)&P->d_tiles, tiles.data(), tiles.size() * sizeof(Tile)))) return rc;
+    {
+        const std::vector<TileDesc> td = make_tile_descs(tiles, jobs, segs);
+        if ((rc = up((void**)&P->d_tiles, td.data(), td.size() * sizeof(TileDesc)))) return rc;
+    }
     if ((rc = up((void**)&P->d_reds, reds.data(), reds.size() * sizeof(RedJob)))) return rc;
     if ((rc = up((void**)&P->d_hd_items, hd_items.data(), hd_items.size() * sizeof(HdItem)))) return rc;
     if ((rc = up((void**)&P->d_hd_blocks, hd_blocks.data(), hd_blocks.size() * sizeof(HdBlock)))) return rc;
@@ -1181,7 +1183,7 @@ static int plan_create_any(const dmrg_ops* ops, const dmrg_term* terms, const do
 
 void dmrg_plan_destroy(dmrg_plan* P) {
     if (!P) return;
-    cudaFree(P->d_jobs); cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
+    cudaFree(P->d_segs); cudaFree(P->d_tiles); cudaFree(P->d_xws);
     cudaFree(P->d_hd_items); cudaFree(P->d_hd_blocks); cudaFree(P->d_hd_tiles); cudaFree(P->d_reds); cudaFree(P->d_pack); cudaFree(P->d_psi_pad); cudaFree(P->d_host_io); cudaFree(P->d_tmaps); cudaFree(P->d_sigz);
     for (auto e : P->ev) cudaEventDestroy(e);
     if (P->dav) davidson_ws_free(P->dav);
@@ -1260,7 +1262,7 @@ int dmrg_sigma(dmrg_plan* P, const double* psi, double* sigma, void* cuda_stream
         }
         for (int li = 0; li < G.nlaunch; li++) {   // more than one launch per group only with split_small (measurement aid)
             const PlanLaunch& L = P->launches[G.first_launch + li];
-            int rc = launch_grouped_gemm(L.variant, P->copy_mode, P->d_jobs, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
+            int rc = launch_grouped_gemm(L.variant, P->copy_mode, P->d_segs, P->d_tiles + L.tile_begin, L.ntiles,
                                          P->ops->d_values, P->d_xws, P->d_psi_pad, acc, P->d_tmaps, st);
             if (rc != DMRG_OK) return rc;
         }

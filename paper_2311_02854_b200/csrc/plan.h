@@ -29,9 +29,8 @@ struct dmrg_plan {
     int64_t psi_size = 0;   // doubles in psi / sigma (2 per number for a complex plan)
     bool cplx = false;      // complex plan (dmrg_plan_create_z)
     double* d_sigz = nullptr;   // complex plan: the two row-planar accumulators of dmrg_sigma (2 * psi_size doubles)
-    dmrg::Job* d_jobs = nullptr;
     dmrg::Seg* d_segs = nullptr;
-    dmrg::Tile* d_tiles = nullptr;
+    dmrg::TileDesc* d_tiles = nullptr;   // one 64-byte record per CTA: the tile and its job (common.h)
     double* d_xws = nullptr;
     int64_t xws_elems = 0;
     std::vector<PlanLaunch> launches;

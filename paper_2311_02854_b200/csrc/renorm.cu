@@ -74,11 +74,11 @@ static int upload(T** dptr, const std::vector<T>& v) {
 }
 
 struct RenormScratch {   // transient device buffers of one dmrg_renormalize call
-    Job* d_jobs = nullptr; Seg* d_segs = nullptr; Tile* d_tiles = nullptr; TensorMap* d_tmaps = nullptr;
+    Seg* d_segs = nullptr; TileDesc* d_tiles = nullptr; TensorMap* d_tmaps = nullptr;
     double *d_w = nullptr, *d_y = nullptr;
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     ~RenormScratch() {
-        cudaFree(d_jobs); cudaFree(d_segs); cudaFree(d_tiles); cudaFree(d_tmaps); cudaFree(d_w); cudaFree(d_y);
+        cudaFree(d_segs); cudaFree(d_tiles); cudaFree(d_tmaps); cudaFree(d_w); cudaFree(d_y);
         if (e0) cudaEventDestroy(e0);
         if (e1) cudaEventDestroy(e1);
     }
@@ -307,9 +307,8 @@ static int renormalize_impl(const dmrg_ops* in, int side, const dmrg_sector* new
     DMRG_CUDA(cudaMalloc(&sc.d_w, sizeof(double) * hw.size()));
     DMRG_CUDA(cudaMemcpyAsync(sc.d_w, hw.data(), sizeof(double) * hw.size(), cudaMemcpyHostToDevice, st));
     DMRG_CUDA(cudaMalloc(&sc.d_y, sizeof(double) * (size_t)std::max<int64_t>(ypeak, 2)));
-    if ((rc = upload(&sc.d_jobs, jobs))) return rc;
     if ((rc = upload(&sc.d_segs, segs))) return rc;
-    if ((rc = upload(&sc.d_tiles, tiles))) return rc;
+    if ((rc = upload(&sc.d_tiles, make_tile_descs(tiles, jobs, segs)))) return rc;
     {
         double* const base[4] = {in->d_values, sc.d_y, sc.d_w, nullptr};
         std::vector<TensorMap> tm;
@@ -323,7 +322,7 @@ static int renormalize_impl(const dmrg_ops* in, int side, const dmrg_sector* new
     int nlaunch = 0;
     for (const Launch& L : launches) {
         if (L.ntiles == 0) continue;
-        if ((rc = launch_grouped_gemm(0, copy_mode, sc.d_jobs, sc.d_segs, sc.d_tiles + L.tile_begin, L.ntiles, in->d_values, sc.d_y, sc.d_w, out->d_values, sc.d_tmaps, st)))
+        if ((rc = launch_grouped_gemm(0, copy_mode, sc.d_segs, sc.d_tiles + L.tile_begin, L.ntiles, in->d_values, sc.d_y, sc.d_w, out->d_values, sc.d_tmaps, st)))
             return rc;
         nlaunch++;
     }
