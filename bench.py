@@ -50,7 +50,7 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="dmrg_plan_options field (copy_mode, split_waves, min_split_stages, max_merged_cols, "
-                         "cost_order_only, split_small, release_r_store, consumer_warps); repeatable")
+                         "cost_order_only, split_small, release_r_store); repeatable")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "shard"],
                     help="N > 1: replicas (default; BASELINE.json fixes the path to one GPU: N independent copies, weak scaling) or "
                          "shard (operator parallelism, PAPER.md:81,162: the terms are partitioned over the ranks and every H psi ends "
@@ -319,7 +319,7 @@ def main():
                           "s1_tflops": st["s1_flops"] / med[0] * 1e-9, "s2_tflops": st["s2_flops"] / med[1] * 1e-9,
                           "launches_per_hpsi": int(st["launches"]), "chunks": int(st["chunks"]),
                           "stats": {k: st[k] for k in ("s1_flops", "s2_flops", "padded_flops", "stage_flops", "warp_flops", "canon_flops", "s1_tiles", "s2_tiles",
-                                                       "s1_fill", "s2_fill", "tiles_8w")}}))
+                                                       "s1_fill", "s2_fill", "s1_stages", "s2_stages")}}))
         plan.destroy()
         ops.free()
         return

@@ -142,9 +142,6 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *                      get a launch of their own (same tiles, same results, more launches)
  *   release_r_store    1 = after packing, free the store's R-side blocks (the plan's packed copy is then the only
  *                      one; the store can serve no further dmrg_plan_create); 0 = keep (default)
- *   consumer_warps     kernel variant: 0 = default, chosen per launch from the mean fill of its 64 x 64 tiles (8 consumer
- *                      warps of 16 x 32 when the tiles are mostly ragged -- small sectors --, 4 warps of 32 x 32 otherwise);
- *                      4 or 8 force one variant.  Same tiles and the same per-element summation order either way.
  *   shard_rank, shard_count   operator parallelism ("distribute operators and partition mu"): with
  *                      shard_count > 1 the plan evaluates only its share of the terms -- one contiguous range of the
  *                      planner's ordered term list (ordered by R operator, so a range needs only its own complementary
@@ -163,8 +160,7 @@ typedef struct {
     int32_t split_small;
     int32_t release_r_store;
     int32_t shard_rank, shard_count;
-    int32_t consumer_warps;
-    int32_t reserved[5];
+    int32_t reserved[6];
 } dmrg_plan_options;
 
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,
@@ -195,7 +191,8 @@ int     dmrg_plan_psi_layout(const dmrg_plan* plan, dmrg_psi_block* out /* [host
  * 14 the same with M and N padded to whole tiles as well; 15 ... padded to each tile's most loaded warp
  * 16 doubles allocated for the X workspace (X intermediates + split-K partial tiles of the largest chunk)
  * 17 tensor maps of the TMA path (one per operand matrix and orientation, 128 bytes each)
- * 18 / 19 mean fill of the stage-1 / stage-2 tiles (8 x 8 fragments used / 64)   20 tiles launched with the 8-warp kernel
+ * 18 / 19 mean fill of the stage-1 / stage-2 tiles (8 x 8 fragments used / 64)
+ * 20 mean K per stage-1 tile   21 mean pipeline stages per stage-2 tile
  *                                           */
 double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
 

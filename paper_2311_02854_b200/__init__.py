@@ -25,7 +25,7 @@ assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
 
 PLANOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("min_split_stages", "<i4"), ("split_waves", "<f8"),
                        ("max_merged_cols", "<i4"), ("cost_order_only", "<i4"), ("split_small", "<i4"), ("release_r_store", "<i4"),
-                       ("shard_rank", "<i4"), ("shard_count", "<i4"), ("consumer_warps", "<i4"), ("reserved", "<i4", (5,))], align=True)
+                       ("shard_rank", "<i4"), ("shard_count", "<i4"), ("reserved", "<i4", (6,))], align=True)
 assert PLANOPT_DT.itemsize == 72
 COPY_LDGSTS, COPY_TMA = 1, 2
 WBLOCK_DT = np.dtype([("old_sector", "<i4"), ("site_state", "<i4"), ("new_sector", "<i4"), ("reserved", "<i4"), ("offset", "<i8")], align=True)
@@ -37,7 +37,7 @@ assert WBLOCK_DT.itemsize == 24 and RTERM_DT.itemsize == 24 and RENORMOPT_DT.ite
 
 STAT_KEYS = ("tasks", "alg_flops", "s1_flops", "s2_flops", "padded_flops", "s1_jobs", "chunks", "launches",
              "plan_device_bytes", "alg_bytes", "s1_tiles", "s2_tiles", "canon_flops", "stage_flops", "tile_flops", "warp_flops",
-             "xws_elems", "tensor_maps", "s1_fill", "s2_fill", "tiles_8w", "s1_stages", "s2_stages")
+             "xws_elems", "tensor_maps", "s1_fill", "s2_fill", "s1_stages", "s2_stages")
 
 EXPORTS = ("dmrg_ops_load", "dmrg_ops_free", "dmrg_ops_device_bytes", "dmrg_plan_create", "dmrg_plan_create_opts", "dmrg_plan_destroy",
            "dmrg_plan_psi_size", "dmrg_plan_shard_terms", "dmrg_plan_num_psi_blocks", "dmrg_plan_psi_layout", "dmrg_plan_stat", "dmrg_sigma",

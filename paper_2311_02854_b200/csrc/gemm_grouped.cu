@@ -492,19 +492,14 @@ constexpr size_t smem_bytes(int nst) {
            (((BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4)) + ((BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4)));
 }
 
-// variant table: must match kVariants.  <BM, BN, consumer warps M x N, stages, register cap>
-// Every variant uses 32x32 warp tiles (16 DMMA per 8 LDS.64 per k-step).
-//   V0 64x64, 2x2 consumer warps, BK = 32, 2 stages (72 KB), 128 registers, no spills -> 3 CTAs/SM.  Measured
-//      against BK = 16 / 2 stages / 96 registers / 4 CTAs/SM: cfg 5 +1.7 %, cfg 3 +1.0 %, cfg 4 -1.6 %, cfg 2 -2.2 %;
-//      3 stages x BK = 16, 4 stages, a second producer warp, double-buffered fragments: all slower.
-//   V1 the same tile with 4x2 consumer warps of 16x32 (8 fragments each, 8 DMMA per 6 LDS.64 per k-step), 72 registers,
-//      still 3 CTAs/SM but twice the resident warps: better on launches whose tiles are mostly ragged / short (cfg 2 +4 %,
-//      cfg 4 +3 %), worse on well-filled ones (cfg 5 -2 %: more shared-memory operand traffic per DMMA).  The planner picks
-//      per launch from the mean tile fill (dmrg_plan_options.consumer_warps).
+// The one instantiation: 64x64 tile, 2x2 consumer warps of 32x32 (16 DMMA per 8 LDS.64 per k-step), BK = 32, 2 stages
+// (72 KB), <= 128 registers, no spills -> 3 CTAs/SM.  Measured against it: BK = 16 with 2 / 3 / 4
+// stages, 3 stages of BK = 32, a second producer warp, double-buffered fragments, 128-wide tiles, 8 consumer warps of
+// 16x32 (better only while the consumer body padded ragged warps to whole warp tiles), a byte ring with up to 8 short
+// stages in flight: all slower.
 #define V0 grouped_gemm_kernel<64, 64, 2, 2, 2, 128>
-#define V1 grouped_gemm_kernel<64, 64, 4, 2, 2, 72>
-constexpr int V0_T = 32 * 5, V1_T = 32 * 9;
-constexpr size_t V0_S = smem_bytes<64, 64>(2), V1_S = smem_bytes<64, 64>(2);
+constexpr int V0_T = 32 * 5;
+constexpr size_t V0_S = smem_bytes<64, 64>(2);
 
 }  // namespace
 
@@ -512,7 +507,6 @@ int gemm_init() {
     static bool done = false;
     if (done) return DMRG_OK;
     DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
-    DMRG_CUDA(cudaFuncSetAttribute(V1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V1_S));
     done = true;
     return DMRG_OK;
 }
@@ -523,7 +517,6 @@ int launch_grouped_gemm(int variant, int copy_mode, const Seg* segs, const TileD
     const unsigned g = (unsigned)ntiles;
     switch (variant) {
         case 0: V0<<<g, V0_T, V0_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
-        case 1: V1<<<g, V1_T, V1_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
     const cudaError_t e = cudaGetLastError();

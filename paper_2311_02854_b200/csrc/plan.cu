@@ -86,11 +86,6 @@ constexpr int64_t kPackBase = int64_t(1) << 50;   // marks b_off values that are
 // DESIGN.md section 9 was taken with 4 resident CTAs per SM; the BK = 32 kernel keeps 3, the unit is kept so that the
 // recorded numbers stay comparable)
 constexpr double kCtaSlots = 148.0 * 4;
-// Kernel variant per launch (measured): the 8-consumer-warp kernel wins where tiles are short-lived or
-// ragged -- stage 1 when the mean K of its tiles is below kMeanKFor8Warps (a tile is then a couple of pipeline stages: latency,
-// not the pipe, is what it waits for), stage 2 when the mean fill of its 64 x 64 tiles is below kFillFor8Warps.
-constexpr double kStagesFor8Warps = 160.0;   // stage 1: mean K (k-columns) per tile
-constexpr double kFillFor8Warps = 0.72;      // stage 2: mean tile fill
 
 struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     int64_t workspace_bytes;
@@ -101,7 +96,6 @@ struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     int split_small;
     bool release_r_store;
     int shard_rank, shard_count;
-    int consumer_warps;   // 0 = per launch from the mean tile fill, 4 or 8 = forced
 };
 
 static PlanPolicy make_policy(const dmrg_plan_options* o) {
@@ -114,7 +108,6 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
     p.release_r_store = o && o->release_r_store;
-    p.consumer_warps = (o && (o->consumer_warps == 4 || o->consumer_warps == 8)) ? o->consumer_warps : 0;
     p.shard_count = (o && o->shard_count > 1) ? o->shard_count : 1;
     p.shard_rank = (o && o->shard_count > 1) ? o->shard_rank : 0;
     return p;
@@ -789,7 +782,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     std::vector<PackDesc> packs;   // packed R store (stage-1 B operands), filled on the device after upload
     std::vector<size_t> pack_segs;  // segments whose b_off is relative to the packed store
     MapTable maps;
-    int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0, tiles8 = 0;
+    int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0;
     double fill_acc1 = 0, fill_acc2 = 0, cost_acc1 = 0, cost_acc2 = 0;
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
     for (int64_t ch = 0; ch < nchunks; ch++) {
@@ -819,15 +812,9 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
             PlanGroup grp{stage, (int)P->launches.size(), 0};
             size_t i = 0;
             const size_t n = tl->tiles.size();
-            // kernel variant of this launch: 8 consumer warps when the tiles are mostly ragged (mean fill of the 64 x 64
-            // tiles below kFillFor8Warps), 4 consumer warps with 32 x 32 warp tiles otherwise
-            const double fill = n ? tl->frag_area / (4096.0 * (double)n) : 1.0;
-            const double mean_stages = n ? tl->cost / (double)n : 0.0;   // pipeline stages (+1) per tile
-            const bool want8 = stage == 1 ? mean_stages < kStagesFor8Warps : fill < kFillFor8Warps;
-            const int variant = pol.consumer_warps == 8 ? 1 : (pol.consumer_warps == 4 ? 0 : (want8 ? 1 : 0));
+            const int variant = 0;   // one kernel variant (64 x 64 tile, 2 x 2 consumer warps)
             (stage == 1 ? cost_acc1 : cost_acc2) += tl->cost;
             (stage == 1 ? fill_acc1 : fill_acc2) += tl->frag_area;
-            if (variant == 1) tiles8 += (int64_t)n;
             auto push_range = [&](size_t lo, size_t hi) {
                 while (lo < hi) {   // grid.x limit: split very long lists
                     const size_t cnt = std::min<size_t>(hi - lo, (size_t)1 << 30);
@@ -889,8 +876,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     P->stats[ST_TENSOR_MAPS] = (double)maps.descs.size();
     P->stats[ST_S1_FILL] = s1_tiles ? fill_acc1 / (4096.0 * s1_tiles) : 0.0;
     P->stats[ST_S2_FILL] = s2_tiles ? fill_acc2 / (4096.0 * s2_tiles) : 0.0;
-    P->stats[ST_TILES_8W] = (double)tiles8;
-    P->stats[ST_S1_STAGES] = s1_tiles ? cost_acc1 / s1_tiles - 1.0 : 0.0;
+    P->stats[ST_S1_STAGES] = s1_tiles ? cost_acc1 / s1_tiles : 0.0;   // stage-1 tile cost = K padded to 4
     P->stats[ST_S2_STAGES] = s2_tiles ? cost_acc2 / s2_tiles - 1.0 : 0.0;
     P->stats[ST_DEVICE_BYTES] = (double)(segs.size() * sizeof(Seg) + tiles.size() * sizeof(TileDesc) +
                                          hd_items.size() * sizeof(HdItem) + hd_blocks.size() * sizeof(HdBlock) + maps.descs.size() * sizeof(TensorMap) +

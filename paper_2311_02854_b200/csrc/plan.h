@@ -16,7 +16,7 @@ struct PlanGroup { int stage; int first_launch, nlaunch; };   // launches of one
 
 enum {
     ST_TASKS = 0, ST_ALG_FLOPS, ST_S1_FLOPS, ST_S2_FLOPS, ST_PADDED_FLOPS, ST_S1_JOBS, ST_CHUNKS, ST_LAUNCHES,
-    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_WARP_FLOPS, ST_XWS_ELEMS, ST_TENSOR_MAPS, ST_S1_FILL, ST_S2_FILL, ST_TILES_8W, ST_S1_STAGES, ST_S2_STAGES, ST_COUNT
+    ST_DEVICE_BYTES, ST_ALG_BYTES, ST_S1_TILES, ST_S2_TILES, ST_CANON_FLOPS, ST_STAGE_FLOPS, ST_TILE_FLOPS, ST_WARP_FLOPS, ST_XWS_ELEMS, ST_TENSOR_MAPS, ST_S1_FILL, ST_S2_FILL, ST_S1_STAGES, ST_S2_STAGES, ST_COUNT
 };
 
 struct DavidsonWs;

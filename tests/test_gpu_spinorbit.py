@@ -141,7 +141,7 @@ def test_plan_options_and_sharding():
     base = _sigma_gpu(plan, psi)
     assert np.abs(base - ref).max() / nrm <= TOL_SIGMA
     plan.destroy()
-    for opt, bitwise in ((dict(copy_mode=1), True), (dict(split_small=16), True), (dict(consumer_warps=4), None),
+    for opt, bitwise in ((dict(copy_mode=1), True), (dict(split_small=16), True),
                          (dict(split_waves=2000.0, min_split_stages=2), False), (dict(max_merged_cols=64), False),
                          (dict(workspace_bytes=1 << 20), False)):
         ws = opt.pop("workspace_bytes", 0)
