@@ -51,7 +51,7 @@ def parse():
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target CPU time of the oracle sample")
     ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE",
                     help="dmrg_plan_options field (copy_mode, split_waves, min_split_stages, max_merged_cols, "
-                         "cost_order_only, split_small, release_r_store); repeatable")
+                         "cost_order_only, split_small, release_r_store, tile_run_stages); repeatable")
     ap.add_argument("--parallelism", default="replicas", choices=["replicas", "shard"],
                     help="N > 1: replicas (default; BASELINE.json fixes the path to one GPU: N independent copies, weak scaling) or "
                          "shard (operator parallelism, PAPER.md:81,162: the terms are partitioned over the ranks and every H psi ends "

@@ -142,6 +142,9 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *                      get a launch of their own (same tiles, same results, more launches)
  *   release_r_store    1 = after packing, free the store's R-side blocks (the plan's packed copy is then the only
  *                      one; the store can serve no further dmrg_plan_create); 0 = keep (default)
+ *   tile_run_stages    stage 1: a CTA computes consecutive M tiles of one GEMM back to back (stage ring running on across
+ *                      them) until it has this many pipeline stages of work, at most 8 tiles (0 = default 32; 1 = one
+ *                      tile per CTA).  Same tiles and the same per-element summation order either way.
  *   shard_rank, shard_count   operator parallelism ("distribute operators and partition mu"): with
  *                      shard_count > 1 the plan evaluates only its share of the terms -- one contiguous range of the
  *                      planner's ordered term list (ordered by R operator, so a range needs only its own complementary
@@ -160,7 +163,8 @@ typedef struct {
     int32_t split_small;
     int32_t release_r_store;
     int32_t shard_rank, shard_count;
-    int32_t reserved[6];
+    int32_t tile_run_stages;
+    int32_t reserved[5];
 } dmrg_plan_options;
 
 int dmrg_plan_create(const dmrg_ops* ops, const dmrg_term* terms, int64_t nterms,

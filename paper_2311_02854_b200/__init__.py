@@ -25,7 +25,7 @@ assert TERM_DT.itemsize == 32 and PSIBLK_DT.itemsize == 32
 
 PLANOPT_DT = np.dtype([("workspace_bytes", "<i8"), ("copy_mode", "<i4"), ("min_split_stages", "<i4"), ("split_waves", "<f8"),
                        ("max_merged_cols", "<i4"), ("cost_order_only", "<i4"), ("split_small", "<i4"), ("release_r_store", "<i4"),
-                       ("shard_rank", "<i4"), ("shard_count", "<i4"), ("reserved", "<i4", (6,))], align=True)
+                       ("shard_rank", "<i4"), ("shard_count", "<i4"), ("tile_run_stages", "<i4"), ("reserved", "<i4", (5,))], align=True)
 assert PLANOPT_DT.itemsize == 72
 COPY_LDGSTS, COPY_TMA = 1, 2
 WBLOCK_DT = np.dtype([("old_sector", "<i4"), ("site_state", "<i4"), ("new_sector", "<i4"), ("reserved", "<i4"), ("offset", "<i8")], align=True)

@@ -89,9 +89,11 @@ static_assert(sizeof(Job) == 40, "Job layout");
 struct Tile {
     int32_t  job;
     int32_t  m0, n0;
-    uint16_t rows, cols;
+    uint16_t rows, cols;   // rows: of the LAST sub-tile when the tile is a run of M sub-tiles (reps > 1); the others are full
+    uint16_t reps = 1;     // consecutive BM-row sub-tiles this CTA computes one after the other (same columns)
+    uint16_t pad_ = 0;
 };
-static_assert(sizeof(Tile) == 16, "Tile layout");
+static_assert(sizeof(Tile) == 20, "Tile layout");
 
 // What the kernel reads per CTA: the tile and everything it needs of its job in ONE 64-byte record, so that a CTA's first
 // global round trip is its only descriptor fetch before the segment list (tile -> job -> first non-identity segment used
@@ -106,7 +108,8 @@ struct alignas(64) TileDesc {
     uint32_t flags;                          // JOB_*
     int32_t  nstages;
     int32_t  a_map0, b_map0;
-    int32_t  pad_[3];
+    int32_t  reps;                           // M sub-tiles of the kernel's BM rows computed back to back by this CTA (rows = those of the last one)
+    int32_t  pad_[2];
 };
 static_assert(sizeof(TileDesc) == 64, "TileDesc layout");
 
@@ -127,7 +130,8 @@ inline std::vector<TileDesc> make_tile_descs(const std::vector<Tile>& tiles, con
         d.flags = J.flags; d.nstages = J.nstages;
         const bool has = d.seg_gemm < d.seg_end;
         d.a_map0 = has ? segs[d.seg_gemm].a_map : 0; d.b_map0 = has ? segs[d.seg_gemm].b_map : 0;
-        d.pad_[0] = d.pad_[1] = d.pad_[2] = 0;
+        d.reps = T.reps;
+        d.pad_[0] = d.pad_[1] = 0;
     }
     return out;
 }

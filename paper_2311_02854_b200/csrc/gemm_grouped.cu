@@ -241,6 +241,7 @@ struct ConsumerCtx {
     const TileDesc* td; const Seg* segs; const double* ops; double* xws; const double* psi; double* sigma;
     uint32_t smem_u32; const StageMeta* meta; uint32_t full_u32, empty_u32;
     int m0, n0, m_lim, n_lim, nstages, lane, wm0, wn0, fm_eff, fn_eff;
+    int it0;   // ring position of this sub-tile's first stage (the ring runs on across the sub-tiles of a CTA)
 };
 
 // Everything one consumer warp does for one tile, with FMe x FNe accumulator fragments (<= the 4 x 4 of a 32x32
@@ -283,7 +284,7 @@ __device__ __forceinline__ void consumer_body(const ConsumerCtx& cx) {
     }
 
     // ---- main loop: wait for a full stage, LDS + DMMA, release it ---------------------------------
-    for (int it = 0; it < cx.nstages; it++) {
+    for (int it = cx.it0; it < cx.it0 + cx.nstages; it++) {
         const int slot = it % NST;
         mbar_wait(cx.full_u32 + 8 * slot, (it / NST) & 1);
         if (any_frag) {
@@ -371,9 +372,13 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     const TileDesc job = tiles[blockIdx.x];   // the tile and its job: one 64-byte record
-    const int m0 = job.m0, n0 = job.n0;
-    const int m_lim = job.rows, n_lim = job.cols;   // <= BM, BN and inside the matrix (planner)
-    const int nstages = job.nstages;
+    const int n0 = job.n0, n_lim = job.cols;   // <= BN and inside the matrix (planner)
+    const int nstages = job.nstages;   // per sub-tile
+    // A CTA computes job.reps sub-tiles of BM rows one after the other (same columns, same segment list; all but the last are
+    // full): the stage ring runs on across them, so the copies of the next sub-tile's first stages are in flight while the
+    // consumers finish and store the current one -- short tiles (stage 1 at small bond dimensions: K = d_R is a few stages)
+    // no longer pay a descriptor fetch and a pipeline fill each.
+    const int reps = job.reps;
     auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
 
     const uint32_t full_u32 = (uint32_t)__cvta_generic_to_shared(bar_full);
@@ -397,11 +402,12 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
             tma_prefetch_desc(tmaps + job.a_map0);   // while the segment descriptor is on its way
             tma_prefetch_desc(tmaps + job.b_map0);
         }
-        Seg ls = segs[lseg];
+        const Seg ls0 = segs[lseg];
+        Seg ls = ls0;
         int lk0 = 0;
         if (copy_mode == COPY_TMA) {
             // ---- TMA: one elected lane, two tensor copies per stage ------------------------------------
-            for (int it = 0; it < nstages; it++) {
+            for (int it = 0, rp = 0, m0 = job.m0, st = 0; rp < reps; it++) {
                 const int slot = it % NST;
                 if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
                 const uint32_t sa = smem_u32 + (uint32_t)slot * (STAGE_ELEMS * 8);
@@ -429,10 +435,15 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
                         }
                     }
                 }
+                if (++st == nstages) {   // next sub-tile: BM rows further down, the segment list again from its start
+                    st = 0; rp++; m0 += BM;
+                    lseg = job.seg_gemm; ls = ls0; lk0 = 0;
+                }
             }
             return;
         }
-        for (int it = 0; it < nstages; it++) {
+        for (int it = 0, rp = 0, m0 = job.m0, st = 0; rp < reps; it++) {
+            const int m_lim = rp + 1 < reps ? BM : job.rows;
             const int slot = it % NST;
             if (it >= NST) mbar_wait(empty_u32 + 8 * slot, ((it / NST) & 1) ^ 1);
             const uint32_t sa = smem_u32 + (uint32_t)slot * (STAGE_ELEMS * 8);
@@ -462,6 +473,10 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
                 lseg++;
                 if (lseg < job.seg_end) ls = segs[lseg];
             }
+            if (++st == nstages) {
+                st = 0; rp++; m0 += BM;
+                lseg = job.seg_gemm; ls = ls0; lk0 = 0;
+            }
         }
         return;
     }
@@ -473,17 +488,22 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
     ConsumerCtx cx;
     cx.td = &job; cx.segs = segs; cx.ops = ops; cx.xws = xws; cx.psi = psi; cx.sigma = sigma;
     cx.smem_u32 = smem_u32; cx.meta = meta; cx.full_u32 = full_u32; cx.empty_u32 = empty_u32;
-    cx.m0 = m0; cx.n0 = n0; cx.m_lim = m_lim; cx.n_lim = n_lim; cx.nstages = nstages; cx.lane = lane;
-    // deal the tile's fragment rows / columns to the WM x WN warps as evenly as possible: the first (fr % W) warp rows get one more
-    const int fr_m = (m_lim + 7) >> 3, fr_n = (n_lim + 7) >> 3;
+    cx.n0 = n0; cx.n_lim = n_lim; cx.nstages = nstages; cx.lane = lane;
     const int wr = warp / WN, wc = warp % WN;
-    const int base_m = fr_m / WM, rem_m = fr_m % WM, base_n = fr_n / WN, rem_n = fr_n % WN;
-    cx.wm0 = (wr * base_m + min(wr, rem_m)) * 8; cx.wn0 = (wc * base_n + min(wc, rem_n)) * 8;
-    cx.fm_eff = base_m + (wr < rem_m ? 1 : 0);
+    const int fr_n = (n_lim + 7) >> 3, base_n = fr_n / WN, rem_n = fr_n % WN;
+    cx.wn0 = (wc * base_n + min(wc, rem_n)) * 8;
     cx.fn_eff = base_n + (wc < rem_n ? 1 : 0);
-    // The whole consumer body (accumulators, main loop, epilogue) is specialised on the warp's fragment rows AND columns, so a
-    // partly filled tile costs exactly its 8 x 8 fragments (a warp without fragments still walks the barriers).
-    dispatch_rows<BM, BN, NST, FM, FN, FM>(cx);
+    for (int rp = 0; rp < reps; rp++) {
+        const int m_lim = rp + 1 < reps ? BM : job.rows;
+        cx.m0 = job.m0 + rp * BM; cx.m_lim = m_lim; cx.it0 = rp * nstages;
+        // deal the sub-tile's fragment rows / columns to the WM x WN warps as evenly as possible: the first (fr % W) warp rows get one more
+        const int fr_m = (m_lim + 7) >> 3, base_m = fr_m / WM, rem_m = fr_m % WM;
+        cx.wm0 = (wr * base_m + min(wr, rem_m)) * 8;
+        cx.fm_eff = base_m + (wr < rem_m ? 1 : 0);
+        // The whole consumer body (accumulators, main loop, epilogue) is specialised on the warp's fragment rows AND columns, so a
+        // partly filled tile costs exactly its 8 x 8 fragments (a warp without fragments still walks the barriers).
+        dispatch_rows<BM, BN, NST, FM, FN, FM>(cx);
+    }
 }
 
 template <int BM, int BN>

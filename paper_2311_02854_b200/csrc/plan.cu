@@ -96,6 +96,7 @@ struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     int split_small;
     bool release_r_store;
     int shard_rank, shard_count;
+    int tile_run_stages;   // stage 1: a CTA computes as many consecutive M tiles as it takes to reach this many pipeline stages (<= 8 tiles)
 };
 
 static PlanPolicy make_policy(const dmrg_plan_options* o) {
@@ -108,6 +109,7 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
     p.release_r_store = o && o->release_r_store;
+    p.tile_run_stages = (o && o->tile_run_stages > 0) ? o->tile_run_stages : 32;
     p.shard_count = (o && o->shard_count > 1) ? o->shard_count : 1;
     p.shard_rank = (o && o->shard_count > 1) ? o->shard_rank : 0;
     return p;
@@ -376,7 +378,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     // The chunks are planned independently of each other by all host threads, each into its own ChunkOut with
     // chunk-local job / segment / tensor-map indices and pack offsets; they are then appended in chunk order (the
     // result does not depend on the thread count).
-    struct TileList { std::vector<Tile> tiles; size_t nbig = 0; double frag_area = 0, cost = 0; };   // frag_area: 8x8 fragments of the tiles x 64   // sorted tiles of one stage; [0, nbig) = large-block jobs (split_small)
+    struct TileList { std::vector<Tile> tiles; size_t nbig = 0, ntiles = 0; double frag_area = 0, cost = 0; };   // ntiles: BM x BN tiles (a run of M sub-tiles counts each)   // frag_area: 8x8 fragments of the tiles x 64   // sorted tiles of one stage; [0, nbig) = large-block jobs (split_small)
     struct ChunkOut {
         std::vector<Job> jobs;
         std::vector<Seg> segs;
@@ -417,7 +419,12 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
                    }) - r.begin();
         out.nbig = nbig;
         out.tiles.reserve(r.size());
-        for (auto& x : r) { out.tiles.push_back(x.t); out.frag_area += frag_area(x.t.rows, x.t.cols); out.cost += x.cost; }
+        for (auto& x : r) {
+            out.tiles.push_back(x.t);
+            out.frag_area += frag_area(x.t.rows, x.t.cols) + (x.t.reps - 1) * frag_area(TILE, x.t.cols);
+            out.ntiles += x.t.reps;
+            out.cost += x.cost;
+        }
     };
 
     auto build_chunk = [&](int64_t ch, ChunkOut& O) -> int {
@@ -565,9 +572,17 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
                 const double kpad4 = 4.0 * ((Keff + 3) / 4);
                 cut_dim(jb.M, bm, cut_m);
                 cut_dim(jb.N, bn, cut_n);
-                for (auto& a : cut_m)
-                    for (auto& b : cut_n)
-                        recs1[v].push_back({{(int32_t)jobs.size(), a.first, b.first, (uint16_t)a.second, (uint16_t)b.second}, kpad4});
+                // short tiles (K = d_R is a few stages) are handed out in runs of consecutive M tiles: one CTA, one descriptor
+                // fetch, the stage ring running on from tile to tile
+                const size_t run = (size_t)std::min(8, std::max(1, (pol.tile_run_stages + jb.nstages - 1) / jb.nstages));
+                for (size_t a0 = 0; a0 < cut_m.size(); a0 += run) {
+                    const size_t a1 = std::min(cut_m.size(), a0 + run);
+                    for (auto& b : cut_n) {
+                        Tile t{(int32_t)jobs.size(), cut_m[a0].first, b.first, (uint16_t)cut_m[a1 - 1].second, (uint16_t)b.second};
+                        t.reps = (uint16_t)(a1 - a0);
+                        recs1[v].push_back({t, kpad4 * (double)(a1 - a0)});
+                    }
+                }
                 padded_flops += 2.0 * frag_area(jb.M, jb.N) * kpad4;
                 stage_flops += 2.0 * frag_area(jb.M, jb.N) * (double)GEMM_BK * jb.nstages;
                 warp_flops += 2.0 * warp_area(cut_m, cut_n, v) * (double)GEMM_BK * jb.nstages;
@@ -825,7 +840,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
             };
             if (tl->nbig > 0 && tl->nbig < n) { push_range(0, tl->nbig); i = tl->nbig; }
             push_range(i, n);
-            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)n;
+            (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)tl->ntiles;
             grp.nlaunch = (int)P->launches.size() - grp.first_launch;
             if (grp.nlaunch > 0) P->groups.push_back(grp);
             stage++;

@@ -215,6 +215,11 @@ def test_plan_options_give_the_same_sigma():
     assert np.array_equal(out, ref)
     out, _ = variant(copy_mode=g.COPY_TMA, cost_order_only=1)
     assert np.array_equal(out, ref)
+    for run in (1, 1000):                          # one stage-1 tile per CTA / runs of up to 8 M tiles per CTA: same tiles, same order
+        for cm in (g.COPY_TMA, g.COPY_LDGSTS):
+            out, st = variant(tile_run_stages=run, copy_mode=cm)
+            assert np.array_equal(out, ref), (run, cm)
+            assert st["s1_tiles"] == plan.stats()["s1_tiles"]
     for kw in (dict(split_waves=4000.0, min_split_stages=1), dict(max_merged_cols=64), dict(workspace_bytes=1, copy_mode=g.COPY_LDGSTS)):
         out, _ = variant(**kw)
         assert np.abs(out - orc).max() / np.linalg.norm(orc) <= TOL_SIGMA, kw
