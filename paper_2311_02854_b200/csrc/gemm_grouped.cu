@@ -352,7 +352,7 @@ __device__ __forceinline__ void dispatch_rows(const ConsumerCtx& cx) {
 // byte counts of the two TMA copies -- or, on the cp.async path, 32 cp.async-completion arrivals + 1 release
 // arrival; either way the arrival publishes the stage metadata; empty: one arrival per consumer warp), so
 // there is no CTA-wide barrier in the main loop and the consumer warps drift freely against each other.
-template <int BM, int BN, int WM, int WN, int NST, int MAXREG>
+template <int BM, int BN, int WM, int WN, int NST, int MAXREG, bool RUNS>
 __global__ void __launch_bounds__(32 * (WM * WN + 1)) __maxnreg__(MAXREG)
 grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ tiles,
                     const double* __restrict__ ops, double* __restrict__ xws, const double* __restrict__ psi,
@@ -378,7 +378,8 @@ grouped_gemm_kernel(const Seg* __restrict__ segs, const TileDesc* __restrict__ t
     // full): the stage ring runs on across them, so the copies of the next sub-tile's first stages are in flight while the
     // consumers finish and store the current one -- short tiles (stage 1 at small bond dimensions: K = d_R is a few stages)
     // no longer pay a descriptor fetch and a pipeline fill each.
-    const int reps = job.reps;
+    // (RUNS = false: the instantiation for launches whose tiles are all single, e.g. stage 2 -- the sub-tile loops fold away)
+    const int reps = RUNS ? job.reps : 1;
     auto space_r = [&](uint32_t sp) -> const double* { return sp == SP_OPS ? ops : (sp == SP_X ? xws : (sp == SP_PSI ? psi : sigma)); };
 
     const uint32_t full_u32 = (uint32_t)__cvta_generic_to_shared(bar_full);
@@ -512,12 +513,13 @@ constexpr size_t smem_bytes(int nst) {
            (((BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4)) + ((BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4)));
 }
 
-// The one instantiation: 64x64 tile, 2x2 consumer warps of 32x32 (16 DMMA per 8 LDS.64 per k-step), BK = 32, 2 stages
+// One tile shape, two instantiations (with / without the loop over a run of M sub-tiles): 64x64 tile, 2x2 consumer warps of 32x32 (16 DMMA per 8 LDS.64 per k-step), BK = 32, 2 stages
 // (72 KB), <= 128 registers, no spills -> 3 CTAs/SM.  Measured against it: BK = 16 with 2 / 3 / 4
 // stages, 3 stages of BK = 32, a second producer warp, double-buffered fragments, 128-wide tiles, 8 consumer warps of
 // 16x32 (better only while the consumer body padded ragged warps to whole warp tiles), a byte ring with up to 8 short
 // stages in flight: all slower.
-#define V0 grouped_gemm_kernel<64, 64, 2, 2, 2, 128>
+#define V0 grouped_gemm_kernel<64, 64, 2, 2, 2, 128, false>
+#define V0R grouped_gemm_kernel<64, 64, 2, 2, 2, 128, true>   // tiles may be runs of M sub-tiles (stage 1)
 constexpr int V0_T = 32 * 5;
 constexpr size_t V0_S = smem_bytes<64, 64>(2);
 
@@ -527,6 +529,7 @@ int gemm_init() {
     static bool done = false;
     if (done) return DMRG_OK;
     DMRG_CUDA(cudaFuncSetAttribute(V0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
+    DMRG_CUDA(cudaFuncSetAttribute(V0R, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)V0_S));
     done = true;
     return DMRG_OK;
 }
@@ -537,6 +540,7 @@ int launch_grouped_gemm(int variant, int copy_mode, const Seg* segs, const TileD
     const unsigned g = (unsigned)ntiles;
     switch (variant) {
         case 0: V0<<<g, V0_T, V0_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
+        case 1: V0R<<<g, V0_T, V0_S, st>>>(segs, tiles, ops, xws, psi, sigma, tmaps, copy_mode); break;
         default: set_error("launch_grouped_gemm: bad variant %d", variant); return DMRG_EINVAL;
     }
     const cudaError_t e = cudaGetLastError();

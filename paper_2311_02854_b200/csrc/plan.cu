@@ -827,7 +827,7 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
             PlanGroup grp{stage, (int)P->launches.size(), 0};
             size_t i = 0;
             const size_t n = tl->tiles.size();
-            const int variant = 0;   // one kernel variant (64 x 64 tile, 2 x 2 consumer warps)
+            const int variant = stage == 1 ? 1 : 0;   // 1: the instantiation whose tiles may be runs of M sub-tiles (stage 1)
             (stage == 1 ? cost_acc1 : cost_acc2) += tl->cost;
             (stage == 1 ? fill_acc1 : fill_acc2) += tl->frag_area;
             auto push_range = [&](size_t lo, size_t hi) {
