@@ -4,7 +4,9 @@
 #include <cstdarg>
 #include <cstdint>
 #include <cstdio>
+#include <algorithm>
 #include <string>
+#include <thread>
 #include <vector>
 
 #include "../../include/dmrg_sigma.h"
@@ -115,28 +117,41 @@ static_assert(sizeof(TileDesc) == 64, "TileDesc layout");
 
 inline std::vector<TileDesc> make_tile_descs(const std::vector<Tile>& tiles, const std::vector<Job>& jobs, const std::vector<Seg>& segs) {
     std::vector<int32_t> first_gemm(jobs.size());
-    for (size_t j = 0; j < jobs.size(); j++) {
-        int32_t s = jobs[j].seg_begin;
-        while (s < jobs[j].seg_end && (segs[s].flags & SEG_A_IDENT)) s++;
-        first_gemm[j] = s;
-    }
     std::vector<TileDesc> out(tiles.size());
-    for (size_t t = 0; t < tiles.size(); t++) {
-        const Tile& T = tiles[t];
-        const Job& J = jobs[T.job];
-        TileDesc& d = out[t];
-        d.c_off = J.c_off; d.ldc = J.ldc; d.m0 = T.m0; d.n0 = T.n0; d.rows = T.rows; d.cols = T.cols;
-        d.seg_begin = J.seg_begin; d.seg_gemm = first_gemm[T.job]; d.seg_end = J.seg_end;
-        d.flags = J.flags; d.nstages = J.nstages;
-        const bool has = d.seg_gemm < d.seg_end;
-        d.a_map0 = has ? segs[d.seg_gemm].a_map : 0; d.b_map0 = has ? segs[d.seg_gemm].b_map : 0;
-        d.reps = T.reps;
-        d.pad_[0] = d.pad_[1] = 0;
-    }
+    const unsigned nthr = std::max(1u, std::min(32u, std::thread::hardware_concurrency()));
+    auto parallel_for = [&](size_t n, auto&& body) {   // body(begin, end) on contiguous slices, all host threads
+        std::vector<std::thread> pool;
+        const size_t per = (n + nthr - 1) / nthr;
+        for (unsigned t = 1; t < nthr; t++)
+            if (t * per < n) pool.emplace_back([&, t] { body(t * per, std::min(n, (t + 1) * per)); });
+        body(0, std::min(n, per));
+        for (auto& th : pool) th.join();
+    };
+    parallel_for(jobs.size(), [&](size_t lo, size_t hi) {
+        for (size_t j = lo; j < hi; j++) {
+            int32_t s = jobs[j].seg_begin;
+            while (s < jobs[j].seg_end && (segs[s].flags & SEG_A_IDENT)) s++;
+            first_gemm[j] = s;
+        }
+    });
+    parallel_for(tiles.size(), [&](size_t lo, size_t hi) {
+        for (size_t t = lo; t < hi; t++) {
+            const Tile& T = tiles[t];
+            const Job& J = jobs[T.job];
+            TileDesc& d = out[t];
+            d.c_off = J.c_off; d.ldc = J.ldc; d.m0 = T.m0; d.n0 = T.n0; d.rows = T.rows; d.cols = T.cols;
+            d.seg_begin = J.seg_begin; d.seg_gemm = first_gemm[T.job]; d.seg_end = J.seg_end;
+            d.flags = J.flags; d.nstages = J.nstages;
+            const bool has = d.seg_gemm < d.seg_end;
+            d.a_map0 = has ? segs[d.seg_gemm].a_map : 0; d.b_map0 = has ? segs[d.seg_gemm].b_map : 0;
+            d.reps = T.reps;
+            d.pad_[0] = d.pad_[1] = 0;
+        }
+    });
     return out;
 }
 
-// tile-shape variants of the grouped GEMM kernel
+// tile shape of the grouped GEMM kernel (one: 64 x 64); launch variant 0 = single tiles, 1 = tiles may be runs of M sub-tiles
 struct TileShape { int bm, bn; };
 constexpr int NUM_VARIANTS = 1;
 extern const TileShape kVariants[NUM_VARIANTS];
@@ -144,12 +159,6 @@ extern const TileShape kVariants[NUM_VARIANTS];
 #define DMRG_GEMM_BK 32
 #endif
 constexpr int GEMM_BK = DMRG_GEMM_BK;   // k-columns per pipeline stage (8, 16 or 32); 32 measured best at cfg 5 / cfg 3
-
-struct GemmLaunch {       // one launch of one kernel variant
-    int     variant;
-    int64_t tile_begin;   // into the plan's device tile array
-    int64_t ntiles;
-};
 
 int launch_grouped_gemm(int variant, int copy_mode, const Seg* segs, const TileDesc* tiles, int64_t ntiles,
                         const double* ops, double* xws, const double* psi, double* sigma, const TensorMap* tmaps, cudaStream_t st);

@@ -800,29 +800,37 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     int64_t pack_top = 0, ws_peak = 0, s1_jobs = 0, s1_tiles = 0, s2_tiles = 0;
     double fill_acc1 = 0, fill_acc2 = 0, cost_acc1 = 0, cost_acc2 = 0;
     double alg_flops = 0, s1_flops = 0, s2_flops = 0, padded_flops = 0, alg_bytes = 0, stage_flops = 0, tile_flops = 0, warp_flops = 0;
+    // pass 1 (serial, cheap): where every chunk's tables go, the global tensor-map ids, launches, packs, diagonal items
+    std::vector<size_t> job_base(nchunks), seg_base(nchunks), tile_base(nchunks);
+    std::vector<int64_t> pack_base(nchunks);
+    std::vector<std::vector<int32_t>> map_ids(nchunks);
+    size_t njobs = 0, nsegs = 0, ntile_recs = 0;
     for (int64_t ch = 0; ch < nchunks; ch++) {
         ChunkOut& O = outs[ch];
         if (O.rc != DMRG_OK) { set_error("%s", O.err.c_str()); return O.rc; }
-        const size_t job_base = jobs.size(), seg_base = segs.size();
-        DMRG_REQUIRE(job_base + O.jobs.size() < ((size_t)1 << 31) && seg_base + O.segs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
-        std::vector<int32_t> map_id(O.maps.descs.size());
+        job_base[ch] = njobs; seg_base[ch] = nsegs; tile_base[ch] = ntile_recs; pack_base[ch] = pack_top;
+        DMRG_REQUIRE(njobs + O.jobs.size() < ((size_t)1 << 31) && nsegs + O.segs.size() < ((size_t)1 << 31), "dmrg_plan_create: descriptor table overflow");
+        std::vector<int32_t>& map_id = map_ids[ch];
+        map_id.resize(O.maps.descs.size());
         for (size_t m = 0; m < O.maps.descs.size(); m++) {
             MapDesc d = O.maps.descs[m];
             if (d.space == MS_PACK) d.off += pack_top;
-            map_id[m] = maps.get(d.space, d.off, d.kind, d.inner, d.outer, d.ld, BoxShape{d.box_inner, d.box_outer});
+            if (d.space == MS_PACK || d.space == MS_X) {
+                // unique inside the chunk already, and a packed stack or an X slice of one chunk is no operand of another:
+                // appended without the (hash) look-up that 4 M of these would cost
+                map_id[m] = (int32_t)maps.descs.size();
+                maps.descs.push_back(d);
+            } else
+                map_id[m] = maps.get(d.space, d.off, d.kind, d.inner, d.outer, d.ld, BoxShape{d.box_inner, d.box_outer});
         }
-        for (Job jb : O.jobs) { jb.seg_begin += (int32_t)seg_base; jb.seg_end += (int32_t)seg_base; jobs.push_back(jb); }
-        for (Seg sg : O.segs) {
-            if (!(sg.flags & SEG_A_IDENT)) { sg.a_map = map_id[sg.a_map]; sg.b_map = map_id[sg.b_map]; }
-            segs.push_back(sg);
-        }
-        for (size_t q : O.pack_segs) { segs[seg_base + q].b_off += pack_top; pack_segs.push_back(seg_base + q); }
+        for (size_t q : O.pack_segs) pack_segs.push_back(nsegs + q);
         for (PackDesc pd : O.packs) { pd.dst += pack_top; packs.push_back(pd); }
         for (auto& h : O.hd) {
             if (h.second.r_off >= kPackBase) h.second.r_off += pack_top;
             hd[h.first].push_back(h.second);
         }
         int stage = 1;
+        size_t tile_cursor = ntile_recs;   // the chunk's tiles: stage 1 then stage 2, each list in its sorted order
         for (TileList* tl : {&O.t1, &O.t2}) {
             PlanGroup grp{stage, (int)P->launches.size(), 0};
             size_t i = 0;
@@ -833,13 +841,13 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
             auto push_range = [&](size_t lo, size_t hi) {
                 while (lo < hi) {   // grid.x limit: split very long lists
                     const size_t cnt = std::min<size_t>(hi - lo, (size_t)1 << 30);
-                    P->launches.push_back({variant, stage, (int64_t)tiles.size(), (int64_t)cnt});
-                    for (size_t j = lo; j < lo + cnt; j++) { Tile t = tl->tiles[j]; t.job += (int32_t)job_base; tiles.push_back(t); }
+                    P->launches.push_back({variant, stage, (int64_t)(tile_cursor + lo), (int64_t)cnt});
                     lo += cnt;
                 }
             };
             if (tl->nbig > 0 && tl->nbig < n) { push_range(0, tl->nbig); i = tl->nbig; }
             push_range(i, n);
+            tile_cursor += n;
             (stage == 1 ? s1_tiles : s2_tiles) += (int64_t)tl->ntiles;
             grp.nlaunch = (int)P->launches.size() - grp.first_launch;
             if (grp.nlaunch > 0) P->groups.push_back(grp);
@@ -849,12 +857,47 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
             P->groups.push_back({3, (int)reds.size(), (int)O.reds.size()});
             reds.insert(reds.end(), O.reds.begin(), O.reds.end());
         }
+        njobs += O.jobs.size(); nsegs += O.segs.size(); ntile_recs = tile_cursor;
         pack_top += O.pack_top;
         ws_peak = std::max(ws_peak, O.ws_peak);
         s1_jobs += O.s1_jobs;
         alg_flops += O.alg_flops; s1_flops += O.s1_flops; s2_flops += O.s2_flops; padded_flops += O.padded_flops; alg_bytes += O.alg_bytes;
         stage_flops += O.stage_flops; tile_flops += O.tile_flops; warp_flops += O.warp_flops;
-        O = ChunkOut();   // release the chunk's host memory
+    }
+    // pass 2 (all host threads): the bulk copies -- jobs, segments (global map ids, pack offsets), tiles -- chunk by chunk
+    jobs.resize(njobs);
+    segs.resize(nsegs);
+    tiles.resize(ntile_recs);
+    {
+        const unsigned nthr = (unsigned)std::max<int64_t>(1, std::min<int64_t>({(int64_t)std::thread::hardware_concurrency(), nchunks, 32}));
+        std::atomic<int64_t> next{0};
+        auto worker = [&]() {
+            for (int64_t ch = next.fetch_add(1); ch < nchunks; ch = next.fetch_add(1)) {
+                ChunkOut& O = outs[ch];
+                const std::vector<int32_t>& map_id = map_ids[ch];
+                const size_t jb0 = job_base[ch], sg0 = seg_base[ch];
+                for (size_t j = 0; j < O.jobs.size(); j++) {
+                    Job jb = O.jobs[j];
+                    jb.seg_begin += (int32_t)sg0; jb.seg_end += (int32_t)sg0;
+                    jobs[jb0 + j] = jb;
+                }
+                for (size_t q = 0; q < O.segs.size(); q++) {
+                    Seg sg = O.segs[q];
+                    if (!(sg.flags & SEG_A_IDENT)) { sg.a_map = map_id[sg.a_map]; sg.b_map = map_id[sg.b_map]; }
+                    segs[sg0 + q] = sg;
+                }
+                for (size_t q : O.pack_segs) segs[sg0 + q].b_off += pack_base[ch];
+                size_t tpos = tile_base[ch];
+                for (TileList* tl : {&O.t1, &O.t2})
+                    for (Tile t : tl->tiles) { t.job += (int32_t)jb0; tiles[tpos++] = t; }
+                O = ChunkOut();   // release the chunk's host memory
+                std::vector<int32_t>().swap(map_ids[ch]);
+            }
+        };
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < nthr; t++) pool.emplace_back(worker);
+        worker();
+        for (auto& th : pool) th.join();
     }
 
     P->stats[ST_ALG_FLOPS] = alg_flops;
