@@ -216,13 +216,21 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     });
 
     // ---- enumerate tasks: (term, psi block, dot transition)  (Eq. 7 at the level of blocks) ------
+    // Terms are independent here: contiguous slices of the ordered term list are expanded by all host threads into slice-local
+    // task lists, which are then concatenated in slice order (the result does not depend on the thread count).
     std::vector<Task> tasks;
     std::vector<int64_t> term_task_begin(nterms + 1, 0);
     std::vector<double> term_flops(nterms, 0.0);
     double canon_flops = 0.0;
-    for (int64_t to = 0; to < nterms; to++) {
+    const unsigned n_enum_thr = (unsigned)std::max<int64_t>(1, std::min<int64_t>({(int64_t)std::thread::hardware_concurrency(), nterms / 64 + 1, 32}));
+    std::vector<std::vector<Task>> slice_tasks(n_enum_thr);
+    std::vector<int64_t> term_ntasks(nterms, 0);
+    auto enumerate_slice = [&](unsigned slice) {
+      std::vector<Task>& tasks = slice_tasks[slice];   // shadows the merged list on purpose
+      const int64_t to_lo = nterms * slice / n_enum_thr, to_hi = nterms * (slice + 1) / n_enum_thr;
+      for (int64_t to = to_lo; to < to_hi; to++) {
         const dmrg_term& T = terms[order[to]];
-        term_task_begin[to] = (int64_t)tasks.size();
+        const size_t ntasks_before = tasks.size();
         const cplx_t* o1 = site_ops + 16 * (size_t)T.dot1;
         const cplx_t* o2 = site_ops + 16 * (size_t)T.dot2;
         const cplx_t coef(T.coef, (Z && coef_im) ? coef_im[order[to]] : 0.0);
@@ -274,8 +282,18 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
                 }
             }
         }
+        term_ntasks[to] = (int64_t)(tasks.size() - ntasks_before);
+      }
+    };
+    {
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < n_enum_thr; t++) pool.emplace_back(enumerate_slice, t);
+        enumerate_slice(0);
+        for (auto& th : pool) th.join();
     }
-    term_task_begin[nterms] = (int64_t)tasks.size();
+    for (int64_t to = 0; to < nterms; to++) term_task_begin[to + 1] = term_task_begin[to] + term_ntasks[to];
+    tasks.reserve((size_t)term_task_begin[nterms]);
+    for (auto& v : slice_tasks) { tasks.insert(tasks.end(), v.begin(), v.end()); std::vector<Task>().swap(v); }
     // ---- operator parallelism: this plan keeps one contiguous range of the ORDERED term list -----------
     // The terms are ordered by R operator, so a range needs only its own complementary operators; ranges are cut where
     // the running canonical cost crosses k/shard_count of the total.  Every rank computes the same cuts (no communication);
