@@ -198,3 +198,37 @@ def test_plan_options_are_validated_and_structural():
     for p_ in (fine, narrow, plan):
         p_.destroy()
     ops.free()
+
+
+def test_tile_runs_only_regroup_stage1_tiles():
+    """dmrg_plan_options.tile_run_stages hands stage-1 tiles out in runs of consecutive M tiles (one CTA, one descriptor
+    fetch): the tiles, the work and the launches stay what they are; the plan holds fewer tile records."""
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr, structure_only=True)
+    single = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, tile_run_stages=1)
+    longer = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, tile_run_stages=1000)
+    a, b, c = plan.stats(), single.stats(), longer.stats()
+    for k in ("s1_tiles", "s2_tiles", "s1_flops", "s2_flops", "padded_flops", "tasks", "chunks", "launches", "s1_fill", "s2_fill"):
+        assert a[k] == b[k] == c[k], k
+    # 64 bytes per tile record: runs shrink the descriptor tables, one tile per CTA is the largest
+    assert c["plan_device_bytes"] <= a["plan_device_bytes"] < b["plan_device_bytes"]
+    for p_ in (single, longer, plan):
+        p_.destroy()
+    ops.free()
+
+
+def test_plan_is_the_same_whatever_the_thread_count():
+    """Terms and chunks are planned by all host threads and merged in order: the tables (here: every statistic and the
+    shard term lists) must not depend on how many threads the machine offers."""
+    import subprocess
+    import sys
+    code = ("import sys, json; sys.path.insert(0, %r); import paper_2311_02854_b200 as g; "
+            "from dmrg_workload.problem import make_direct_problem; "
+            "pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3); "
+            "ops, plan = g.load_problem(pr, structure_only=True, workspace_bytes=1 << 22); "
+            "print(json.dumps([plan.stats(), [int(t) for t in plan.shard_terms()[:50]]]))") % ROOT
+    outs = []
+    for cpus in ("0", None):
+        cmd = [sys.executable, "-c", code] if cpus is None else ["taskset", "-c", cpus, sys.executable, "-c", code]
+        outs.append(subprocess.run(cmd, check=True, capture_output=True, text=True).stdout.strip().splitlines()[-1])
+    assert outs[0] == outs[1]
