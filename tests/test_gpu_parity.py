@@ -227,6 +227,44 @@ def test_plan_options_give_the_same_sigma():
     ops.free()
 
 
+@pytest.mark.parametrize("copy_mode", [2, 1])
+def test_sigma_and_hdiag_write_nothing_outside_their_vectors(copy_mode):
+    """compute-sanitizer is closed on this GPU pool, so the bounds are checked by hand: sigma, the diagonal and psi sit
+    between guard bands holding a sentinel, the plan is forced into many chunks / split-K parts / tile runs with ragged
+    last sub-tiles, and after the calls the guards must be untouched, psi unchanged, sigma == the unguarded result."""
+    g = _gpu()
+    from dmrg_workload.problem import make_direct_problem
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr)
+    psi = random_psi(pr.psi_size, 21)
+    ref = _sigma_gpu(plan, psi)
+    plan.destroy()
+    n, G = pr.psi_size, 4096
+    sentinel = -1.2345e300
+    for kw in (dict(), dict(workspace_bytes=1 << 20, split_waves=4000.0, min_split_stages=1, tile_run_stages=1000)):
+        ws = kw.pop("workspace_bytes", 0)
+        p2 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, ws, copy_mode=copy_mode, **kw)
+        bufs = []
+        for _ in range(3):   # psi, sigma, diag
+            b = torch.full((n + 2 * G,), sentinel, dtype=torch.float64, device="cuda")
+            bufs.append(b)
+        d_psi, d_sig, d_dia = (b[G:G + n] for b in bufs)
+        d_psi.copy_(torch.from_numpy(psi))
+        p2.sigma(d_psi, d_sig, torch.cuda.current_stream())
+        p2.hdiag(d_dia, torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        for b in bufs:
+            assert bool((b[:G] == sentinel).all()) and bool((b[G + n:] == sentinel).all())
+        assert np.array_equal(d_psi.cpu().numpy(), psi)
+        out = d_sig.cpu().numpy()
+        if not kw:
+            assert np.array_equal(out, ref)
+        assert np.abs(out - ref).max() / np.linalg.norm(ref) <= TOL_SIGMA
+        assert np.isfinite(d_dia.cpu().numpy()).all()
+        p2.destroy()
+    ops.free()
+
+
 def test_release_r_store_frees_the_r_side_and_changes_nothing():
     """dmrg_plan_options.release_r_store: once stage 1 and the diagonal read the plan's packed copy of the R blocks, the
     store's R-side allocation is freed.  sigma is bitwise the same, the diagonal still matches the oracle, the store
