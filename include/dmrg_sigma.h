@@ -207,6 +207,8 @@ double  dmrg_plan_stat(const dmrg_plan* plan, int32_t key);
  * sigma element is accumulated by one thread block in plan order, no floating-point atomics.
  * A plan owns one X workspace and one padded copy of psi: calls on the same plan must be ordered (same stream,
  * or externally synchronised); use one plan per concurrent stream.
+ * The call allocates nothing and never synchronises (per-stage timing off, no communicator attached): it may be issued
+ * on a stream that is being captured into a CUDA graph, and the graph replayed (tests/test_gpu_parity.py).
  */
 int dmrg_sigma(dmrg_plan* plan, const double* psi, double* sigma, void* cuda_stream);
 

@@ -265,6 +265,34 @@ def test_sigma_and_hdiag_write_nothing_outside_their_vectors(copy_mode):
     ops.free()
 
 
+def test_sigma_can_be_captured_in_a_cuda_graph():
+    """dmrg_sigma only enqueues work on the caller's stream (no allocation, no synchronisation): it can be captured in a
+    CUDA graph and replayed -- the replay reads whatever psi holds then and gives bitwise the direct call's sigma."""
+    g = _gpu()
+    from dmrg_workload.problem import make_direct_problem
+    pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
+    ops, plan = g.load_problem(pr)
+    psi1, psi2 = random_psi(pr.psi_size, 31), random_psi(pr.psi_size, 32)
+    ref1, ref2 = _sigma_gpu(plan, psi1), _sigma_gpu(plan, psi2)
+    d_psi = torch.from_numpy(psi1).cuda()
+    d_sig = torch.zeros_like(d_psi)
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.graph(graph, stream=side):
+        plan.sigma(d_psi, d_sig, side)
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(d_sig.cpu().numpy(), ref1)
+    d_psi.copy_(torch.from_numpy(psi2))
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(d_sig.cpu().numpy(), ref2)
+    del graph
+    plan.destroy()
+    ops.free()
+
+
 def test_release_r_store_frees_the_r_side_and_changes_nothing():
     """dmrg_plan_options.release_r_store: once stage 1 and the diagonal read the plan's packed copy of the R blocks, the
     store's R-side allocation is freed.  sigma is bitwise the same, the diagonal still matches the oracle, the store
