@@ -513,8 +513,8 @@ constexpr size_t smem_bytes(int nst) {
            (((BM * KPAD > BK * (BM + 4)) ? BM * KPAD : BK * (BM + 4)) + ((BN * KPAD > BK * (BN + 4)) ? BN * KPAD : BK * (BN + 4)));
 }
 
-// One tile shape, two instantiations (with / without the loop over a run of M sub-tiles): 64x64 tile, 2x2 consumer warps of 32x32 (16 DMMA per 8 LDS.64 per k-step), BK = 32, 2 stages
-// (72 KB), <= 128 registers, no spills -> 3 CTAs/SM.  Measured against it: BK = 16 with 2 / 3 / 4
+// One tile shape, two instantiations (with / without the loop over a run of M sub-tiles): 64x64 tile, 2x2 consumer warps
+// of 32x32 (16 DMMA per 8 LDS.64 per k-step), BK = 32, 2 stages (72 KB), 114 / 128 registers, no spills -> 3 CTAs/SM.  Measured against it: BK = 16 with 2 / 3 / 4
 // stages, 3 stages of BK = 32, a second producer warp, double-buffered fragments, 128-wide tiles, 8 consumer warps of
 // 16x32 (better only while the consumer body padded ragged warps to whole warp tiles), a byte ring with up to 8 short
 // stages in flight: all slower.
