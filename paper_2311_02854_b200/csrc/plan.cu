@@ -328,19 +328,27 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     // ---- chunk the (ordered) terms by X workspace --------------------------------------------------
     auto x_elems = [zdim](const Task& k) { return (int64_t)k.dLi * zdim * round_up2(k.dRo); };
     int64_t ws_elems = workspace_bytes / 8;
-    {
-        int64_t max_term = 0;
-        std::unordered_map<int64_t, char> seen;
-        for (int64_t to = 0; to < nterms; to++) {
-            seen.clear();
-            int64_t need = 0;
-            for (int64_t i = term_task_begin[to]; i < term_task_begin[to + 1]; i++) {
-                const Task& k = tasks[i];
-                if (k.r_off < 0) continue;
-                if (seen.emplace(xkey(k.r_off, k.r_trans, k.in_blk, nblk), 1).second) need += x_elems(k);
+    {   // the workspace must hold the X products of the largest single term (terms are independent here: all host threads)
+        std::vector<int64_t> slice_max(n_enum_thr, 0);
+        auto max_slice = [&](unsigned slice) {
+            std::unordered_map<int64_t, char> seen;
+            const int64_t to_lo = nterms * slice / n_enum_thr, to_hi = nterms * (slice + 1) / n_enum_thr;
+            for (int64_t to = to_lo; to < to_hi; to++) {
+                seen.clear();
+                int64_t need = 0;
+                for (int64_t i = term_task_begin[to]; i < term_task_begin[to + 1]; i++) {
+                    const Task& k = tasks[i];
+                    if (k.r_off < 0) continue;
+                    if (seen.emplace(xkey(k.r_off, k.r_trans, k.in_blk, nblk), 1).second) need += x_elems(k);
+                }
+                slice_max[slice] = std::max(slice_max[slice], need);
             }
-            max_term = std::max(max_term, need);
-        }
+        };
+        std::vector<std::thread> pool;
+        for (unsigned t = 1; t < n_enum_thr; t++) pool.emplace_back(max_slice, t);
+        max_slice(0);
+        for (auto& th : pool) th.join();
+        const int64_t max_term = *std::max_element(slice_max.begin(), slice_max.end());
         ws_elems = std::max<int64_t>(std::max(ws_elems, max_term), 2);
     }
     std::vector<int64_t> chunk_begin;   // term_ord of the first term of each chunk
