@@ -133,8 +133,8 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *                      2 = TMA: one cp.async.bulk.tensor.2d per operand and pipeline stage through per-matrix
  *                      tensor maps the plan builds (the TMA unit zero-fills ragged tails)
  *   split_waves        split-K granularity of stage 2: a sigma block's K-loop is cut into parts no longer than
- *                      1/split_waves of the chunk's ideally balanced run time (0 = default 200)
- *   min_split_stages   ... but never shorter than this many GEMM_BK-wide pipeline stages (0 = default 24)
+ *                      1/split_waves of the chunk's ideally balanced run time (0 = default 100)
+ *   min_split_stages   ... but never shorter than this many GEMM_BK-wide pipeline stages (0 = default 96)
  *   max_merged_cols    widest N-merged stage-1 GEMM in columns (0 = default 4096)
  *   cost_order_only    1 = launch tiles in pure cost order; 0 (default) = inside a cost bucket, stage-2 tiles
  *                      follow (L sector of the sigma block, split-K part) so that they share L blocks in L2

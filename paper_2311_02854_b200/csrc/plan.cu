@@ -103,8 +103,10 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     PlanPolicy p;
     p.workspace_bytes = (o && o->workspace_bytes > 0) ? o->workspace_bytes : (int64_t(8) << 30);
     p.copy_mode = (o && (o->copy_mode == COPY_LDGSTS || o->copy_mode == COPY_TMA)) ? o->copy_mode : COPY_TMA;
-    p.split_waves = (o && o->split_waves > 0) ? o->split_waves : 200.0;
-    p.min_split_stages = (o && o->min_split_stages > 0) ? (double)o->min_split_stages : 768.0 / GEMM_BK;   // K = 768 per part at least
+    // split-K defaults re-measured on the final round-2 kernel (profiles/r2_summary.md section 6): 100 waves, parts of at least
+    // K = 3072 (96 stages): cfg2 -3.7 %, cfg3 -1.0 %, cfg4 -0.5 %, cfg5 -0.4 % against the 200 waves / K = 768 of round 1
+    p.split_waves = (o && o->split_waves > 0) ? o->split_waves : 100.0;
+    p.min_split_stages = (o && o->min_split_stages > 0) ? (double)o->min_split_stages : 3072.0 / GEMM_BK;
     p.max_merged_cols = (o && o->max_merged_cols >= 64) ? (int64_t)(o->max_merged_cols & ~1) : int64_t(4096);
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
