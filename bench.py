@@ -32,8 +32,8 @@ if ROOT not in sys.path:
 METRIC = "fp64_tflops_per_hpsi"
 # dram__bytes_read.sum + dram__bytes_write.sum of all GEMM launches of one H psi, from a committed ncu launch list
 # (NOT measured by this run): config -> (bytes, source)
-NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (1.684e12, "profiles/r2_cfg5_launches.csv (round 2, final kernel; 42 GEMM launches of the second dmrg_sigma call)"),
-                           "cfg4": (2.024e11, "profiles/r2_cfg4_split_small_launches.csv (round 2, final kernel; 12 GEMM launches of the second dmrg_sigma call)")}
+NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (2.006e12, "profiles/r2_cfg5_launches.csv (round 2, final kernel; 42 GEMM launches of the second dmrg_sigma call)"),
+                           "cfg4": (2.294e11, "profiles/r2_cfg4_split_small_launches.csv (round 2, final kernel; 12 GEMM launches of the second dmrg_sigma call)")}
 UNIT = "TFLOP/s"
 
 
