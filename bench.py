@@ -44,6 +44,9 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="cfg5", help="cfg1..cfg5 of BASELINE.json (default: the headline K=73 D=3000); so2 / so3: the spin-orbit "
                                                      "variants (complex FP64, N only; SURVEY section 8(f) NEXT-4) of cfg2 / cfg3, --sigma-only only")
+    ap.add_argument("--bond-dim", type=int, default=0, metavar="D",
+                    help="override the bond dimension of a direct-fill config (cfg3-5; footprint experiments, e.g. the largest D that "
+                         "fits one GPU: DESIGN.md section 5); the workload name says so")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="X workspace (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -261,7 +264,7 @@ def main():
                        "tflops_full_size_steps": sum(r["flops"] for r in big) / max(1e-9, sum(r["device_ms"] for r in big)) * 1e-9,
                        "seconds_total": pr.seconds["total"], "seconds_chains": pr.seconds["chains"]}
     else:
-        pr = make_config(args.config)
+        pr = make_config(args.config, D=args.bond_dim) if args.bond_dim > 0 else make_config(args.config)
         t_gen = time.perf_counter() - t0
         t0 = time.perf_counter()
         ops = g.OpsStore(pr.secL, pr.secR, pr.ops, pr.blocks, pr.values, pr.lin_ptr, pr.lin_op, pr.lin_coef)
