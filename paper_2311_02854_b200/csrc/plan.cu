@@ -95,6 +95,7 @@ struct PlanPolicy {   // dmrg_plan_options with the defaults filled in
     bool tile_order;
     int split_small;
     bool release_r_store;
+    bool release_staged;   // release_r_store == 2: always park the R side on the host while the pack is filled
     int shard_rank, shard_count;
     int tile_run_stages;   // stage 1: a CTA computes as many consecutive M tiles as it takes to reach this many pipeline stages (<= 8 tiles)
 };
@@ -111,6 +112,7 @@ static PlanPolicy make_policy(const dmrg_plan_options* o) {
     p.tile_order = !(o && o->cost_order_only);
     p.split_small = (o && o->split_small > 0) ? o->split_small : 0;
     p.release_r_store = o && o->release_r_store;
+    p.release_staged = o && o->release_r_store == 2;
     p.tile_run_stages = (o && o->tile_run_stages > 0) ? o->tile_run_stages : 32;
     p.shard_count = (o && o->shard_count > 1) ? o->shard_count : 1;
     p.shard_rank = (o && o->shard_count > 1) ? o->shard_rank : 0;
@@ -975,6 +977,29 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
     };
     DMRG_CUDA(cudaMalloc(&P->d_psi_pad, sizeof(double) * (size_t)P->psi_pad_elems));
     if (Z) DMRG_CUDA(cudaMalloc(&P->d_sigz, sizeof(double) * (size_t)std::max<int64_t>(2 * P->psi_size, 2)));
+    // release_r_store near the memory limit: the R-side originals and their packed copy do not fit side by side.  The R side
+    // is then parked on the HOST, its device allocation freed before the pack is allocated, and the pack filled from
+    // staging windows (below).  Chosen when the free memory does not cover pack + X workspace + tensor maps, or forced (2).
+    std::vector<double> host_r;
+    int64_t host_r_rel0 = 0;   // offset of the R-side allocation in the store's address space (doubles)
+    if (kReleaseR && S->side_alloc[1]) {
+        size_t free_b = 0, total_b = 0;
+        DMRG_CUDA(cudaMemGetInfo(&free_b, &total_b));
+        const double need = 8.0 * (double)pack_top + 8.0 * (double)P->xws_elems + 8.0 * (double)P->psi_pad_elems + 128.0 * (double)maps.descs.size() +
+                            64.0 * (double)tiles.size() + 64.0 * (double)segs.size() + 2e9;
+        if (pol.release_staged || need > (double)free_b) {
+            dmrg_ops* Sm = const_cast<dmrg_ops*>(S);
+            host_r_rel0 = (int64_t)(Sm->side_alloc[1] - Sm->d_values);
+            host_r.resize(Sm->side_bytes[1] / sizeof(double));
+            DMRG_CUDA(cudaMemcpy(host_r.data(), Sm->side_alloc[1], Sm->side_bytes[1], cudaMemcpyDeviceToHost));
+            cudaFree(Sm->side_alloc[1]);
+            Sm->owned.erase(std::remove(Sm->owned.begin(), Sm->owned.end(), Sm->side_alloc[1]), Sm->owned.end());
+            Sm->device_bytes -= (int64_t)Sm->side_bytes[1];
+            Sm->side_alloc[1] = nullptr;
+            Sm->side_bytes[1] = 0;
+            Sm->r_released = true;
+        }
+    }
     DMRG_CUDA(cudaMalloc(&P->d_pack, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     DMRG_CUDA(cudaMemset(P->d_pack, 0, sizeof(double) * (size_t)std::max<int64_t>(pack_top, 2)));
     {   // the GEMM kernel addresses the packed store relative to the operator store (one flat device address space)
@@ -1003,7 +1028,39 @@ static int plan_build(dmrg_plan* P, const dmrg_term* terms, const double* coef_i
         if ((rc = encode_tensor_maps(maps.descs, base, tm))) return rc;
         if ((rc = up((void**)&P->d_tmaps, tm.data(), tm.size() * sizeof(TensorMap)))) return rc;
     }
-    if (!packs.empty()) {
+    if (!packs.empty() && !host_r.empty()) {
+        // staged fill: packs in the order of their source blocks, windows of the parked R side copied back one at a time
+        std::sort(packs.begin(), packs.end(), [](const PackDesc& a, const PackDesc& b) { return a.src < b.src; });
+        auto extent = [](const PackDesc& d) { return (int64_t)(d.trans ? d.dRi : d.dRo) * d.src_ld; };
+        int64_t win = int64_t(1) << 29;   // 4 GiB of doubles
+        for (const PackDesc& d : packs) win = std::max(win, extent(d));
+        win = std::min<int64_t>(win, (int64_t)host_r.size());
+        double* d_stage = nullptr;
+        PackDesc* d_packs = nullptr;
+        DMRG_CUDA(cudaMalloc(&d_stage, sizeof(double) * (size_t)std::max<int64_t>(win, 2)));
+        DMRG_CUDA(cudaMalloc(&d_packs, packs.size() * sizeof(PackDesc)));
+        DMRG_CUDA(cudaMemcpy(d_packs, packs.data(), packs.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));
+        for (size_t i0 = 0; i0 < packs.size();) {
+            const int64_t w0 = packs[i0].src;
+            size_t i1 = i0;
+            int64_t w1 = w0;
+            while (i1 < packs.size() && packs[i1].src + extent(packs[i1]) - w0 <= win) { w1 = std::max(w1, packs[i1].src + extent(packs[i1])); i1++; }
+            DMRG_REQUIRE(i1 > i0 && w0 >= host_r_rel0 && w1 - host_r_rel0 <= (int64_t)host_r.size(), "dmrg_plan_create: packed-store source outside the R side of the store");
+            DMRG_CUDA(cudaMemcpy(d_stage, host_r.data() + (w0 - host_r_rel0), sizeof(double) * (size_t)(w1 - w0), cudaMemcpyHostToDevice));
+            const double* ops_win = d_stage - w0;   // address arithmetic only: ops_win[src + x] = d_stage[src - w0 + x]
+            for (size_t y0 = i0; y0 < i1; y0 += 32768) {
+                const unsigned ny = (unsigned)std::min<size_t>(32768, i1 - y0);
+                if (Z) pack_r_z_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, ops_win, P->d_pack);
+                else pack_r_kernel<<<dim3(4, ny), 256>>>(d_packs + y0, ops_win, P->d_pack);
+            }
+            DMRG_CUDA(cudaGetLastError());
+            DMRG_CUDA(cudaDeviceSynchronize());
+            i0 = i1;
+        }
+        cudaFree(d_packs);
+        cudaFree(d_stage);
+        std::vector<double>().swap(host_r);
+    } else if (!packs.empty()) {
         PackDesc* d_packs = nullptr;
         DMRG_CUDA(cudaMalloc(&d_packs, packs.size() * sizeof(PackDesc)));
         DMRG_CUDA(cudaMemcpy(d_packs, packs.data(), packs.size() * sizeof(PackDesc), cudaMemcpyHostToDevice));

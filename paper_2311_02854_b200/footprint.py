@@ -42,10 +42,11 @@ def footprint(K, nL, N, D, ws_gib, max_space=30, banded=True):
            "plan_gb": st["plan_device_bytes"] / 1e9, "x_workspace_gb": 8 * st["xws_elems"] / 1e9, "chunks": int(st["chunks"]),
            "davidson_gb": (2 * max_space + 3) * 8 * plan.psi_size / 1e9}
     out["total_gb"] = out["store_gb"] + out["plan_gb"] + out["davidson_gb"]
-    # release_r_store: the steady state drops the R-side originals, but while the plan is created the store and the plan's
-    # packed copy exist side by side (measured: D = 4500 fails in dmrg_plan_create although its steady state would fit)
+    # release_r_store: the steady state drops the R-side originals.  Where the originals and the plan's packed copy do not
+    # fit side by side while the plan is created, dmrg_plan_create parks the R side in host memory first (needs that
+    # much host RAM; measured: D = 4500 runs that way), so the steady state is what has to fit.
     out["total_release_r_gb"] = out["total_gb"] - min(out["store_r_side_gb_upper"], out["store_gb"])
-    out["peak_release_r_gb"] = max(out["total_release_r_gb"], out["store_gb"] + out["plan_gb"])
+    out["host_parking_gb"] = min(out["store_r_side_gb_upper"], out["store_gb"]) if out["store_gb"] + out["plan_gb"] > (HBM_BYTES - RESERVE) / 1e9 else 0.0
     plan.destroy()
     ops.free()
     return out
@@ -66,7 +67,7 @@ def main():
         r = footprint(a.K, a.nL, a.N, D, a.workspace_gib)
         r["plan_seconds"] = time.perf_counter() - t0
         r["fits"] = r["total_gb"] <= cap
-        r["fits_release_r"] = r["peak_release_r_gb"] <= cap
+        r["fits_release_r"] = r["total_release_r_gb"] <= cap
         if r["fits"]:
             best["keep"] = D
         if r["fits_release_r"]:

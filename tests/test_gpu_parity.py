@@ -293,10 +293,12 @@ def test_sigma_can_be_captured_in_a_cuda_graph():
     ops.free()
 
 
-def test_release_r_store_frees_the_r_side_and_changes_nothing():
+@pytest.mark.parametrize("mode", [1, 2])
+def test_release_r_store_frees_the_r_side_and_changes_nothing(mode):
     """dmrg_plan_options.release_r_store: once stage 1 and the diagonal read the plan's packed copy of the R blocks, the
     store's R-side allocation is freed.  sigma is bitwise the same, the diagonal still matches the oracle, the store
-    shrinks, and it refuses to serve a second plan."""
+    shrinks, and it refuses to serve a second plan.  Mode 2 forces the path taken near the memory limit: the R side is
+    parked on the host and freed BEFORE the pack is allocated, the pack filled from staging windows."""
     g = _gpu()
     from dmrg_workload.problem import make_direct_problem
     pr = make_direct_problem(16, 7, 16, 0, D=200, seed=3)
@@ -305,7 +307,7 @@ def test_release_r_store_frees_the_r_side_and_changes_nothing():
     ref = _sigma_gpu(plan, psi)
     plan.destroy()
     before = ops.device_bytes
-    plan2 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, release_r_store=1)
+    plan2 = g.Plan(ops, pr.term_coef, pr.term_idx, pr.site_ops, pr.site_parity, pr.N_tot, pr.twoSz_tot, release_r_store=mode)
     assert ops.device_bytes < 0.75 * before
     assert np.array_equal(_sigma_gpu(plan2, psi), ref)
     d = torch.empty(pr.psi_size, dtype=torch.float64, device="cuda")
