@@ -144,7 +144,9 @@ int64_t dmrg_ops_device_bytes(const dmrg_ops* ops);   /* HBM held by the store *
  *                      one; the store can serve no further dmrg_plan_create); 0 = keep (default).  When the free
  *                      device memory does not hold the originals and the pack side by side, the R side is parked in
  *                      HOST memory (its size, pageable) and freed before the pack is allocated, and the pack is filled
- *                      from 4 GiB staging windows; 2 = always take that path
+ *                      from 4 GiB staging windows; 2 = always take that path.  (On that path the R side is given up
+ *                      before the rest of the plan is allocated: if dmrg_plan_create then fails, e.g. DMRG_ENOMEM, the
+ *                      store is left without its R side and must be loaded again.)
  *   tile_run_stages    stage 1: a CTA computes consecutive M tiles of one GEMM back to back (stage ring running on across
  *                      them) until it has this many pipeline stages of work, at most 8 tiles (0 = default 32; 1 = one
  *                      tile per CTA).  Same tiles and the same per-element summation order either way.
