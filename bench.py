@@ -33,7 +33,9 @@ METRIC = "fp64_tflops_per_hpsi"
 # dram__bytes_read.sum + dram__bytes_write.sum of all GEMM launches of one H psi, from a committed ncu launch list
 # (NOT measured by this run): config -> (bytes, source)
 NCU_DRAM_BYTES_PER_HPSI = {"cfg5": (2.006e12, "profiles/r2_cfg5_launches.csv (round 2, final kernel; 42 GEMM launches of the second dmrg_sigma call)"),
-                           "cfg4": (2.294e11, "profiles/r2_cfg4_split_small_launches.csv (round 2, final kernel; 12 GEMM launches of the second dmrg_sigma call)")}
+                           "cfg4": (2.294e11, "profiles/r2_cfg4_split_small_launches.csv (round 2, final kernel; 12 GEMM launches of the second dmrg_sigma call)"),
+                           "cfg3": (1.641e11, "profiles/r2_cfg3_launches.csv (round 2, final kernel; 4 GEMM launches of the second dmrg_sigma call)"),
+                           "cfg2": (9.88e9, "profiles/r2_cfg2_launches.csv (round 2, final kernel; 2 GEMM launches of the second dmrg_sigma call)")}
 UNIT = "TFLOP/s"
 
 
